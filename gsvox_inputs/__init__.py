@@ -1,0 +1,193 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs (and small test variants).
+
+This module is the ONLY code shared by the fp64 oracle (oracle/) and the CUDA path
+(paper_2503_22139_b200/).  It holds none of the voxelizer's arithmetic: it only draws
+positions, scales, quaternions, weights and upstream gradients with numpy's PCG64
+(`numpy.random.default_rng`), in fp64, and casts to fp32 ONCE; both sides are handed
+the same fp32 arrays.  The recipe is SURVEY.md section 8(d) "Concrete synthetic inputs",
+restated in DESIGN.md; these inputs stand in for the paper's XCAT / MDACC / SPARE
+volumes, which are not available — only shapes are borrowed.
+
+Conventions common to all configs: origin (0,0,0), spacing (1,1,1) (voxel units),
+"uniform in the grid" = U(-0.5, n_k - 0.5) per axis, unit quaternions = normalised
+N(0, I4) in (w,x,y,z) order, "log-uniform a-b" = exp(U(ln a, ln b)), upstream gradient
+N(0,1) in the output layout [C, nz, ny, nx], seed = config number - 1.
+"""
+from dataclasses import dataclass, field
+
+import numpy as np
+
+
+@dataclass
+class Case:
+    name: str
+    dims: tuple                 # (nx, ny, nz)
+    channels: int
+    pos: np.ndarray             # [n,3] fp32
+    scale: np.ndarray           # [n,3] fp32
+    quat: np.ndarray            # [n,4] fp32 (w,x,y,z)
+    weight: np.ndarray          # [n,C] fp32
+    origin: tuple = (0.0, 0.0, 0.0)
+    spacing: tuple = (1.0, 1.0, 1.0)
+    seed: object = 0
+    _grad_seed: object = field(default=None, repr=False)
+
+    @property
+    def n(self):
+        return int(self.pos.shape[0])
+
+    @property
+    def grid(self):
+        return (np.asarray(self.origin, np.float32), np.asarray(self.spacing, np.float32),
+                np.asarray(self.dims, np.int32))
+
+    @property
+    def voxels(self):
+        return int(self.dims[0]) * int(self.dims[1]) * int(self.dims[2])
+
+    def grad_out(self):
+        """Upstream gradient N(0,1), fp32, [C, nz, ny, nx]; drawn on demand (it is large)."""
+        rng = np.random.default_rng(self._grad_seed)
+        nx, ny, nz = self.dims
+        return rng.standard_normal((self.channels, nz, ny, nx), dtype=np.float32)
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _uniform_in_grid(rng, n, dims):
+    d = np.asarray(dims, dtype=np.float64)
+    return rng.uniform(-0.5, d - 0.5, size=(n, 3))
+
+
+def _log_uniform(rng, a, b, size):
+    return np.exp(rng.uniform(np.log(a), np.log(b), size=size))
+
+
+def _unit_quats(rng, n):
+    q = rng.standard_normal((n, 4))
+    return q / np.linalg.norm(q, axis=1, keepdims=True)
+
+
+def _case(name, dims, ch, pos, scale, quat, weight, seed, **kw):
+    gs = [int(x) for x in np.atleast_1d(seed)] + [0x67726164]   # separate stream for grad_out
+    return Case(name, tuple(int(d) for d in dims), ch, _f32(pos), _f32(scale), _f32(quat),
+                _f32(weight).reshape(len(pos), ch), seed=seed, _grad_seed=gs, **kw)
+
+
+def config1(n=2000, dims=(64, 64, 64), seed=0):
+    """Tiny voxelizer: 64^3, 2,000 Gaussians, scales logU(0.5,3) per axis, w U(0,1)."""
+    rng = np.random.default_rng(seed)
+    pos = _uniform_in_grid(rng, n, dims)
+    scale = _log_uniform(rng, 0.5, 3.0, (n, 3))
+    quat = _unit_quats(rng, n)
+    w = rng.uniform(0.0, 1.0, size=(n, 1))
+    return _case("config1_tiny", dims, 1, pos, scale, quat, w, seed)
+
+
+def config2(n=100_000, dims=(256, 256, 128), seed=1):
+    """Reference-frame CBCT: centres uniform in volume inside a torso-like ellipsoid,
+    scales logU(1,4), 3-tissue attenuation mix {0.02,0.2,0.5} with p=(0.6,0.3,0.1) + N(0,0.01)."""
+    rng = np.random.default_rng(seed)
+    d = np.asarray(dims, dtype=np.float64)
+    centre = (d - 1.0) / 2.0
+    semi = np.array([0.45, 0.35, 0.48]) * d
+    pts = np.empty((0, 3))
+    while pts.shape[0] < n:                       # rejection sampling in the unit ball
+        u = rng.uniform(-1.0, 1.0, size=(2 * n, 3))
+        pts = np.concatenate([pts, u[(u * u).sum(1) <= 1.0]])
+    pos = centre + semi * pts[:n]
+    scale = _log_uniform(rng, 1.0, 4.0, (n, 3))
+    quat = _unit_quats(rng, n)
+    tissue = rng.choice(np.array([0.02, 0.2, 0.5]), size=n, p=[0.6, 0.3, 0.1])
+    w = (tissue + rng.normal(0.0, 0.01, size=n)).reshape(n, 1)
+    return _case("config2_cbct", dims, 1, pos, scale, quat, w, seed)
+
+
+_LEVELS = {1: (1_000, 16.0, 32.0), 2: (8_000, 6.0, 12.0), 3: (64_000, 2.0, 5.0)}
+
+
+def config3(level, dims=(128, 128, 64), seed=2, n=None, channels=9):
+    """Motion-basis DVF field, one level (1, 2 or 3): 9-channel features N(0,1),
+    N = 1k / 8k / 64k, scales logU(16,32) / (6,12) / (2,5)."""
+    n0, a, b = _LEVELS[level]
+    n = n0 if n is None else n
+    rng = np.random.default_rng([seed, level])
+    pos = _uniform_in_grid(rng, n, dims)
+    scale = _log_uniform(rng, a, b, (n, 3))
+    quat = _unit_quats(rng, n)
+    w = rng.standard_normal((n, channels))
+    return _case("config3_dvf_level%d" % level, dims, channels, pos, scale, quat, w, [seed, level])
+
+
+def config4(n=500_000, dims=(256, 256, 256), seed=3):
+    """Training step at scale: 70% isotropic s0~logU(0.7,5); 30% anisotropic, three
+    independent logU(0.7,5) draws redrawn until max/min <= 6; w U(0,0.5)."""
+    rng = np.random.default_rng(seed)
+    pos = _uniform_in_grid(rng, n, dims)
+    iso = rng.uniform(size=n) < 0.7
+    s0 = _log_uniform(rng, 0.7, 5.0, n)
+    scale = np.repeat(s0[:, None], 3, axis=1)
+    aniso = np.flatnonzero(~iso)
+    s = _log_uniform(rng, 0.7, 5.0, (aniso.size, 3))
+    bad = np.flatnonzero(s.max(1) / s.min(1) > 6.0)
+    while bad.size:
+        s[bad] = _log_uniform(rng, 0.7, 5.0, (bad.size, 3))
+        bad = bad[s[bad].max(1) / s[bad].min(1) > 6.0]
+    scale[aniso] = s
+    quat = _unit_quats(rng, n)
+    w = rng.uniform(0.0, 0.5, size=(n, 1))
+    return _case("config4_train", dims, 1, pos, scale, quat, w, seed)
+
+
+def config5(n=2_000_000, dims=(512, 512, 256), seed=4):
+    """Load-imbalance stress: 95% small Gaussians (s logU(0.5,2)) in 16 Gaussian blobs
+    (centres in the central 70% of each axis, blob sigma U(8,24), positions not clipped),
+    5% needles s = (U(10,20), 0.5, 0.5) uniform in the grid; w U(0,1)."""
+    rng = np.random.default_rng(seed)
+    d = np.asarray(dims, dtype=np.float64)
+    n_needle = int(round(0.05 * n))
+    n_blob = n - n_needle
+    blob_c = rng.uniform(0.15 * d - 0.5, 0.85 * d - 0.5, size=(16, 3))
+    blob_sigma = rng.uniform(8.0, 24.0, size=16)
+    which = rng.integers(0, 16, size=n_blob)
+    pos_b = blob_c[which] + blob_sigma[which, None] * rng.standard_normal((n_blob, 3))
+    scale_b = _log_uniform(rng, 0.5, 2.0, (n_blob, 3))
+    pos_n = _uniform_in_grid(rng, n_needle, dims)
+    scale_n = np.stack([rng.uniform(10.0, 20.0, size=n_needle),
+                        np.full(n_needle, 0.5), np.full(n_needle, 0.5)], axis=1)
+    pos = np.concatenate([pos_b, pos_n])
+    scale = np.concatenate([scale_b, scale_n])
+    perm = rng.permutation(n)                      # interleave needles with blob members
+    pos, scale = pos[perm], scale[perm]
+    quat = _unit_quats(rng, n)
+    w = rng.uniform(0.0, 1.0, size=(n, 1))
+    return _case("config5_stress", dims, 1, pos, scale, quat, w, seed)
+
+
+def subvolume_case(n=600, dims=(37, 29, 21), channels=3, seed=11,
+                   origin=(-13.5, 4.25, 100.0), spacing=(2.0, 1.5, 0.75)):
+    """A ragged, anisotropic-spacing sub-grid with a non-zero origin and unnormalised
+    quaternions, most Gaussians partly or wholly outside (the 32^3 TV sub-volume query of
+    PAPER.md:128-130 and the coarse Stage-2 grid of PAPER.md:136 exercise these arguments)."""
+    rng = np.random.default_rng(seed)
+    d = np.asarray(dims, dtype=np.float64)
+    o = np.asarray(origin, dtype=np.float64)
+    h = np.asarray(spacing, dtype=np.float64)
+    ext = d * h
+    pos = o + rng.uniform(-0.4, 1.4, size=(n, 3)) * ext
+    scale = _log_uniform(rng, 0.6, 6.0, (n, 3))
+    quat = rng.standard_normal((n, 4)) * rng.uniform(0.2, 5.0, size=(n, 1))
+    w = rng.standard_normal((n, channels))
+    return _case("subvolume", dims, channels, pos, scale, quat, w, seed,
+                 origin=tuple(origin), spacing=tuple(spacing))
+
+
+FULL = {
+    "config1": lambda: [config1()],
+    "config2": lambda: [config2()],
+    "config3": lambda: [config3(1), config3(2), config3(3)],
+    "config4": lambda: [config4()],
+    "config5": lambda: [config5()],
+}

@@ -1,0 +1,152 @@
+"""ctypes front end of the fp64 CPU oracle (oracle/gsvox_oracle.c).
+
+TEST INFRASTRUCTURE ONLY.  Importers allowed: tests/, __graft_entry__.smoke(),
+bench.py's cpu_baseline and --impl reference legs.  The product package
+(paper_2503_22139_b200) never imports this module and this module never imports it.
+
+All functions take numpy arrays (fp32 inputs, as handed to the CUDA path) and
+return fp64 numpy arrays.  `grid` is (origin[3], spacing[3], dims[3]) with
+dims = (nx, ny, nz); volumes are laid out [C, nz, ny, nx] (reading A7).
+"""
+import ctypes as C
+
+import numpy as np
+
+from .build import build as _build
+
+KAPPA = 3.0          # the product's fixed cutoff (north_star: "3-sigma"); a parameter here
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build())
+        fp, dp, ip, lp, bp = (C.POINTER(C.c_float), C.POINTER(C.c_double),
+                              C.POINTER(C.c_int32), C.POINTER(C.c_int64), C.POINTER(C.c_uint8))
+        L.gsvox_oracle_threads.restype = C.c_int
+        L.gsvox_oracle_geometry.argtypes = [fp, fp, fp, C.c_int64, fp, fp, ip, C.c_double,
+                                            dp, dp, ip, bp]
+        L.gsvox_oracle_forward.argtypes = [fp, fp, fp, fp, C.c_int64, C.c_int32, fp, fp, ip,
+                                           C.c_double, dp, lp]
+        L.gsvox_oracle_forward_at.argtypes = [fp, fp, fp, fp, C.c_int64, C.c_int32, fp, fp, ip,
+                                              C.c_double, lp, C.c_int64, dp]
+        L.gsvox_oracle_backward.argtypes = [fp, fp, fp, fp, C.c_int64, C.c_int32, fp, fp, ip,
+                                            C.c_double, fp, dp, dp, dp, dp]
+        L.gsvox_oracle_backward_for.argtypes = [fp, fp, fp, fp, C.c_int64, C.c_int32, fp, fp, ip,
+                                                C.c_double, fp, lp, C.c_int64, dp, dp, dp, dp]
+        _lib = L
+    return _lib
+
+
+def threads() -> int:
+    return int(lib().gsvox_oracle_threads())
+
+
+def _f32(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    if shape is not None:
+        a = a.reshape(shape)
+    return a
+
+
+def _p(a, ct):
+    return a.ctypes.data_as(C.POINTER(ct))
+
+
+def _grid(grid):
+    origin, spacing, dims = grid
+    o = _f32(origin, (3,))
+    h = _f32(spacing, (3,))
+    d = np.ascontiguousarray(dims, dtype=np.int32).reshape(3)
+    return o, h, d
+
+
+def _check(rc):
+    if rc != 0:
+        raise RuntimeError("gsvox oracle error %d" % rc)
+
+
+def _params(pos, scale, quat):
+    pos, scale, quat = _f32(pos), _f32(scale), _f32(quat)
+    n = pos.shape[0] if pos.ndim == 2 else pos.size // 3
+    return pos.reshape(n, 3), scale.reshape(n, 3), quat.reshape(n, 4), n
+
+
+def geometry(pos, scale, quat, grid, kappa=KAPPA):
+    """-> dict(M [n,6] xx,xy,xz,yy,yz,zz; R [n,3,3]; box [n,6] lo xyz, hi xyz; flags [n])."""
+    pos, scale, quat, n = _params(pos, scale, quat)
+    o, h, d = _grid(grid)
+    M = np.zeros((n, 6)); R = np.zeros((n, 9))
+    box = np.zeros((n, 6), dtype=np.int32); flags = np.zeros(n, dtype=np.uint8)
+    _check(lib().gsvox_oracle_geometry(_p(pos, C.c_float), _p(scale, C.c_float), _p(quat, C.c_float),
+                                       n, _p(o, C.c_float), _p(h, C.c_float), _p(d, C.c_int32),
+                                       float(kappa), _p(M, C.c_double), _p(R, C.c_double),
+                                       _p(box, C.c_int32), _p(flags, C.c_uint8)))
+    return {"M": M, "R": R.reshape(n, 3, 3), "box": box, "flags": flags}
+
+
+def forward(pos, scale, quat, weight, grid, kappa=KAPPA, return_pairs=False):
+    """-> out [C, nz, ny, nx] fp64 (and P_def, the number of pairs inside the cutoff)."""
+    pos, scale, quat, n = _params(pos, scale, quat)
+    weight = _f32(weight).reshape(n, -1) if n else _f32(weight).reshape(0, max(1, np.shape(weight)[-1]))
+    ch = weight.shape[1]
+    o, h, d = _grid(grid)
+    out = np.empty((ch, int(d[2]), int(d[1]), int(d[0])))
+    pairs = C.c_int64(0)
+    _check(lib().gsvox_oracle_forward(_p(pos, C.c_float), _p(scale, C.c_float), _p(quat, C.c_float),
+                                      _p(weight, C.c_float), n, ch, _p(o, C.c_float),
+                                      _p(h, C.c_float), _p(d, C.c_int32), float(kappa),
+                                      _p(out, C.c_double), C.byref(pairs)))
+    return (out, int(pairs.value)) if return_pairs else out
+
+
+def forward_at(pos, scale, quat, weight, grid, voxels, kappa=KAPPA):
+    """Brute force at linear voxel indices v = (k*ny + j)*nx + i  -> [C, m] fp64."""
+    pos, scale, quat, n = _params(pos, scale, quat)
+    weight = _f32(weight).reshape(n, -1)
+    ch = weight.shape[1]
+    o, h, d = _grid(grid)
+    vox = np.ascontiguousarray(voxels, dtype=np.int64).reshape(-1)
+    out = np.zeros((ch, vox.size))
+    _check(lib().gsvox_oracle_forward_at(_p(pos, C.c_float), _p(scale, C.c_float), _p(quat, C.c_float),
+                                         _p(weight, C.c_float), n, ch, _p(o, C.c_float),
+                                         _p(h, C.c_float), _p(d, C.c_int32), float(kappa),
+                                         _p(vox, C.c_int64), vox.size, _p(out, C.c_double)))
+    return out
+
+
+def backward(pos, scale, quat, weight, grid, grad_out, kappa=KAPPA):
+    """-> (dL/dw [n,C], dL/dp [n,3], dL/ds [n,3], dL/dq [n,4]) fp64."""
+    pos, scale, quat, n = _params(pos, scale, quat)
+    weight = _f32(weight).reshape(n, -1)
+    ch = weight.shape[1]
+    o, h, d = _grid(grid)
+    g = _f32(grad_out).reshape(ch, int(d[2]), int(d[1]), int(d[0]))
+    gw = np.zeros((n, ch)); gp = np.zeros((n, 3)); gs = np.zeros((n, 3)); gq = np.zeros((n, 4))
+    _check(lib().gsvox_oracle_backward(_p(pos, C.c_float), _p(scale, C.c_float), _p(quat, C.c_float),
+                                       _p(weight, C.c_float), n, ch, _p(o, C.c_float),
+                                       _p(h, C.c_float), _p(d, C.c_int32), float(kappa),
+                                       _p(g, C.c_float), _p(gw, C.c_double), _p(gp, C.c_double),
+                                       _p(gs, C.c_double), _p(gq, C.c_double)))
+    return gw, gp, gs, gq
+
+
+def backward_for(pos, scale, quat, weight, grid, grad_out, ids, kappa=KAPPA):
+    """Gradients of the listed Gaussians only -> (gw [m,C], gp [m,3], gs [m,3], gq [m,4])."""
+    pos, scale, quat, n = _params(pos, scale, quat)
+    weight = _f32(weight).reshape(n, -1)
+    ch = weight.shape[1]
+    o, h, d = _grid(grid)
+    g = _f32(grad_out).reshape(ch, int(d[2]), int(d[1]), int(d[0]))
+    ids = np.ascontiguousarray(ids, dtype=np.int64).reshape(-1)
+    m = ids.size
+    gw = np.zeros((m, ch)); gp = np.zeros((m, 3)); gs = np.zeros((m, 3)); gq = np.zeros((m, 4))
+    _check(lib().gsvox_oracle_backward_for(_p(pos, C.c_float), _p(scale, C.c_float),
+                                           _p(quat, C.c_float), _p(weight, C.c_float), n, ch,
+                                           _p(o, C.c_float), _p(h, C.c_float), _p(d, C.c_int32),
+                                           float(kappa), _p(g, C.c_float), _p(ids, C.c_int64), m,
+                                           _p(gw, C.c_double), _p(gp, C.c_double),
+                                           _p(gs, C.c_double), _p(gq, C.c_double)))
+    return gw, gp, gs, gq
