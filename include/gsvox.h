@@ -1,0 +1,156 @@
+/*
+ * gsvox.h — C ABI of the B200-native differentiable 3D Gaussian voxelizer.
+ *
+ * The operation (PAPER.md = /root/reference/PAPER.md):
+ *   Eq. 4   G_i(x) = w_i exp(-1/2 (x-p_i)^T Sigma_i^-1 (x-p_i))
+ *   Eq. 5   out(x) = sum_i G_i(x)                     ("voxelization")
+ *   PAPER.md:104          differentiable wrt every Gaussian parameter
+ *   PAPER.md:106-108      signed, multi-channel values (motion-basis components)
+ *   PAPER.md:128-130,136  arbitrary sub-grids and resolutions (origin/spacing/dims)
+ * with Sigma_i = R(q_i) diag(s_i)^2 R(q_i)^T and each Gaussian cut off at the axis-aligned
+ * bounding box of its 3-sigma ellipsoid (BASELINE.json north_star; DESIGN.md readings
+ * A1-A16).  Backward treats that box as frozen.
+ *
+ * Conventions
+ *   - Every `const float*` / `float*` below is a DEVICE pointer unless the name ends in
+ *     `_host`.  The caller owns all buffers; the library never allocates or frees device
+ *     memory.  All device work is enqueued on `stream` (a cudaStream_t passed as void*);
+ *     gsvox_preprocess / gsvox_forward / gsvox_backward never synchronise with the host.
+ *   - Layouts: pos [n,3], scale [n,3], quat [n,4] = (w,x,y,z) (need not be normalised),
+ *     weight [n,C], volumes [C,nz,ny,nx] with x fastest, all fp32, densely packed.
+ *   - Voxel (i,j,k) has its CENTRE at origin + (i*hx, j*hy, k*hz).
+ *   - A Gaussian with a non-finite parameter, a scale <= 0 or a zero quaternion is
+ *     skipped: it contributes nothing and all its gradients are 0.
+ *   - Return value: GSVOX_OK (0) or a negative error code; gsvox_error_string() names it.
+ *     Conditions only the device can see (key capacity exceeded) set a flag in the plan:
+ *     forward/backward then write zeros and gsvox_plan_status() reports the overflow.
+ *   - A plan is bound to one workspace and one grid.  gsvox_preprocess() may be called
+ *     any number of times on it (every training step); forward/backward use the geometry
+ *     of the latest preprocess.  Distinct plans may be used from distinct threads/streams.
+ */
+#ifndef GSVOX_H
+#define GSVOX_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GSVOX_OK            0
+#define GSVOX_EINVAL       -1   /* null pointer, n < 0, dims < 1, spacing <= 0, C out of range */
+#define GSVOX_EWORKSPACE   -2   /* workspace too small or misaligned                          */
+#define GSVOX_ECUDA        -3   /* a CUDA runtime call or launch failed                       */
+#define GSVOX_ENOTREADY    -4   /* forward/backward before preprocess                         */
+#define GSVOX_ELIMIT       -5   /* size beyond the library limits below                       */
+
+#define GSVOX_MAX_CHANNELS  16          /* 1 <= C <= 16                                       */
+#define GSVOX_MAX_DIM       32760       /* per-axis voxel count                               */
+#define GSVOX_BRICK         8           /* bricks are 8x8x8 voxels                            */
+#define GSVOX_SIGMA_CUTOFF  3.0         /* fixed (north_star)                                 */
+
+typedef struct {
+    float   origin[3];   /* world position of the centre of voxel (0,0,0), order x,y,z      */
+    float   spacing[3];  /* world units per voxel along x,y,z, > 0                           */
+    int32_t dims[3];     /* nx, ny, nz                                                        */
+} gsvox_grid;
+
+typedef struct gsvox_plan gsvox_plan;   /* opaque host object; device state lives in the workspace */
+
+/* Size of the device workspace for up to n_max Gaussians, channels C <= max_channels and at most
+ * key_capacity (brick, Gaussian) keys.  A key is one Gaussian touching one 8^3 brick; if a
+ * preprocess needs more than key_capacity keys the plan overflows (see gsvox_plan_status).   */
+int gsvox_workspace_bytes(int64_t n_max, int32_t max_channels, const gsvox_grid* grid,
+                          int64_t key_capacity, size_t* bytes);
+
+/* Create a plan over caller-owned device memory `workspace` (256-byte aligned, at least
+ * gsvox_workspace_bytes() long).  No device work is enqueued.                                 */
+int gsvox_plan_create(int64_t n_max, int32_t max_channels, const gsvox_grid* grid,
+                      int64_t key_capacity, void* workspace, size_t workspace_bytes,
+                      gsvox_plan** plan);
+void gsvox_plan_destroy(gsvox_plan* plan);
+
+/* Steps a1+a2: per-Gaussian inverse covariance and voxel box (Eq. 4's Sigma^-1,
+ * reading A5 for the box), then brick binning: per-brick lists of the Gaussians whose box
+ * meets the brick.  n <= n_max.                                                              */
+int gsvox_preprocess(gsvox_plan* plan, const float* pos, const float* scale, const float* quat,
+                     int64_t n, void* stream);
+
+/* Step a3: out[c,k,j,i] = sum_i w_ic exp(-1/2 d^T Sigma_i^-1 d) over the Gaussians whose box
+ * holds voxel (i,j,k) (Eq. 5).  `out` is OVERWRITTEN, zeros where no Gaussian reaches.        */
+int gsvox_forward(gsvox_plan* plan, const float* weight, int32_t channels, float* out,
+                  void* stream);
+
+/* Steps a4+a5: given grad_out = dL/dout, write dL/dweight [n,C], dL/dpos [n,3],
+ * dL/dscale [n,3], dL/dquat [n,4] (wrt the unnormalised quaternion).  All four OVERWRITTEN.
+ * fp32 atomics make the last bits run-to-run dependent.                                       */
+int gsvox_backward(gsvox_plan* plan, const float* weight, int32_t channels,
+                   const float* grad_out, float* grad_weight, float* grad_pos,
+                   float* grad_scale, float* grad_quat, void* stream);
+
+/* Device-side outcome of the latest preprocess.  SYNCHRONISES `stream`.
+ *   keys_needed        number of (brick, Gaussian) keys the input produces
+ *   overflow           1 if keys_needed > key_capacity (forward/backward wrote zeros)
+ *   skipped_gaussians  degenerate inputs that were skipped
+ *   pairs              P_def: (Gaussian, voxel) pairs inside the cutoff = sum of box volumes  */
+typedef struct {
+    int64_t keys_needed;
+    int64_t pairs;
+    int32_t skipped_gaussians;
+    int32_t overflow;
+} gsvox_status;
+int gsvox_plan_status(gsvox_plan* plan, gsvox_status* status, void* stream);
+
+/* Debug/parity read-back of the latest preprocess (SYNCHRONISES): integer voxel boxes
+ * box_host [n,6] = lo_x,lo_y,lo_z,hi_x,hi_y,hi_z inclusive (0,0,0,-1,-1,-1 when empty or
+ * skipped) and the inverse covariance in index units minv_host [n,6] = xx,xy,xz,yy,yz,zz
+ * (M_idx = H M_world H, H = diag(spacing)).  Either pointer may be NULL.  HOST pointers.     */
+int gsvox_plan_geometry_host(gsvox_plan* plan, int32_t* box_host, float* minv_host, void* stream);
+
+/* Debug/parity read-back of the binning (SYNCHRONISES).  HOST pointers.
+ *   brick_start_host [nbricks+1]  CSR offsets into the key array, brick id = (bz*nby+by)*nbx+bx
+ *   key_gaussian_host [keys]      Gaussian id of every key, grouped by brick (any order within) */
+int gsvox_plan_bins_host(gsvox_plan* plan, int64_t* brick_start_host, int32_t* key_gaussian_host,
+                         int64_t key_host_capacity, void* stream);
+
+/* Per-kernel CUDA-event timing.  When enabled every kernel launched by the three calls above
+ * is bracketed by events on `stream`; gsvox_plan_timings() SYNCHRONISES and returns the
+ * accumulated milliseconds and launch counts since the last reset, indexed by GSVOX_K_*.     */
+enum {
+    GSVOX_K_PREPROCESS = 0,   /* a1  per-Gaussian record + box                   */
+    GSVOX_K_COUNT,            /* a2  keys per bin                                 */
+    GSVOX_K_SCAN,             /* a2  exclusive scan over bins                     */
+    GSVOX_K_SCATTER,          /* a2  write keys                                   */
+    GSVOX_K_FORWARD,          /* a3                                               */
+    GSVOX_K_BACKWARD,         /* a4                                               */
+    GSVOX_K_EPILOGUE,         /* a5  chain rule to scale/quat/pos                 */
+    GSVOX_K_MEMSET,           /* zero-fills issued by the library                 */
+    GSVOX_K_COUNT_KINDS
+};
+int gsvox_plan_set_timing(gsvox_plan* plan, int32_t enabled);
+int gsvox_plan_timings(gsvox_plan* plan, double* ms /*[GSVOX_K_COUNT_KINDS]*/,
+                       int64_t* launches /*[GSVOX_K_COUNT_KINDS]*/, int32_t reset, void* stream);
+
+/* End-to-end step on HOST buffers (bench.py's e2e leg): copies pos/scale/quat/weight/grad_out
+ * host->device, runs preprocess + forward + backward, copies out and the four gradients
+ * device->host, all on `stream`, then SYNCHRONISES.  `staging` is caller-owned device memory of
+ * at least gsvox_host_staging_bytes(); host buffers should be pinned.  out_host may be NULL
+ * (skip the volume read-back) and grad_out_host may be NULL (forward only).                   */
+int gsvox_host_staging_bytes(int64_t n_max, int32_t max_channels, const gsvox_grid* grid, size_t* bytes);
+int gsvox_step_host(gsvox_plan* plan, void* staging, size_t staging_bytes,
+                    const float* pos_host, const float* scale_host, const float* quat_host,
+                    const float* weight_host, int64_t n, int32_t channels,
+                    const float* grad_out_host, float* out_host,
+                    float* grad_weight_host, float* grad_pos_host, float* grad_scale_host,
+                    float* grad_quat_host, void* stream);
+
+const char* gsvox_error_string(int code);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char* gsvox_last_cuda_error(void);
+int gsvox_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSVOX_H */

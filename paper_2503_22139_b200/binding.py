@@ -1,0 +1,226 @@
+"""Thin Python binding of the gsvox C ABI (include/gsvox.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the CUDA
+kernels of libgsvox.so.  There is no CPU fallback: if the library is missing or cannot be
+loaded the import of this module's functions fails loudly.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgsvox.so")
+
+K_NAMES = ["preprocess", "count", "scan", "scatter", "forward", "backward", "epilogue", "memset"]
+
+EXPORTS = [
+    "gsvox_workspace_bytes", "gsvox_plan_create", "gsvox_plan_destroy", "gsvox_preprocess",
+    "gsvox_forward", "gsvox_backward", "gsvox_plan_status", "gsvox_plan_geometry_host",
+    "gsvox_plan_bins_host", "gsvox_plan_set_timing", "gsvox_plan_timings",
+    "gsvox_host_staging_bytes", "gsvox_step_host", "gsvox_error_string",
+    "gsvox_last_cuda_error", "gsvox_version",
+]
+
+
+class GsvoxGrid(C.Structure):
+    _fields_ = [("origin", C.c_float * 3), ("spacing", C.c_float * 3), ("dims", C.c_int32 * 3)]
+
+
+class GsvoxStatus(C.Structure):
+    _fields_ = [("keys_needed", C.c_int64), ("pairs", C.c_int64),
+                ("skipped_gaussians", C.c_int32), ("overflow", C.c_int32)]
+
+
+class GsvoxError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load libgsvox.so (built in-tree by paper_2503_22139_b200/build.py).  Never falls back."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise GsvoxError("libgsvox.so is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                         "(or python paper_2503_22139_b200/build.py); there is no CPU fallback")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, i32, szp = C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_size_t)
+    gp = C.POINTER(GsvoxGrid)
+    L.gsvox_workspace_bytes.argtypes = [i64, i32, gp, i64, szp]
+    L.gsvox_plan_create.argtypes = [i64, i32, gp, i64, vp, C.c_size_t, C.POINTER(vp)]
+    L.gsvox_plan_destroy.argtypes = [vp]
+    L.gsvox_plan_destroy.restype = None
+    L.gsvox_preprocess.argtypes = [vp, vp, vp, vp, i64, vp]
+    L.gsvox_forward.argtypes = [vp, vp, i32, vp, vp]
+    L.gsvox_backward.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp]
+    L.gsvox_plan_status.argtypes = [vp, C.POINTER(GsvoxStatus), vp]
+    L.gsvox_plan_geometry_host.argtypes = [vp, vp, vp, vp]
+    L.gsvox_plan_bins_host.argtypes = [vp, vp, vp, i64, vp]
+    L.gsvox_plan_set_timing.argtypes = [vp, i32]
+    L.gsvox_plan_timings.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), i32, vp]
+    L.gsvox_host_staging_bytes.argtypes = [i64, i32, gp, szp]
+    L.gsvox_step_host.argtypes = [vp, vp, C.c_size_t, vp, vp, vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp]
+    L.gsvox_error_string.argtypes = [C.c_int]
+    L.gsvox_error_string.restype = C.c_char_p
+    L.gsvox_last_cuda_error.restype = C.c_char_p
+    L.gsvox_version.restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != 0:
+        L = lib()
+        msg = L.gsvox_error_string(rc).decode()
+        extra = L.gsvox_last_cuda_error().decode()
+        raise GsvoxError("gsvox error %d: %s%s" % (rc, msg, (" [" + extra + "]") if extra and rc == -3 else ""))
+
+
+def make_grid(origin, spacing, dims):
+    g = GsvoxGrid()
+    for k in range(3):
+        g.origin[k] = float(origin[k]); g.spacing[k] = float(spacing[k]); g.dims[k] = int(dims[k])
+    return g
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t, name):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise GsvoxError("%s must be a contiguous float32 CUDA tensor" % name)
+    return C.c_void_p(t.data_ptr())
+
+
+def _host(t, name):
+    if t is None:
+        return None
+    if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+        raise GsvoxError("%s must be a contiguous float32 CPU tensor" % name)
+    return C.c_void_p(t.data_ptr())
+
+
+class Plan:
+    """gsvox_plan + the torch-owned workspace it lives in."""
+
+    def __init__(self, n_max, grid, max_channels=1, key_capacity=None, device="cuda"):
+        origin, spacing, dims = grid
+        self.grid = make_grid(origin, spacing, dims)
+        self.dims = tuple(int(d) for d in dims)
+        self.n_max = int(n_max)
+        self.max_channels = int(max_channels)
+        if key_capacity is None:
+            # a key is one Gaussian touching one 8^3 brick; never more than n * nbricks
+            nbricks = 1
+            for d in self.dims:
+                nbricks *= (d + 7) // 8
+            key_capacity = min(self.n_max * nbricks, max(1 << 22, 64 * self.n_max))
+        self.key_capacity = int(key_capacity)
+        self.device = torch.device(device)
+        nbytes = C.c_size_t(0)
+        _check(lib().gsvox_workspace_bytes(self.n_max, self.max_channels, C.byref(self.grid),
+                                           self.key_capacity, C.byref(nbytes)))
+        self.workspace_bytes = int(nbytes.value)
+        self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        self._h = C.c_void_p(None)
+        _check(lib().gsvox_plan_create(self.n_max, self.max_channels, C.byref(self.grid), self.key_capacity,
+                                       C.c_void_p(base), self.workspace_bytes, C.byref(self._h)))
+        self.n = None
+        self._staging = None
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().gsvox_plan_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    __del__ = close
+
+    # --- the three hot-path calls -----------------------------------------------------
+    def preprocess(self, pos, scale, quat):
+        n = int(pos.shape[0])
+        _check(lib().gsvox_preprocess(self._h, _dev(pos, "pos"), _dev(scale, "scale"), _dev(quat, "quat"),
+                                      n, _stream()))
+        self.n = n
+
+    def forward(self, weight, out=None):
+        ch = int(weight.shape[1])
+        nx, ny, nz = self.dims
+        if out is None:
+            out = torch.empty((ch, nz, ny, nx), dtype=torch.float32, device=self.device)
+        _check(lib().gsvox_forward(self._h, _dev(weight, "weight"), ch, _dev(out, "out"), _stream()))
+        return out
+
+    def backward(self, weight, grad_out, grads=None):
+        n, ch = int(weight.shape[0]), int(weight.shape[1])
+        if grads is None:
+            mk = lambda k: torch.empty((n, k), dtype=torch.float32, device=self.device)
+            grads = (mk(ch), mk(3), mk(3), mk(4))
+        gw, gp, gs, gq = grads
+        _check(lib().gsvox_backward(self._h, _dev(weight, "weight"), ch, _dev(grad_out, "grad_out"),
+                                    _dev(gw, "grad_weight"), _dev(gp, "grad_pos"), _dev(gs, "grad_scale"),
+                                    _dev(gq, "grad_quat"), _stream()))
+        return grads
+
+    # --- synchronising helpers --------------------------------------------------------
+    def status(self):
+        s = GsvoxStatus()
+        _check(lib().gsvox_plan_status(self._h, C.byref(s), _stream()))
+        return {"keys_needed": int(s.keys_needed), "pairs": int(s.pairs),
+                "skipped_gaussians": int(s.skipped_gaussians), "overflow": bool(s.overflow)}
+
+    def geometry(self):
+        box = torch.empty((self.n, 6), dtype=torch.int32)
+        minv = torch.empty((self.n, 6), dtype=torch.float32)
+        _check(lib().gsvox_plan_geometry_host(self._h, C.c_void_p(box.data_ptr()), C.c_void_p(minv.data_ptr()),
+                                              _stream()))
+        return box.numpy(), minv.numpy()
+
+    def bins(self):
+        nb = [(d + 7) // 8 for d in self.dims]
+        nbricks = nb[0] * nb[1] * nb[2]
+        start = torch.empty(nbricks + 1, dtype=torch.int64)
+        _check(lib().gsvox_plan_bins_host(self._h, C.c_void_p(start.data_ptr()), None, 0, _stream()))
+        total = int(start[-1])
+        keys = torch.empty(max(total, 1), dtype=torch.int32)
+        _check(lib().gsvox_plan_bins_host(self._h, C.c_void_p(start.data_ptr()), C.c_void_p(keys.data_ptr()),
+                                          total, _stream()))
+        return start.numpy(), keys.numpy()[:total]
+
+    def set_timing(self, on):
+        _check(lib().gsvox_plan_set_timing(self._h, 1 if on else 0))
+
+    def timings(self, reset=True):
+        ms = (C.c_double * len(K_NAMES))()
+        cnt = (C.c_int64 * len(K_NAMES))()
+        _check(lib().gsvox_plan_timings(self._h, ms, cnt, 1 if reset else 0, _stream()))
+        return ({k: float(ms[i]) for i, k in enumerate(K_NAMES)},
+                {k: int(cnt[i]) for i, k in enumerate(K_NAMES)})
+
+    # --- end-to-end on host buffers ---------------------------------------------------
+    def step_host(self, pos, scale, quat, weight, grad_out=None, out=None, grads=None):
+        """Host (pinned) tensors in, host tensors out; H2D/D2H copies happen inside the call."""
+        n, ch = int(pos.shape[0]), int(weight.shape[1])
+        if self._staging is None:
+            nbytes = C.c_size_t(0)
+            _check(lib().gsvox_host_staging_bytes(self.n_max, self.max_channels, C.byref(self.grid), C.byref(nbytes)))
+            self._staging_bytes = int(nbytes.value)
+            self._staging = torch.empty(self._staging_bytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self._staging.data_ptr() + 255) & ~255
+        gw = gp = gs = gq = None
+        if grad_out is not None:
+            gw, gp, gs, gq = grads
+        _check(lib().gsvox_step_host(self._h, C.c_void_p(base), self._staging_bytes,
+                                     _host(pos, "pos"), _host(scale, "scale"), _host(quat, "quat"),
+                                     _host(weight, "weight"), n, ch, _host(grad_out, "grad_out"), _host(out, "out"),
+                                     _host(gw, "grad_weight"), _host(gp, "grad_pos"), _host(gs, "grad_scale"),
+                                     _host(gq, "grad_quat"), _stream()))
+        self.n = n
+        return out, grads

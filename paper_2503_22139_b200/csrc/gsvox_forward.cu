@@ -1,0 +1,213 @@
+// gsvox_forward.cu — step a3: per-brick forward accumulation (Eq. 5).
+//
+// One CTA of 64 threads per 8^3 brick; thread t owns the x-row (y = t&7, z = t>>3) of the brick,
+// i.e. 8 consecutive voxels per channel, accumulated in registers and written once.  The brick's
+// keys are staged 64 at a time into shared memory: each thread gathers one 64-byte Gaussian
+// record (four LDG.128, L2-resident: a record is shared by ~20 bricks), rebases the centre to
+// brick-local coordinates and derives the brick-local row mask (which of the 64 rows lie inside
+// the Gaussian's box in y,z) and x mask.  Warps then walk the staged batch; a warp whose 32 rows
+// miss the box skips the key.
+//
+// Along a row the exponent of Eq. 4 is the parabola E(k) = Es - A (k - xs)^2 (base 2), with
+// xs, Es from the LDL^T form of the record (sum of squares, no cancellation).  For A <= 1 the
+// eight values are produced by a centre-out multiplicative recurrence from k = 3:
+//     G(k+1) = G(k) r(k),  r(k+1) = r(k) c,  c = 2^(-2A)      (exact identity for a parabola)
+// 3 MUFU.EX2 + 14 FMUL per row instead of 8 MUFU: the kernel is then FMA-pipe bound, not
+// MUFU bound (16 vs 128 lanes/clk/SM).  Narrow Gaussians (A > 1, under ~0.85 voxel along x)
+// take the direct path, one EX2 per voxel: the recurrence would lose accuracy and could
+// underflow there (error budget).
+#include "gsvox_internal.cuh"
+
+namespace gsvox {
+
+constexpr int kFwdThreads = 64;
+constexpr int kFwdBatch = 64;
+constexpr float kRecurrenceMaxA = 1.0f;
+
+__device__ __forceinline__ float ex2f(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+template <int CH> struct FwdRec { static constexpr int kWords = (13 + CH + 3) & ~3; };
+
+// Stage key `k` of this brick into shared memory slot `dst`.
+template <int CH>
+__device__ __forceinline__ void stage_key(float* __restrict__ dst, const GsRec* __restrict__ rec,
+                                          const float* __restrict__ weight, int wstride, int c0,
+                                          uint32_t gid, int b0x, int b0y, int b0z)
+{
+    const float4* rp = reinterpret_cast<const float4*>(rec + gid);
+    float4 a = __ldg(rp), b = __ldg(rp + 1), c = __ldg(rp + 2), d = __ldg(rp + 3);
+    // a = cf.xyz, cexp | b = ci.xyz, negA | c = nl01, nl02, l12, nD1 | d = nD2, lo/hi packed
+    int cix = __float_as_int(b.x), ciy = __float_as_int(b.y), ciz = __float_as_int(b.z);
+    int w1 = __float_as_int(d.y), w2 = __float_as_int(d.z), w3 = __float_as_int(d.w);
+    int lox = (int16_t)(w1 & 0xffff), loy = (int16_t)(w1 >> 16), loz = (int16_t)(w2 & 0xffff);
+    int hix = (int16_t)(w2 >> 16), hiy = (int16_t)(w3 & 0xffff), hiz = (int16_t)(w3 >> 16);
+    int x0 = max(lox - b0x, 0), x1 = min(hix - b0x, 7);
+    int y0 = max(loy - b0y, 0), y1 = min(hiy - b0y, 7);
+    int z0 = max(loz - b0z, 0), z1 = min(hiz - b0z, 7);
+    uint32_t ym = ((2u << y1) - (1u << y0)) & 0xffu;               // bits y0..y1
+    uint32_t zm = ((2u << z1) - (1u << z0)) & 0xffu;
+    uint32_t xm = ((2u << x1) - (1u << x0)) & 0xffu;
+    uint32_t rep = ym * 0x01010101u;                                // ym in all four bytes
+    uint32_t sel0 = ((zm & 1u) ? 0xffu : 0u) | ((zm & 2u) ? 0xff00u : 0u) |
+                    ((zm & 4u) ? 0xff0000u : 0u) | ((zm & 8u) ? 0xff000000u : 0u);
+    uint32_t zh = zm >> 4;
+    uint32_t sel1 = ((zh & 1u) ? 0xffu : 0u) | ((zh & 2u) ? 0xff00u : 0u) |
+                    ((zh & 4u) ? 0xff0000u : 0u) | ((zh & 8u) ? 0xff000000u : 0u);
+    uint32_t flags = xm | ((-b.w > kRecurrenceMaxA) ? 0x100u : 0u);
+    float4* o = reinterpret_cast<float4*>(dst);
+    o[0] = make_float4((float)(cix - b0x) + a.x, (float)(ciy - b0y) + a.y, (float)(ciz - b0z) + a.z, b.w);
+    o[1] = make_float4(c.x, c.y, c.z, c.w);
+    o[2] = make_float4(d.x, a.w, __uint_as_float(rep & sel0), __uint_as_float(rep & sel1));
+    dst[12] = __uint_as_float(flags);
+    #pragma unroll
+    for (int ch = 0; ch < CH; ++ch) dst[13 + ch] = __ldg(weight + (size_t)gid * wstride + c0 + ch);
+}
+
+template <int CH, bool VEC>
+__global__ void __launch_bounds__(kFwdThreads)
+k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
+          const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
+          const float* __restrict__ weight, int wstride, int c0,
+          float* __restrict__ out, GridDev gd)
+{
+    constexpr int W = FwdRec<CH>::kWords;
+    __shared__ __align__(16) float s_rec[2][kFwdBatch * W];
+
+    const int tid = threadIdx.x;
+    const int b = blockIdx.x;
+    const int bx = b % gd.nb[0], by = (b / gd.nb[0]) % gd.nb[1], bz = b / (gd.nb[0] * gd.nb[1]);
+    const int b0x = bx * kBrick, b0y = by * kBrick, b0z = bz * kBrick;
+    const int ry = tid & 7, rz = tid >> 3;
+    const float fy = (float)ry, fz = (float)rz;
+    const int wsel = tid >> 5, lane = tid & 31;
+
+    float acc[CH][8];
+    #pragma unroll
+    for (int ch = 0; ch < CH; ++ch)
+        #pragma unroll
+        for (int k = 0; k < 8; ++k) acc[ch][k] = 0.f;
+
+    uint32_t kbeg = 0, kend = 0;
+    if (!status->overflow) { kbeg = bin_start[b]; kend = bin_start[b + 1]; }
+
+    int buf = 0;
+    for (uint32_t base = kbeg; base < kend; base += kFwdBatch, buf ^= 1) {
+        float* sb = s_rec[buf];
+        uint32_t k = base + tid;
+        if (k < kend) stage_key<CH>(sb + tid * W, rec, weight, wstride, c0, keys[k], b0x, b0y, b0z);
+        __syncthreads();
+        const int nb = min((uint32_t)kFwdBatch, kend - base);
+        for (int j = 0; j < nb; ++j) {
+            const float4* r = reinterpret_cast<const float4*>(sb + j * W);
+            const float4 r2 = r[2];
+            const uint32_t mrow = __float_as_uint(wsel ? r2.w : r2.z);
+            if (mrow == 0u) continue;                               // warp-uniform skip
+            const float4 r0 = r[0], r1 = r[1];
+            const uint32_t flags = __float_as_uint(sb[j * W + 12]);
+            const bool inside = (mrow >> lane) & 1u;
+            // row geometry: u2 = dz, u1 = dy + l12 dz, xs = cx - l01 dy - l02 dz
+            const float dy = fy - r0.y, dz = fz - r0.z;
+            const float u1 = fmaf(r1.z, dz, dy);
+            const float xs = fmaf(r1.y, dz, fmaf(r1.x, dy, r0.x));
+            const float Es = fmaf(r2.x * dz, dz, (r1.w * u1) * u1);
+            const float negA = r0.w;
+            float wv[CH];
+            #pragma unroll
+            for (int ch = 0; ch < CH; ++ch) wv[ch] = inside ? sb[j * W + 13 + ch] : 0.f;
+
+            if (!(flags & 0x100u)) {
+                // centre-out recurrence from k = 3
+                const float t3 = 3.0f - xs;
+                const float nAt = negA * t3;
+                const float E3 = fmaf(nAt, t3, Es);
+                const float Lf = fminf(fmaf(nAt, 2.0f, negA), 120.f);     // E(4) - E(3)
+                const float Lb = fminf(fmaf(nAt, -2.0f, negA), 120.f);    // E(2) - E(3)
+                const float cc = r2.y;
+                float G[8];
+                G[3] = ex2f(E3);
+                float rf = ex2f(Lf), rb = ex2f(Lb);
+                G[4] = G[3] * rf; rf *= cc; G[5] = G[4] * rf; rf *= cc; G[6] = G[5] * rf; rf *= cc; G[7] = G[6] * rf;
+                G[2] = G[3] * rb; rb *= cc; G[1] = G[2] * rb; rb *= cc; G[0] = G[1] * rb;
+                if ((flags & 0xffu) == 0xffu) {
+                    #pragma unroll
+                    for (int k2 = 0; k2 < 8; ++k2)
+                        #pragma unroll
+                        for (int ch = 0; ch < CH; ++ch) acc[ch][k2] = fmaf(wv[ch], G[k2], acc[ch][k2]);
+                } else {
+                    #pragma unroll
+                    for (int k2 = 0; k2 < 8; ++k2) {
+                        const float g = (flags & (1u << k2)) ? G[k2] : 0.f;
+                        #pragma unroll
+                        for (int ch = 0; ch < CH; ++ch) acc[ch][k2] = fmaf(wv[ch], g, acc[ch][k2]);
+                    }
+                }
+            } else {
+                // direct path: one EX2 per voxel
+                #pragma unroll
+                for (int k2 = 0; k2 < 8; ++k2) {
+                    const float t = (float)k2 - xs;
+                    float g = ex2f(fmaf(negA * t, t, Es));
+                    g = (flags & (1u << k2)) ? g : 0.f;
+                    #pragma unroll
+                    for (int ch = 0; ch < CH; ++ch) acc[ch][k2] = fmaf(wv[ch], g, acc[ch][k2]);
+                }
+            }
+        }
+    }
+
+    // write the row once (zeros for empty bricks); x fastest, [C, nz, ny, nx]
+    const int gy = b0y + ry, gz = b0z + rz;
+    if (gy < gd.dims[1] && gz < gd.dims[2]) {
+        const size_t plane = (size_t)gd.dims[0] * gd.dims[1] * gd.dims[2];
+        const size_t rowoff = ((size_t)gz * gd.dims[1] + gy) * gd.dims[0] + b0x;
+        #pragma unroll
+        for (int ch = 0; ch < CH; ++ch) {
+            float* o = out + (size_t)(c0 + ch) * plane + rowoff;
+            if (VEC) {
+                if (b0x + 3 < gd.dims[0])
+                    __stcs(reinterpret_cast<float4*>(o), make_float4(acc[ch][0], acc[ch][1], acc[ch][2], acc[ch][3]));
+                if (b0x + 7 < gd.dims[0])
+                    __stcs(reinterpret_cast<float4*>(o) + 1, make_float4(acc[ch][4], acc[ch][5], acc[ch][6], acc[ch][7]));
+            } else {
+                #pragma unroll
+                for (int k2 = 0; k2 < 8; ++k2)
+                    if (b0x + k2 < gd.dims[0]) o[k2] = acc[ch][k2];
+            }
+        }
+    }
+}
+
+template <int CH>
+static int launch_fwd_ch(gsvox_plan* p, const float* weight, int C, int c0, float* out, cudaStream_t st)
+{
+    LaunchScope ls(p, GSVOX_K_FORWARD, st);
+    bool vec = (p->gd.dims[0] % 4 == 0) && (((uintptr_t)out & 15) == 0);
+    if (vec)
+        k_forward<CH, true><<<p->nbins, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
+                                                               weight, C, c0, out, p->gd);
+    else
+        k_forward<CH, false><<<p->nbins, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
+                                                                weight, C, c0, out, p->gd);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
+
+int launch_forward(gsvox_plan* p, const float* weight, int channels, float* out, cudaStream_t st)
+{
+    // channel groups of 9, 3, 1: C = 9 (motion-basis fields) and C = 1 (CBCT) are single launches
+    int c0 = 0, rc = GSVOX_OK;
+    while (c0 < channels && rc == GSVOX_OK) {
+        int left = channels - c0;
+        if (left >= 9)      { rc = launch_fwd_ch<9>(p, weight, channels, c0, out, st); c0 += 9; }
+        else if (left >= 3) { rc = launch_fwd_ch<3>(p, weight, channels, c0, out, st); c0 += 3; }
+        else                { rc = launch_fwd_ch<1>(p, weight, channels, c0, out, st); c0 += 1; }
+    }
+    return rc;
+}
+
+}  // namespace gsvox

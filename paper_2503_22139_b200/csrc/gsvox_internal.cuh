@@ -1,0 +1,117 @@
+// gsvox_internal.cuh — shared declarations of the CUDA path (sm_100a only).
+// Not part of the public boundary (include/gsvox.h) and never seen by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/gsvox.h"
+
+namespace gsvox {
+
+// ------------------------------------------------------------------------------------------
+// Per-Gaussian geometry record written by a1 (k_preprocess), 64 B, read by a3/a4 with four
+// 16-byte loads.  Index space: voxel (i,j,k) sits at integer coordinates (i,j,k).
+//   centre   = ci + cf   (integer part + fp32 fraction in [-0.5,0.5]: brick-local coordinates
+//              (ci - brick_origin) + cf then carry ~1e-7 voxel of error whatever the grid size)
+//   exponent (base 2) of Eq. 4 through the LDL^T factorisation of M_idx = H Sigma^-1 H:
+//              E = -( A u0^2 + D1 u1^2 + D2 u2^2 ),  u2 = dz, u1 = dy + l12 dz,
+//              u0 = dx + l01 dy + l02 dz,  A = kappa2*M00, kappa2 = log2(e)/2
+//            a sum of squares: no cancellation for needle-like Gaussians (kernels)
+//   cexp     = 2^(-2A), rounded from fp64: ratio of successive ratios along an x-row
+//   box      = inclusive voxel box (reading A5), int16; empty <=> hi[0] < lo[0]
+// ------------------------------------------------------------------------------------------
+struct __align__(16) GsRec {
+    float   cf[3];      //  0
+    float   cexp;       // 12
+    int32_t ci[3];      // 16
+    float   negA;       // 28   -A
+    float   nl01, nl02; // 32   -l01, -l02
+    float   l12;        // 40
+    float   nD1, nD2;   // 44   -D1, -D2 (already times kappa2)
+    int16_t lo[3];      // 52
+    int16_t hi[3];      // 58
+};
+static_assert(sizeof(GsRec) == 64, "GsRec must be 64 bytes");
+
+// What a5 (chain rule) needs from the inputs, copied so that the caller's arrays need not
+// outlive gsvox_preprocess().
+struct __align__(16) GsAux {
+    float q[4];
+    float s[3];
+    uint32_t valid;     // 0 = skipped (degenerate input)
+};
+static_assert(sizeof(GsAux) == 32, "GsAux must be 32 bytes");
+
+// Device-resident counters of one preprocess.
+struct DevStatus {
+    unsigned long long keys_needed;
+    unsigned long long pairs;
+    unsigned int skipped;
+    unsigned int overflow;
+    unsigned int pad[2];
+};
+
+struct GridDev {
+    double origin[3];
+    double spacing[3];
+    int dims[3];
+    int nb[3];          // bricks per axis
+    int nbricks;
+};
+
+constexpr int kBrick = GSVOX_BRICK;
+constexpr int kBrickVox = kBrick * kBrick * kBrick;
+constexpr int kScanItemsPerBlock = 2048;     // k_scan_*: 256 threads x 8 items
+
+inline __host__ __device__ int acc_stride(int channels) { return (9 + channels + 3) & ~3; }
+
+}  // namespace gsvox
+
+// The host-side plan (opaque in the public header).
+struct gsvox_plan {
+    gsvox_grid grid;
+    gsvox::GridDev gd;
+    int64_t n_max;
+    int32_t max_channels;
+    int64_t key_capacity;
+    int64_t n;                 // Gaussians of the latest preprocess, -1 before the first
+    // device pointers, all inside the caller's workspace
+    gsvox::DevStatus* status;
+    gsvox::GsRec* rec;
+    gsvox::GsAux* aux;
+    uint32_t* bin_count;       // [nbins+1]  counts, then write cursors
+    uint32_t* bin_start;       // [nbins+1]  exclusive scan of counts
+    uint32_t* scan_partial;    // [scan blocks]
+    uint32_t* keys;            // [key_capacity] Gaussian id per key, grouped by brick
+    float* acc;                // [n_max * acc_stride(max_channels)] backward accumulators
+    int nbins;
+    // timing
+    int timing;
+    double ms[GSVOX_K_COUNT_KINDS];
+    int64_t launches[GSVOX_K_COUNT_KINDS];
+    struct Pending { cudaEvent_t a, b; int kind; };
+    Pending* pending;
+    int n_pending, cap_pending;
+};
+
+namespace gsvox {
+
+// RAII bracket around one kernel launch: counts it and, when timing is on, records events.
+struct LaunchScope {
+    gsvox_plan* p; int kind; cudaStream_t st; cudaEvent_t a, b; bool timed;
+    LaunchScope(gsvox_plan* plan, int kind_, cudaStream_t s);
+    ~LaunchScope();
+};
+
+int cuda_fail(cudaError_t e, const char* what);          // records text, returns GSVOX_ECUDA
+#define GSVOX_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) \
+        return gsvox::cuda_fail(e__, #call); } while (0)
+
+// stage entry points implemented in the other .cu files
+int launch_preprocess(gsvox_plan* p, const float* pos, const float* scale, const float* quat,
+                      int64_t n, cudaStream_t st);
+int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st);
+int launch_forward(gsvox_plan* p, const float* weight, int channels, float* out, cudaStream_t st);
+int launch_backward(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
+                    float* gw, float* gp, float* gs, float* gq, cudaStream_t st);
+
+}  // namespace gsvox

@@ -1,0 +1,283 @@
+// gsvox_preprocess.cu — steps a1 (per-Gaussian geometry) and a2 (brick binning).
+//
+// a1  k_preprocess: one thread per Gaussian, fp64.  Follows DESIGN.md "forward definition"
+//     steps 1-5 (Eq. 4; Sigma = R S S^T R^T per north_star).  The box bounds use
+//     the operation order of reading A5 with explicitly rounded intrinsics (__dmul_rn, ...),
+//     so no FMA contraction can change an integer bound.
+// a2  counting sort of (brick, Gaussian) keys by brick: k_count -> 3-kernel exclusive scan ->
+//     k_scatter.  Order inside a brick is whatever the atomics produce (sums are order
+//     independent within tolerance, reading A13).
+#include "gsvox_internal.cuh"
+
+namespace gsvox {
+
+__device__ __forceinline__ bool finite_d(double v) { return isfinite(v); }
+
+__global__ void __launch_bounds__(256)
+k_preprocess(const float* __restrict__ pos, const float* __restrict__ scale,
+             const float* __restrict__ quat, int n, GridDev gd,
+             GsRec* __restrict__ rec, GsAux* __restrict__ aux, DevStatus* __restrict__ status)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long my_pairs = 0; unsigned int my_skipped = 0;
+    if (i < n) {
+        double p[3], s[3], q[4];
+        for (int k = 0; k < 3; ++k) { p[k] = (double)pos[3 * i + k]; s[k] = (double)scale[3 * i + k]; }
+        for (int k = 0; k < 4; ++k) q[k] = (double)quat[4 * i + k];
+        bool bad = false;
+        for (int k = 0; k < 3; ++k) bad |= !finite_d(p[k]) || !finite_d(s[k]) || !(s[k] > 0.0);
+        for (int k = 0; k < 4; ++k) bad |= !finite_d(q[k]);
+        bad |= (q[0] == 0.0 && q[1] == 0.0 && q[2] == 0.0 && q[3] == 0.0);
+
+        GsAux a;
+        for (int k = 0; k < 4; ++k) a.q[k] = (float)q[k];
+        for (int k = 0; k < 3; ++k) a.s[k] = (float)s[k];
+        a.valid = bad ? 0u : 1u;
+        aux[i] = a;
+
+        GsRec r;
+        r.cf[0] = r.cf[1] = r.cf[2] = 0.f; r.cexp = 1.f; r.ci[0] = r.ci[1] = r.ci[2] = 0;
+        r.negA = r.nl01 = r.nl02 = r.l12 = r.nD1 = r.nD2 = 0.f;
+        r.lo[0] = r.lo[1] = r.lo[2] = 0; r.hi[0] = r.hi[1] = r.hi[2] = -1;
+        if (bad) { my_skipped = 1; }
+        else {
+            // step 1: normalise (reading A5 order: ((r*r + x*x) + y*y) + z*z)
+            double n2 = __dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(q[0], q[0]), __dmul_rn(q[1], q[1])),
+                                            __dmul_rn(q[2], q[2])), __dmul_rn(q[3], q[3]));
+            double nn = __dsqrt_rn(n2);
+            double qr = __ddiv_rn(q[0], nn), qx = __ddiv_rn(q[1], nn),
+                   qy = __ddiv_rn(q[2], nn), qz = __ddiv_rn(q[3], nn);
+            // step 2: rotation matrix, entries as written in the definition
+            double R[9];
+            #define MUL __dmul_rn
+            #define ADD __dadd_rn
+            #define SUB __dsub_rn
+            R[0] = SUB(1.0, MUL(2.0, ADD(MUL(qy, qy), MUL(qz, qz))));
+            R[1] = MUL(2.0, SUB(MUL(qx, qy), MUL(qr, qz)));
+            R[2] = MUL(2.0, ADD(MUL(qx, qz), MUL(qr, qy)));
+            R[3] = MUL(2.0, ADD(MUL(qx, qy), MUL(qr, qz)));
+            R[4] = SUB(1.0, MUL(2.0, ADD(MUL(qx, qx), MUL(qz, qz))));
+            R[5] = MUL(2.0, SUB(MUL(qy, qz), MUL(qr, qx)));
+            R[6] = MUL(2.0, SUB(MUL(qx, qz), MUL(qr, qy)));
+            R[7] = MUL(2.0, ADD(MUL(qy, qz), MUL(qr, qx)));
+            R[8] = SUB(1.0, MUL(2.0, ADD(MUL(qx, qx), MUL(qy, qy))));
+            // steps 4-5: r_k = 3 sqrt(Sigma_kk), integer box clipped to the grid
+            double s0 = MUL(s[0], s[0]), s1 = MUL(s[1], s[1]), s2 = MUL(s[2], s[2]);
+            bool empty = false; int lo[3], hi[3];
+            #pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                double Skk = ADD(ADD(MUL(MUL(R[3 * k], R[3 * k]), s0),
+                                     MUL(MUL(R[3 * k + 1], R[3 * k + 1]), s1)),
+                                 MUL(MUL(R[3 * k + 2], R[3 * k + 2]), s2));
+                double rk = MUL(GSVOX_SIGMA_CUTOFF, __dsqrt_rn(Skk));
+                double l = ceil(__ddiv_rn(SUB(SUB(p[k], rk), gd.origin[k]), gd.spacing[k]));
+                double h = floor(__ddiv_rn(SUB(ADD(p[k], rk), gd.origin[k]), gd.spacing[k]));
+                double top = (double)(gd.dims[k] - 1);
+                if (l < 0.0) l = 0.0;
+                if (h > top) h = top;
+                if (!(h >= l)) { empty = true; lo[k] = 0; hi[k] = -1; }
+                else { lo[k] = (int)l; hi[k] = (int)h; }
+            }
+            #undef MUL
+            #undef ADD
+            #undef SUB
+            if (!empty) {
+                my_pairs = (unsigned long long)(hi[0] - lo[0] + 1) * (unsigned long long)(hi[1] - lo[1] + 1)
+                         * (unsigned long long)(hi[2] - lo[2] + 1);
+                // step 3 in index units: M = H R diag(1/s^2) R^T H, H = diag(spacing)
+                double is2[3] = { 1.0 / s0, 1.0 / s1, 1.0 / s2 };
+                double M[6]; int t = 0;
+                for (int a2 = 0; a2 < 3; ++a2)
+                    for (int b = a2; b < 3; ++b) {
+                        double acc = 0.0;
+                        for (int j = 0; j < 3; ++j) acc += R[3 * a2 + j] * is2[j] * R[3 * b + j];
+                        M[t++] = acc * gd.spacing[a2] * gd.spacing[b];      // xx xy xz yy yz zz
+                    }
+                // LDL^T, x eliminated first (x is the row direction of a3/a4)
+                const double k2 = 0.72134752044448170368;                  // log2(e)/2
+                double D0 = M[0], l01 = M[1] / D0, l02 = M[2] / D0;
+                double D1 = M[3] - M[1] * l01;
+                double l12 = (M[4] - M[1] * l02) / D1;
+                double D2 = M[5] - M[2] * l02 - l12 * l12 * D1;
+                if (!(D1 > 0.0)) { D1 = 0.0; l12 = 0.0; }                   // rounding guard
+                if (!(D2 > 0.0)) D2 = 0.0;
+                r.negA = (float)(-k2 * D0); r.nl01 = (float)(-l01); r.nl02 = (float)(-l02);
+                r.l12 = (float)l12; r.nD1 = (float)(-k2 * D1); r.nD2 = (float)(-k2 * D2);
+                r.cexp = (float)exp2(-2.0 * k2 * D0);
+                for (int k = 0; k < 3; ++k) {
+                    double c = (p[k] - gd.origin[k]) / gd.spacing[k];
+                    double ci = rint(c);
+                    if (ci > 1073741824.0) ci = 1073741824.0;
+                    if (ci < -1073741824.0) ci = -1073741824.0;
+                    r.ci[k] = (int)ci; r.cf[k] = (float)(c - ci);
+                    r.lo[k] = (int16_t)lo[k]; r.hi[k] = (int16_t)hi[k];
+                }
+            }
+        }
+        rec[i] = r;
+    }
+    // block-level totals -> one atomic per block
+    __shared__ unsigned long long sh_pairs[8]; __shared__ unsigned int sh_skip[8];
+    for (int o = 16; o > 0; o >>= 1) {
+        my_pairs += __shfl_xor_sync(0xffffffffu, my_pairs, o);
+        my_skipped += __shfl_xor_sync(0xffffffffu, my_skipped, o);
+    }
+    int w = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) { sh_pairs[w] = my_pairs; sh_skip[w] = my_skipped; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long tp = 0; unsigned int ts = 0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) { tp += sh_pairs[k]; ts += sh_skip[k]; }
+        if (tp) atomicAdd(&status->pairs, tp);
+        if (ts) atomicAdd(&status->skipped, ts);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a2: keys.  Eight lanes cooperate on one Gaussian and stride over the bricks of its box.
+// MODE 0: count keys per brick.  MODE 1: claim a slot per key and write the Gaussian id.
+// ------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(256)
+k_keys(const GsRec* __restrict__ rec, int n, GridDev gd, uint32_t* __restrict__ bin_count,
+       uint32_t* __restrict__ keys, const DevStatus* __restrict__ status)
+{
+    if (MODE == 1 && status->overflow) return;
+    int g = (blockIdx.x * blockDim.x + threadIdx.x) >> 3;
+    int sub = threadIdx.x & 7;
+    if (g >= n) return;
+    const int4* rp = reinterpret_cast<const int4*>(rec + g);
+    int4 w3 = __ldg(rp + 3);                      // bytes 48..63: nD2, lo[3], hi[3]
+    int lox = (int16_t)(w3.y & 0xffff), loy = (int16_t)(w3.y >> 16);
+    int loz = (int16_t)(w3.z & 0xffff), hix = (int16_t)(w3.z >> 16);
+    int hiy = (int16_t)(w3.w & 0xffff), hiz = (int16_t)(w3.w >> 16);
+    if (hix < lox) return;
+    int bx0 = lox >> 3, by0 = loy >> 3, bz0 = loz >> 3;
+    int ex = (hix >> 3) - bx0 + 1, ey = (hiy >> 3) - by0 + 1, ez = (hiz >> 3) - bz0 + 1;
+    int total = ex * ey * ez;
+    for (int t = sub; t < total; t += 8) {
+        int tx = t % ex, r = t / ex, ty = r % ey, tz = r / ey;
+        int b = ((bz0 + tz) * gd.nb[1] + (by0 + ty)) * gd.nb[0] + (bx0 + tx);
+        if (MODE == 0) atomicAdd(&bin_count[b], 1u);
+        else { uint32_t slot = atomicAdd(&bin_count[b], 1u); keys[slot] = (uint32_t)g; }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Exclusive scan over the nbins counters, three launches (reduce, scan of partials, apply).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_scan_reduce(const uint32_t* __restrict__ cnt, int nbins, uint32_t* __restrict__ partial)
+{
+    int base = blockIdx.x * kScanItemsPerBlock;
+    uint32_t s = 0;
+    for (int k = threadIdx.x; k < kScanItemsPerBlock; k += 256) {
+        int idx = base + k;
+        if (idx < nbins) s += cnt[idx];
+    }
+    __shared__ uint32_t sh[8];
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) { uint32_t t = 0; for (int k = 0; k < 8; ++k) t += sh[k]; partial[blockIdx.x] = t; }
+}
+
+__global__ void __launch_bounds__(1024)
+k_scan_partials(uint32_t* __restrict__ partial, int nblocks, DevStatus* __restrict__ status,
+                unsigned long long key_capacity)
+{
+    // single block: serial-per-thread chunks + warp scans; nblocks is small (<= a few thousand)
+    __shared__ unsigned long long sh[1024];
+    int per = (nblocks + 1023) / 1024;
+    int b0 = threadIdx.x * per;
+    unsigned long long s = 0;
+    for (int k = 0; k < per; ++k) if (b0 + k < nblocks) s += partial[b0 + k];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+        unsigned long long v = (threadIdx.x >= o) ? sh[threadIdx.x - o] : 0ull;
+        __syncthreads();
+        sh[threadIdx.x] += v;
+        __syncthreads();
+    }
+    unsigned long long run = sh[threadIdx.x] - s;           // exclusive prefix of this chunk
+    for (int k = 0; k < per; ++k)
+        if (b0 + k < nblocks) { uint32_t v = partial[b0 + k]; partial[b0 + k] = (uint32_t)run; run += v; }
+    if (threadIdx.x == 1023) {
+        unsigned long long total = sh[1023];
+        status->keys_needed = total;
+        status->overflow = (total > key_capacity || total > 0xfffffff0ull) ? 1u : 0u;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_scan_apply(uint32_t* __restrict__ cnt, int nbins, const uint32_t* __restrict__ partial,
+             uint32_t* __restrict__ start)
+{
+    // 256 threads x 8 consecutive items; counts are replaced by write cursors (= start)
+    __shared__ uint32_t sh[8];
+    int base = blockIdx.x * kScanItemsPerBlock + threadIdx.x * 8;
+    uint32_t v[8]; uint32_t s = 0;
+    #pragma unroll
+    for (int k = 0; k < 8; ++k) { v[k] = (base + k < nbins) ? cnt[base + k] : 0u; s += v[k]; }
+    uint32_t inc = s;
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) sh[w] = inc;
+    __syncthreads();
+    uint32_t woff = 0;
+    for (int k = 0; k < w; ++k) woff += sh[k];
+    uint32_t run = partial[blockIdx.x] + woff + inc - s;
+    #pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        if (base + k < nbins) { start[base + k] = run; cnt[base + k] = run; }
+        run += v[k];
+    }
+    // sentinel start[nbins] = total
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 255) start[nbins] = run;
+}
+
+int launch_preprocess(gsvox_plan* p, const float* pos, const float* scale, const float* quat,
+                      int64_t n, cudaStream_t st)
+{
+    { LaunchScope ls(p, GSVOX_K_MEMSET, st);
+      GSVOX_CUDA(cudaMemsetAsync(p->status, 0, sizeof(DevStatus), st)); }
+    { LaunchScope ls(p, GSVOX_K_MEMSET, st);
+      GSVOX_CUDA(cudaMemsetAsync(p->bin_count, 0, sizeof(uint32_t) * (size_t)(p->nbins + 1), st)); }
+    if (n > 0) {
+        LaunchScope ls(p, GSVOX_K_PREPROCESS, st);
+        int blocks = (int)((n + 255) / 256);
+        k_preprocess<<<blocks, 256, 0, st>>>(pos, scale, quat, (int)n, p->gd, p->rec, p->aux, p->status);
+        GSVOX_CUDA(cudaGetLastError());
+    }
+    return GSVOX_OK;
+}
+
+int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
+{
+    int kblocks = (int)((n * 8 + 255) / 256);
+    if (n > 0) {
+        LaunchScope ls(p, GSVOX_K_COUNT, st);
+        k_keys<0><<<kblocks, 256, 0, st>>>(p->rec, (int)n, p->gd, p->bin_count, p->keys, p->status);
+        GSVOX_CUDA(cudaGetLastError());
+    }
+    int sblocks = (p->nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock;
+    { LaunchScope ls(p, GSVOX_K_SCAN, st);
+      k_scan_reduce<<<sblocks, 256, 0, st>>>(p->bin_count, p->nbins, p->scan_partial);
+      GSVOX_CUDA(cudaGetLastError()); }
+    { LaunchScope ls(p, GSVOX_K_SCAN, st);
+      k_scan_partials<<<1, 1024, 0, st>>>(p->scan_partial, sblocks, p->status,
+                                          (unsigned long long)p->key_capacity);
+      GSVOX_CUDA(cudaGetLastError()); }
+    { LaunchScope ls(p, GSVOX_K_SCAN, st);
+      k_scan_apply<<<sblocks, 256, 0, st>>>(p->bin_count, p->nbins, p->scan_partial, p->bin_start);
+      GSVOX_CUDA(cudaGetLastError()); }
+    if (n > 0) {
+        LaunchScope ls(p, GSVOX_K_SCATTER, st);
+        k_keys<1><<<kblocks, 256, 0, st>>>(p->rec, (int)n, p->gd, p->bin_count, p->keys, p->status);
+        GSVOX_CUDA(cudaGetLastError());
+    }
+    return GSVOX_OK;
+}
+
+}  // namespace gsvox

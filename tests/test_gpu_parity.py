@@ -1,0 +1,280 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element,
+on identical seeded fp32 inputs.  Tolerances are north_star's:
+    forward   max|err| <= 1e-5 * max|out| + 1e-6
+    gradients relative L2 error <= 1e-4 per parameter group (w, p, s, q)
+Integer work (voxel boxes, key sets) must be bit-exact.  Run with `-m gpu` on a B200.
+"""
+import numpy as np
+import pytest
+
+import gsvox_inputs
+import oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+FWD_REL, FWD_ABS, GRAD_REL = 1e-5, 1e-6, 1e-4
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2503_22139_b200 as p
+    p.lib()                                     # fails loudly if the extension is missing
+    torch.cuda.set_device(0)
+    return p
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(pkg, case, grad=None, key_capacity=None, max_channels=None):
+    plan = pkg.Plan(max(case.n, 1), case.grid, max_channels=max_channels or case.channels,
+                    key_capacity=key_capacity)
+    pos, scale, quat, w = dev(case.pos), dev(case.scale), dev(case.quat), dev(case.weight)
+    plan.preprocess(pos, scale, quat)
+    if key_capacity is None:
+        st = plan.status()
+        if st["overflow"]:                      # default capacity too small: size it exactly
+            plan = pkg.Plan(max(case.n, 1), case.grid, max_channels=max_channels or case.channels,
+                            key_capacity=st["keys_needed"])
+            plan.preprocess(pos, scale, quat)
+    out = plan.forward(w)
+    grads = None
+    if grad is not None:
+        grads = plan.backward(w, dev(grad))
+    torch.cuda.synchronize()
+    return plan, out.cpu().numpy(), None if grads is None else [g.cpu().numpy() for g in grads]
+
+
+def check_forward(out, ref):
+    err = np.abs(out.astype(np.float64) - ref).max()
+    tol = FWD_REL * np.abs(ref).max() + FWD_ABS
+    assert err <= tol, "forward max|err| %.3e > tol %.3e" % (err, tol)
+    return err, tol
+
+
+def check_grads(grads, refs):
+    rels = {}
+    for name, a, b in zip(("w", "p", "s", "q"), grads, refs):
+        nb = np.linalg.norm(b)
+        rel = np.linalg.norm(a.astype(np.float64) - b) / nb if nb > 0 else np.abs(a).max()
+        rels[name] = rel
+        assert rel <= GRAD_REL, "grad %s rel L2 %.3e > %.1e" % (name, rel, GRAD_REL)
+    return rels
+
+
+def check_geometry_and_bins(plan, case):
+    """Boxes bit-identical to the oracle (reading A5); M_idx within 1e-5 relative; every
+    (brick, Gaussian) key present exactly once; P_def identical."""
+    geo = oracle.geometry(case.pos, case.scale, case.quat, case.grid)
+    box, minv = plan.geometry()
+    assert np.array_equal(box, geo["box"]), "voxel boxes differ from the oracle: %d mismatches" % \
+        int((box != geo["box"]).any(1).sum())
+    h = np.asarray(case.spacing, np.float64)
+    scale6 = np.array([h[0] * h[0], h[0] * h[1], h[0] * h[2], h[1] * h[1], h[1] * h[2], h[2] * h[2]])
+    live = geo["box"][:, 3] >= geo["box"][:, 0]
+    Mi = geo["M"] * scale6
+    nrm = np.linalg.norm(Mi[live], axis=1, keepdims=True)
+    assert np.all(np.abs(minv[live] - Mi[live]) <= 1e-5 * nrm)
+    st = plan.status()
+    ext = np.clip(geo["box"][:, 3:] - geo["box"][:, :3] + 1, 0, None).astype(np.int64)
+    assert st["pairs"] == int(ext.prod(1).sum())
+    assert st["skipped_gaussians"] == int((geo["flags"] & 1).sum())
+    # expected key multiset from the oracle boxes
+    b = geo["box"].astype(np.int64)
+    nbk = (b[:, 3:] >> 3) - (b[:, :3] >> 3) + 1
+    nbk[~live] = 0
+    assert st["keys_needed"] == int(nbk.prod(1).sum())
+    start, keys = plan.bins()
+    assert start[0] == 0 and start[-1] == st["keys_needed"] and np.all(np.diff(start) >= 0)
+    nb = [(d + 7) // 8 for d in case.dims]
+    brick_of_key = np.repeat(np.arange(len(start) - 1), np.diff(start))
+    got = set(zip(brick_of_key.tolist(), keys.tolist()))
+    assert len(got) == len(keys), "duplicate (brick, Gaussian) keys"
+    if case.n <= 5000:
+        exp = set()
+        for g in np.flatnonzero(live):
+            for bz in range(b[g, 2] >> 3, (b[g, 5] >> 3) + 1):
+                for by in range(b[g, 1] >> 3, (b[g, 4] >> 3) + 1):
+                    for bx in range(b[g, 0] >> 3, (b[g, 3] >> 3) + 1):
+                        exp.add(((bz * nb[1] + by) * nb[0] + bx, int(g)))
+        assert got == exp
+    return st
+
+
+def full_parity(pkg, case, **kw):
+    g = case.grad_out()
+    plan, out, grads = run_gpu(pkg, case, grad=g, **kw)
+    st = check_geometry_and_bins(plan, case)
+    assert not st["overflow"]
+    ref = oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid)
+    check_forward(out, ref)
+    refs = oracle.backward(case.pos, case.scale, case.quat, case.weight, case.grid, g)
+    check_grads(grads, refs)
+    return plan
+
+
+# ------------------------------------------------------------------ small / medium cases
+def test_config1_tiny_full(pkg):
+    full_parity(pkg, gsvox_inputs.config1())
+
+
+def test_subvolume_anisotropic_spacing_three_channels(pkg):
+    """Ragged dims (37,29,21), non-zero origin, spacing (2,1.5,0.75), unnormalised quaternions,
+    C = 3, most Gaussians partly outside: the arguments PAPER.md:128-136 exercise."""
+    full_parity(pkg, gsvox_inputs.subvolume_case())
+
+
+@pytest.mark.parametrize("channels", [2, 4, 5, 9, 13])
+def test_channel_counts(pkg, channels):
+    full_parity(pkg, gsvox_inputs.subvolume_case(n=300, channels=channels, seed=20 + channels))
+
+
+@pytest.mark.parametrize("level,n", [(1, 60), (2, 400), (3, 3000)])
+def test_config3_levels_reduced(pkg, level, n):
+    """Config 3 recipe (C = 9, 128x128x64) at a reduced Gaussian count so the oracle stays in seconds."""
+    full_parity(pkg, gsvox_inputs.config3(level, n=n))
+
+
+def test_config4_recipe_reduced(pkg):
+    full_parity(pkg, gsvox_inputs.config4(n=20000, dims=(96, 88, 72)))
+
+
+def test_config5_recipe_reduced_needles_and_blobs(pkg):
+    full_parity(pkg, gsvox_inputs.config5(n=20000, dims=(128, 96, 64)))
+
+
+def test_narrow_and_wide_gaussians(pkg):
+    """Scales from 0.15 voxel (sub-voxel, direct-exponential path, mostly empty boxes) to 40 voxels."""
+    rng = np.random.default_rng(77)
+    n, dims = 1500, (50, 44, 38)
+    case = gsvox_inputs.config1(n=n, dims=dims, seed=77)
+    case.scale[:] = np.exp(rng.uniform(np.log(0.15), np.log(40.0), (n, 3))).astype(np.float32)
+    case.scale[:200] = np.exp(rng.uniform(np.log(0.15), np.log(0.9), (200, 3))).astype(np.float32)
+    full_parity(pkg, case)
+
+
+def test_single_isolated_gaussians_worst_case_tolerance(pkg):
+    """max|out| = w: the tolerance is relative to ONE Gaussian's peak, the hardest case for the
+    row recurrence.  Sweeps sub-voxel offsets, scales around the recurrence/direct switch, rotations."""
+    rng = np.random.default_rng(5)
+    dims = (40, 40, 40)
+    for s0 in (0.5, 0.8, 0.84, 0.86, 1.0, 1.3, 2.0, 4.5):
+        for rep in range(4):
+            case = gsvox_inputs.config1(n=1, dims=dims, seed=1000 + rep)
+            case.pos[:] = (19.5 + rng.uniform(-4, 4, 3)).astype(np.float32)
+            case.scale[:] = (s0 * np.exp(rng.uniform(-0.1, 0.1, 3))).astype(np.float32)
+            case.weight[:] = 1.0
+            plan, out, _ = run_gpu(pkg, case)
+            ref = oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid)
+            check_forward(out, ref)
+
+
+def test_far_grid_coordinates_keep_accuracy(pkg):
+    """A sub-grid far from the world origin with fine spacing: index-space centres ~3e4 voxels
+    are split into integer + fraction, so brick-local coordinates stay accurate."""
+    case = gsvox_inputs.subvolume_case(n=400, dims=(48, 40, 36), channels=1, seed=31,
+                                       origin=(1000.0, -2000.0, 512.0), spacing=(0.5, 0.25, 0.125))
+    case.scale[:] *= 0.3
+    full_parity(pkg, case)
+
+
+# --------------------------------------------------------------------------- edge cases
+def test_degenerate_empty_and_outside(pkg):
+    case = gsvox_inputs.config1(n=64, dims=(24, 20, 18), seed=3)
+    case.scale[1, 2] = 0.0; case.scale[2, 0] = -1.0; case.quat[3] = 0.0
+    case.pos[4, 1] = np.nan; case.scale[5, 1] = np.inf; case.pos[6] = (-500, 5, 5)
+    case.scale[7] = 0.05; case.pos[7] = (5.5, 5.5, 5.5)
+    g = case.grad_out()
+    plan, out, grads = run_gpu(pkg, case, grad=g)
+    st = check_geometry_and_bins(plan, case)
+    assert st["skipped_gaussians"] == 5
+    ref = oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid)
+    check_forward(out, ref)
+    refs = oracle.backward(case.pos, case.scale, case.quat, case.weight, case.grid, g)
+    check_grads(grads, refs)
+    for a in grads:
+        assert np.isfinite(a).all() and not a[1:8].any()
+
+
+def test_zero_gaussians_writes_zeros(pkg):
+    case = gsvox_inputs.config1(n=0, dims=(17, 9, 10))
+    plan = pkg.Plan(4, case.grid)
+    plan.preprocess(dev(case.pos.reshape(0, 3)), dev(case.scale.reshape(0, 3)), dev(case.quat.reshape(0, 4)))
+    out = torch.full((1, 10, 9, 17), 7.0, device="cuda")
+    plan.forward(dev(case.weight.reshape(0, 1)), out=out)
+    torch.cuda.synchronize()
+    assert not out.cpu().numpy().any()
+    assert plan.status()["keys_needed"] == 0
+
+
+def test_key_overflow_is_reported_and_outputs_are_zero(pkg):
+    case = gsvox_inputs.config1(n=500, dims=(32, 32, 32), seed=9)
+    g = case.grad_out()
+    plan, out, grads = run_gpu(pkg, case, grad=g, key_capacity=100)
+    st = plan.status()
+    assert st["overflow"] and st["keys_needed"] > 100
+    assert not out.any() and all(not a.any() for a in grads)
+    plan2, out2, _ = run_gpu(pkg, case, key_capacity=st["keys_needed"])
+    assert not plan2.status()["overflow"]
+    check_forward(out2, oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid))
+
+
+def test_plan_reuse_across_steps_and_weight_changes(pkg):
+    """The plan is rebuilt every training step (parameters change each
+    iteration); weights may change between forward calls without a new preprocess."""
+    a = gsvox_inputs.config1(n=800, dims=(40, 36, 28), seed=1)
+    b = gsvox_inputs.config1(n=650, dims=(40, 36, 28), seed=2)
+    plan = pkg.Plan(800, a.grid)
+    for case in (a, b, a):
+        plan.preprocess(dev(case.pos), dev(case.scale), dev(case.quat))
+        out = plan.forward(dev(case.weight)).cpu().numpy()
+        check_forward(out, oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid))
+    w2 = (-2.0 * a.weight).astype(np.float32)
+    out = plan.forward(dev(w2)).cpu().numpy()
+    check_forward(out, oracle.forward(a.pos, a.scale, a.quat, w2, a.grid))
+
+
+def test_forward_is_run_to_run_stable_within_tolerance(pkg):
+    case = gsvox_inputs.config1(n=3000, dims=(48, 48, 48), seed=4)
+    _, o1, g1 = run_gpu(pkg, case, grad=case.grad_out())
+    _, o2, g2 = run_gpu(pkg, case, grad=case.grad_out())
+    assert np.abs(o1 - o2).max() <= 1e-6 * np.abs(o1).max()
+    for x, y in zip(g1, g2):
+        assert np.linalg.norm(x - y) <= 1e-5 * np.linalg.norm(x)
+
+
+def test_host_buffer_step_matches_device_path(pkg):
+    case = gsvox_inputs.config1(n=1200, dims=(40, 32, 24), seed=6)
+    g = case.grad_out()
+    plan = pkg.Plan(case.n, case.grid)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    out = torch.empty((1, 24, 32, 40)).pin_memory()
+    grads = tuple(torch.empty((case.n, k)).pin_memory() for k in (1, 3, 3, 4))
+    plan.step_host(pin(case.pos), pin(case.scale), pin(case.quat), pin(case.weight), pin(g), out, grads)
+    check_forward(out.numpy(), oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid))
+    check_grads([t.numpy() for t in grads],
+                oracle.backward(case.pos, case.scale, case.quat, case.weight, case.grid, g))
+
+
+# ------------------------------------------------- BASELINE.json configs at full size
+# The oracle finishes every full-size config in seconds on the GPU box's host cores, so the
+# comparison is element by element over the whole volume and every Gaussian, not sampled.
+def test_config2_cbct_full_size(pkg):
+    full_parity(pkg, gsvox_inputs.config2())
+
+
+@pytest.mark.parametrize("level", [1, 2, 3])
+def test_config3_dvf_full_size(pkg, level):
+    full_parity(pkg, gsvox_inputs.config3(level))
+
+
+def test_config4_training_step_full_size(pkg):
+    full_parity(pkg, gsvox_inputs.config4())
+
+
+def test_config5_stress_full_size(pkg):
+    full_parity(pkg, gsvox_inputs.config5())
