@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of the gsvox hot path (preprocess + forward + backward).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+Workload: BASELINE.json configs[3], "Training step at scale": 256^3 fp32 grid, 500k Gaussians,
+C = 1, upstream gradient N(0,1); one step = gsvox_preprocess + gsvox_forward + gsvox_backward
+(binning included: Gaussian parameters change every training step).
+Metric: Gaussian-voxel evaluations per second = P_def (pairs inside the 3-sigma box cutoff, the
+oracle's loop count) / time of one forward+backward step; whole-job aggregate over N GPUs.
+Multi-GPU: the path does not shard in this build ("replicas only"): each rank runs an
+independent replica of the step; no data-path collective.  Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np
+
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.4: SMs x FP32 lanes x FMA x max SM clock
+METRIC = "gaussian_voxel_evals_per_s_fwd_bwd"
+UNIT = "pairs/s"
+
+
+def flops_per_pair(channels):
+    """Canonical algorithmic flops per (Gaussian, voxel) pair."""
+    return 18 + 2 * channels, 58 + 4 * channels
+
+
+def get_case(cfg):
+    import gsvox_inputs
+    if cfg == 4:
+        return gsvox_inputs.config4()
+    if cfg == 1:
+        return gsvox_inputs.config1()
+    if cfg == 2:
+        return gsvox_inputs.config2()
+    if cfg == 5:
+        return gsvox_inputs.config5()
+    if cfg in (31, 32, 33):
+        return gsvox_inputs.config3(cfg - 30)
+    raise SystemExit("unknown --config %r" % cfg)
+
+
+def workload_config(case, extra=None):
+    c = {"workload": case.name, "grid": list(case.dims), "gaussians": case.n, "channels": case.channels,
+         "step": "gsvox_preprocess+gsvox_forward+gsvox_backward", "parallelism": "replicas",
+         "l2_policy": "working set > L2 (volume + gradient + keys + records ~250 MB vs 126 MB L2), no flush"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clock/throttle sampling during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, uuid):
+        self.proc = None
+        self.lines = []
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", uuid, "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                clk, cmax = float(f[0]), float(f[1])
+            except ValueError:
+                continue
+            mx.append(cmax)
+            if t0 - 0.02 <= ts <= t1 + 0.08:
+                sm.append(clk)
+                try:
+                    power.append(float(f[2]))
+                except ValueError:
+                    pass
+                for nm, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+        if not sm:                                   # region shorter than a sample: take the nearest
+            sm = [float(l.split(",")[0]) for _, l in self.lines[-2:]] if self.lines else []
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "power_w_max": max(power) if power else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------ reference arm
+def oracle_step(case, ids, grad):
+    import oracle
+    sub = lambda a: np.ascontiguousarray(a[ids])
+    t0 = time.perf_counter()
+    _, pairs = oracle.forward(sub(case.pos), sub(case.scale), sub(case.quat), sub(case.weight), case.grid,
+                              return_pairs=True)
+    oracle.backward(sub(case.pos), sub(case.scale), sub(case.quat), sub(case.weight), case.grid, grad)
+    return time.perf_counter() - t0, pairs
+
+
+def run_reference(args):
+    """The oracle as it stands, on the host cores, on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    case = get_case(args.config)
+    grad = case.grad_out()
+    # size the sample so the whole run ends within a few minutes: probe 2% of the Gaussians
+    probe = np.arange(0, case.n, 50)
+    dt, pairs = oracle_step(case, probe, grad)
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    frac = min(1.0, max(0.002, 0.02 * budget / max(dt, 1e-3)))
+    stride = max(1, int(round(1.0 / frac)))
+    ids = np.arange(0, case.n, stride)
+    for _ in range(args.warmup):
+        oracle_step(case, ids, grad)
+    total, pairs = 0.0, 0
+    for _ in range(args.steps):
+        dt, pairs = oracle_step(case, ids, grad)
+        total += dt
+    ms = 1e3 * total / args.steps
+    value = pairs / (ms * 1e-3)
+    sample = "every %d-th Gaussian of %s (%d of %d, %d pairs), full grid, forward+backward" % (
+        stride, case.name, ids.size, case.n, pairs)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(case, {"sample": sample}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2503_22139_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    pkg.lib()
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    case = get_case(args.config)
+    C = case.channels
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    pos, scale, quat, w = dev(case.pos), dev(case.scale), dev(case.quat), dev(case.weight)
+    grad_np = case.grad_out()
+    grad = dev(grad_np)
+    nx, ny, nz = case.dims
+
+    plan = pkg.Plan(case.n, case.grid, max_channels=C)
+    plan.preprocess(pos, scale, quat)
+    st = plan.status()
+    if st["overflow"]:
+        plan = pkg.Plan(case.n, case.grid, max_channels=C, key_capacity=int(1.05 * st["keys_needed"]))
+        plan.preprocess(pos, scale, quat)
+        st = plan.status()
+    assert not st["overflow"]
+    pairs, keys = st["pairs"], st["keys_needed"]
+    out = torch.empty((C, nz, ny, nx), dtype=torch.float32, device="cuda")
+    grads = tuple(torch.empty((case.n, k), dtype=torch.float32, device="cuda") for k in (C, 3, 3, 4))
+
+    def step():
+        plan.preprocess(pos, scale, quat)
+        plan.forward(w, out=out)
+        plan.backward(w, grad, grads=grads)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    uuid = str(torch.cuda.get_device_properties(local).uuid)
+    sampler = ClockSampler("GPU-" + uuid if not uuid.startswith("GPU-") else uuid)
+    time.sleep(0.15)
+    _, l0 = plan.timings(reset=True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.time()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    ms_total = ev0.elapsed_time(ev1)
+    _, launches = plan.timings(reset=True)
+    n_launch = sum(launches.values())
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    value = world * pairs / (ms_step * 1e-3)
+
+    line = None
+    if rank == 0:
+        # ---- per-kernel durations: the same loop again with the library's event brackets on
+        plan.set_timing(True)
+        for _ in range(args.steps):
+            step()
+        kms, kcnt = plan.timings(reset=True)
+        plan.set_timing(False)
+        per_step = {k: kms[k] / args.steps for k in kms}
+        f_fwd, f_bwd = flops_per_pair(C)
+        dom = "backward" if per_step["backward"] >= per_step["forward"] else "forward"
+        dom_ms = kms[dom] / max(1, kcnt[dom])
+        dom_flops = pairs * (f_bwd if dom == "backward" else f_fwd)
+        achieved = dom_flops / (dom_ms * 1e-3) / 1e12
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(case.name, {}).get(dom)
+            except Exception:
+                traffic = None
+        roofline = {"bound": "alu", "kernel": "k_" + dom, "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
+                    "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
+                    "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); no FP32 entry in MEASURED_PEAKS.json",
+                    "flops_per_pair": f_bwd if dom == "backward" else f_fwd, "pairs": pairs,
+                    "kernel_ms": dom_ms, "kernel_ms_per_step": per_step,
+                    "step_canonical_tflops": pairs * (f_fwd + f_bwd) / (ms_step * 1e-3) / 1e12,
+                    "step_frac": pairs * (f_fwd + f_bwd) / (ms_step * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}
+
+        # ---- end to end through the C ABI with HOST (pinned) buffers
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hp, hs, hq, hw, hg = pin(case.pos), pin(case.scale), pin(case.quat), pin(case.weight), pin(grad_np)
+        hout = torch.empty((C, nz, ny, nx), dtype=torch.float32).pin_memory()
+        hgr = tuple(torch.empty((case.n, k), dtype=torch.float32).pin_memory() for k in (C, 3, 3, 4))
+        e2e_steps = max(3, min(args.steps, 20))
+        for _ in range(3):
+            plan.step_host(hp, hs, hq, hw, hg, hout, hgr)
+        torch.cuda.synchronize()
+        e0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            plan.step_host(hp, hs, hq, hw, hg, hout, hgr)
+        torch.cuda.synchronize()
+        e_ms = 1e3 * (time.perf_counter() - e0) / e2e_steps
+        h2d = sum(t_.numel() * 4 for t_ in (hp, hs, hq, hw, hg))
+        d2h = hout.numel() * 4 + sum(t_.numel() * 4 for t_ in hgr)
+        e2e = {"value": world * pairs / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms, "steps": e2e_steps,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "note": "gsvox_step_host: pinned host buffers in and out, copies inside the timed region"}
+
+        # ---- the oracle beside it, bounded sample, host cores
+        cpu = None
+        if not args.no_cpu_baseline:
+            import oracle
+            stride = 1 if case.n <= 600_000 else 4
+            ids = np.arange(0, case.n, stride)
+            dt, cp = oracle_step(case, ids, grad_np)
+            cpu = {"value": cp / dt, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+                   "seconds": dt, "sample": "every %d-th Gaussian of %s (%d pairs), full grid, forward+backward, fp64"
+                   % (stride, case.name, cp)}
+
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": workload_config(case, {"pairs_P_def": pairs, "keys": keys}),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=4, help="4 (headline), 1, 2, 5, or 31/32/33 for config 3 levels")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
