@@ -58,6 +58,23 @@ def workload_config(case, extra=None):
     return c
 
 
+def read_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    committed `ncu --set full` capture (profiles/traffic.csv); None if not captured."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    best = None
+    for ln in open(path):
+        f = [x.strip() for x in ln.split(",")]
+        if len(f) >= 4 and f[0] == workload and f[1] == kernel:
+            try:
+                best = float(f[2]) + float(f[3])
+            except ValueError:
+                pass
+    return best
+
+
 # ------------------------------------------------------------------------------- clocks
 class ClockSampler:
     """nvidia-smi clock/throttle sampling during the timed region (B200_PROFILING.md recipe)."""
@@ -164,23 +181,16 @@ def run_reference(args):
 # ------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import torch
-    import torch.distributed as dist
     import paper_2503_22139_b200 as pkg
+    from paper_2503_22139_b200.dist import Ranks, whole_job_rate
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     pkg.lib()
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    ranks = Ranks(backend="nccl")
+    rank, world, local = ranks.rank, ranks.world, ranks.local
+    barrier = ranks.barrier
 
     case = get_case(args.config)
     C = case.channels
@@ -227,11 +237,7 @@ def run_ours(args):
     ms_total = ev0.elapsed_time(ev1)
     _, launches = plan.timings(reset=True)
     n_launch = sum(launches.values())
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
-    value = world * pairs / (ms_step * 1e-3)
+    value, ms_step = whole_job_rate(pairs, ranks, ms_total, args.steps)
 
     line = None
     if rank == 0:
@@ -247,13 +253,7 @@ def run_ours(args):
         dom_ms = kms[dom] / max(1, kcnt[dom])
         dom_flops = pairs * (f_bwd if dom == "backward" else f_fwd)
         achieved = dom_flops / (dom_ms * 1e-3) / 1e12
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tpath):
-            try:
-                traffic = json.load(open(tpath)).get(case.name, {}).get(dom)
-            except Exception:
-                traffic = None
+        traffic = read_traffic(case.name, dom)
         roofline = {"bound": "alu", "kernel": "k_" + dom, "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
                     "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); no FP32 entry in MEASURED_PEAKS.json",
@@ -298,9 +298,7 @@ def run_ours(args):
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": workload_config(case, {"pairs_P_def": pairs, "keys": keys}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu}
-    if world > 1:
-        dist.barrier()
-        dist.destroy_process_group()
+    ranks.close()
     if line is not None:
         print(json.dumps(line), flush=True)
 

@@ -1,0 +1,57 @@
+"""Multi-GPU plumbing of bench.py: one process per GPU, "replicas only" (section
+multi-GPU): every rank runs an independent replica of the step on its own GPU, there is no
+data-path collective.  torch.distributed is used for the rendezvous, the barriers around the timed
+region and the max-over-ranks reduction of the device time.  Backend nccl on GPUs, gloo in the CPU
+tests (tests/test_dist_gloo.py, world_size 2)."""
+import os
+
+import torch
+import torch.distributed as dist
+
+
+class Ranks:
+    def __init__(self, backend=None):
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.backend = backend or ("nccl" if torch.cuda.is_available() else "gloo")
+        self.on = self.world > 1
+        if self.on and not dist.is_initialized():
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            kw = {}
+            if self.backend == "nccl":
+                kw["device_id"] = torch.device("cuda", self.local)
+            dist.init_process_group(self.backend, rank=self.rank, world_size=self.world, **kw)
+
+    def _dev(self):
+        return torch.device("cuda", self.local) if self.backend == "nccl" else torch.device("cpu")
+
+    def barrier(self):
+        if self.on:
+            dist.barrier()
+        if self.backend == "nccl" and torch.cuda.is_available():
+            torch.cuda.synchronize()
+
+    def max_over_ranks(self, value):
+        t = torch.tensor([float(value)], dtype=torch.float64, device=self._dev())
+        if self.on:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(self, value):
+        t = torch.tensor([float(value)], dtype=torch.float64, device=self._dev())
+        if self.on:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    def close(self):
+        if self.on and dist.is_initialized():
+            dist.barrier()
+            dist.destroy_process_group()
+
+
+def whole_job_rate(units_per_rank, ranks, ms_total, steps):
+    """value = units all ranks processed / max-over-ranks time (weak scaling, replicas)."""
+    ms_step = ranks.max_over_ranks(ms_total) / steps
+    total_units = ranks.sum_over_ranks(units_per_rank)
+    return total_units / (ms_step * 1e-3), ms_step

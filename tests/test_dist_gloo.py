@@ -1,0 +1,61 @@
+"""CPU test (gloo, world_size 2) of the N>1 host logic bench.py uses: rendezvous on 127.0.0.1,
+barriers, max-over-ranks of the device time, whole-job aggregate (replicas, weak scaling)."""
+import os
+import socket
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+from paper_2503_22139_b200.dist import Ranks, whole_job_rate
+r = Ranks(backend="gloo")
+r.barrier()
+ms_total = 100.0 if r.rank == 0 else 250.0           # rank 1 is the slow replica
+value, ms_step = whole_job_rate(1000.0 * (r.rank + 1), r, ms_total, steps=10)
+mx = r.max_over_ranks(r.rank * 7.0)
+r.close()
+print(json.dumps({"rank": r.rank, "world": r.world, "value": value, "ms_step": ms_step, "mx": mx}))
+"""
+
+
+def free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def test_two_rank_gloo_max_time_and_aggregate():
+    import json
+    port = free_port()
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", LOCAL_RANK=str(rank),
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, "-c", WORKER % ROOT], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = []
+    for p in procs:
+        o, e = p.communicate(timeout=120)
+        assert p.returncode == 0, e[-2000:]
+        outs.append(json.loads(o.strip().splitlines()[-1]))
+    for o in outs:
+        assert o["world"] == 2
+        assert o["ms_step"] == 25.0                      # max over ranks (250 ms / 10 steps)
+        assert abs(o["value"] - 3000.0 / 0.025) < 1e-6   # all ranks' units / max time
+        assert o["mx"] == 7.0
+
+
+def test_single_process_needs_no_process_group():
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    code = ("import sys; sys.path.insert(0, %r)\n"
+            "from paper_2503_22139_b200.dist import Ranks, whole_job_rate\n"
+            "r = Ranks(backend='gloo'); v, ms = whole_job_rate(500.0, r, 50.0, 5); r.close(); print(v, ms)") % ROOT
+    out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0, out.stderr[-2000:]
+    v, ms = out.stdout.split()
+    assert float(ms) == 10.0 and abs(float(v) - 50000.0) < 1e-9
