@@ -57,7 +57,7 @@ static bool grid_ok(const gsvox_grid* g)
     return true;
 }
 
-struct Layout { size_t status, rec, aux, bin_count, bin_start, scan_partial, keys, acc, total; int nbins, nb[3]; };
+struct Layout { size_t status, rec, aux, bin_count, bin_start, scan_partial, keys, acc, total; int nbins, nbricks, nb[3]; };
 
 static size_t up256(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -69,6 +69,8 @@ static int make_layout(int64_t n_max, int32_t max_channels, const gsvox_grid* g,
     if (n_max > 0x7ffffff0LL / 8 || key_capacity > 0xfffffff0LL) return GSVOX_ELIMIT;
     int64_t nbins = 1;
     for (int k = 0; k < 3; ++k) { L->nb[k] = (g->dims[k] + kBrick - 1) / kBrick; nbins *= L->nb[k]; }
+    L->nbricks = (int)nbins;
+    nbins *= kNumClasses;
     if (nbins > 0x7ffffff0LL) return GSVOX_ELIMIT;
     L->nbins = (int)nbins;
     size_t off = 0;
@@ -114,7 +116,7 @@ extern "C" int gsvox_plan_create(int64_t n_max, int32_t max_channels, const gsvo
         p->gd.origin[k] = (double)grid->origin[k]; p->gd.spacing[k] = (double)grid->spacing[k];
         p->gd.dims[k] = grid->dims[k]; p->gd.nb[k] = L.nb[k];
     }
-    p->gd.nbricks = L.nbins;
+    p->gd.nbricks = L.nbricks;
     p->n_max = n_max; p->max_channels = max_channels; p->key_capacity = key_capacity; p->n = -1;
     char* w = (char*)workspace;
     p->status = (DevStatus*)(w + L.status); p->rec = (GsRec*)(w + L.rec); p->aux = (GsAux*)(w + L.aux);

@@ -22,7 +22,6 @@ namespace gsvox {
 
 constexpr int kFwdThreads = 64;
 constexpr int kFwdBatch = 64;
-constexpr float kRecurrenceMaxA = 1.0f;
 
 __device__ __forceinline__ float ex2f(float x)
 {
@@ -93,7 +92,7 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
         for (int k = 0; k < 8; ++k) acc[ch][k] = 0.f;
 
     uint32_t kbeg = 0, kend = 0;
-    if (!status->overflow) { kbeg = bin_start[b]; kend = bin_start[b + 1]; }
+    if (!status->overflow) { kbeg = bin_start[b * kNumClasses]; kend = bin_start[(b + 1) * kNumClasses]; }
 
     int buf = 0;
     for (uint32_t base = kbeg; base < kend; base += kFwdBatch, buf ^= 1) {
@@ -188,10 +187,10 @@ static int launch_fwd_ch(gsvox_plan* p, const float* weight, int C, int c0, floa
     LaunchScope ls(p, GSVOX_K_FORWARD, st);
     bool vec = (p->gd.dims[0] % 4 == 0) && (((uintptr_t)out & 15) == 0);
     if (vec)
-        k_forward<CH, true><<<p->nbins, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
+        k_forward<CH, true><<<p->gd.nbricks, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
                                                                weight, C, c0, out, p->gd);
     else
-        k_forward<CH, false><<<p->nbins, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
+        k_forward<CH, false><<<p->gd.nbricks, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
                                                                 weight, C, c0, out, p->gd);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;

@@ -77,7 +77,7 @@ extern "C" int gsvox_plan_bins_host(gsvox_plan* p, int64_t* brick_start_host, in
     std::vector<uint32_t> hs((size_t)p->nbins + 1);
     GSVOX_CUDA(cudaMemcpyAsync(hs.data(), p->bin_start, hs.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
     GSVOX_CUDA(cudaStreamSynchronize(st));
-    for (size_t i = 0; i < hs.size(); ++i) brick_start_host[i] = (int64_t)hs[i];
+    for (int i = 0; i <= p->gd.nbricks; ++i) brick_start_host[i] = (int64_t)hs[(size_t)i * kNumClasses];
     int64_t total = (int64_t)hs[p->nbins];
     if (key_gaussian_host) {
         if (total > key_host_capacity || total > p->key_capacity) return GSVOX_EWORKSPACE;

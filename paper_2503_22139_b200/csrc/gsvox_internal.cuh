@@ -61,6 +61,20 @@ struct GridDev {
 constexpr int kBrick = GSVOX_BRICK;
 constexpr int kBrickVox = kBrick * kBrick * kBrick;
 constexpr int kScanItemsPerBlock = 2048;     // k_scan_*: 256 threads x 8 items
+constexpr float kRecurrenceMaxA = 1.0f;      // rows with A > 1 (narrow along x) take one EX2 per voxel
+
+// Bins of the counting sort are (brick, class): inside a brick, keys are ordered so that the 32
+// keys a backward warp works on have similar trip counts and the same code path (a4 runs one
+// THREAD per key).  class 0: direct-exponential keys (A > kRecurrenceMaxA); 1..8: keys whose box
+// covers only part of the brick's x extent, by decreasing row count; 9..16: x-full keys, same.
+constexpr int kNumClasses = 17;
+__host__ __device__ __forceinline__ int key_class(bool direct, int x0, int x1, int y0, int y1, int z0, int z1)
+{
+    if (direct) return 0;
+    const int nrows = (y1 - y0 + 1) * (z1 - z0 + 1);
+    const int rc = 7 - ((nrows - 1) >> 3);
+    return 1 + ((x0 == 0 && x1 == 7) ? 8 : 0) + rc;
+}
 
 inline __host__ __device__ int acc_stride(int channels) { return (9 + channels + 3) & ~3; }
 
@@ -78,7 +92,7 @@ struct gsvox_plan {
     gsvox::DevStatus* status;
     gsvox::GsRec* rec;
     gsvox::GsAux* aux;
-    uint32_t* bin_count;       // [nbins+1]  counts, then write cursors
+    uint32_t* bin_count;       // [nbins+1]  counts, then write cursors; nbins = nbricks * kNumClasses
     uint32_t* bin_start;       // [nbins+1]  exclusive scan of counts
     uint32_t* scan_partial;    // [scan blocks]
     uint32_t* keys;            // [key_capacity] Gaussian id per key, grouped by brick
@@ -113,5 +127,6 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st);
 int launch_forward(gsvox_plan* p, const float* weight, int channels, float* out, cudaStream_t st);
 int launch_backward(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
                     float* gw, float* gp, float* gs, float* gq, cudaStream_t st);
+int launch_epilogue(gsvox_plan* p, int channels, float* gw, float* gp, float* gs, float* gq, cudaStream_t st);
 
 }  // namespace gsvox

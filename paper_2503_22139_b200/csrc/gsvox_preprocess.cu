@@ -4,8 +4,8 @@
 //     steps 1-5 (Eq. 4; Sigma = R S S^T R^T per north_star).  The box bounds use
 //     the operation order of reading A5 with explicitly rounded intrinsics (__dmul_rn, ...),
 //     so no FMA contraction can change an integer bound.
-// a2  counting sort of (brick, Gaussian) keys by brick: k_count -> 3-kernel exclusive scan ->
-//     k_scatter.  Order inside a brick is whatever the atomics produce (sums are order
+// a2  counting sort of (brick, Gaussian) keys by (brick, class): k_keys<0> -> 3-kernel exclusive
+//     scan -> k_keys<1>.  Order inside a brick is whatever the atomics produce (sums are order
 //     independent within tolerance, reading A13).
 #include "gsvox_internal.cuh"
 
@@ -148,6 +148,7 @@ k_keys(const GsRec* __restrict__ rec, int n, GridDev gd, uint32_t* __restrict__ 
     if (g >= n) return;
     const int4* rp = reinterpret_cast<const int4*>(rec + g);
     int4 w3 = __ldg(rp + 3);                      // bytes 48..63: nD2, lo[3], hi[3]
+    const bool direct = -__int_as_float(__ldg(rp + 1).w) > kRecurrenceMaxA;      // negA at byte 28
     int lox = (int16_t)(w3.y & 0xffff), loy = (int16_t)(w3.y >> 16);
     int loz = (int16_t)(w3.z & 0xffff), hix = (int16_t)(w3.z >> 16);
     int hiy = (int16_t)(w3.w & 0xffff), hiz = (int16_t)(w3.w >> 16);
@@ -157,7 +158,10 @@ k_keys(const GsRec* __restrict__ rec, int n, GridDev gd, uint32_t* __restrict__ 
     int total = ex * ey * ez;
     for (int t = sub; t < total; t += 8) {
         int tx = t % ex, r = t / ex, ty = r % ey, tz = r / ey;
-        int b = ((bz0 + tz) * gd.nb[1] + (by0 + ty)) * gd.nb[0] + (bx0 + tx);
+        const int bx = bx0 + tx, by = by0 + ty, bz = bz0 + tz;
+        const int cls = key_class(direct, max(lox - 8 * bx, 0), min(hix - 8 * bx, 7), max(loy - 8 * by, 0),
+                                  min(hiy - 8 * by, 7), max(loz - 8 * bz, 0), min(hiz - 8 * bz, 7));
+        int b = ((bz * gd.nb[1] + by) * gd.nb[0] + bx) * kNumClasses + cls;
         if (MODE == 0) atomicAdd(&bin_count[b], 1u);
         else { uint32_t slot = atomicAdd(&bin_count[b], 1u); keys[slot] = (uint32_t)g; }
     }
