@@ -4,18 +4,20 @@
 // i.e. 8 consecutive voxels per channel, accumulated in registers and written once.  The brick's
 // keys are staged 64 at a time into shared memory: each thread gathers one 64-byte Gaussian
 // record (four LDG.128, L2-resident: a record is shared by ~20 bricks), rebases the centre to
-// brick-local coordinates and derives the brick-local row mask (which of the 64 rows lie inside
-// the Gaussian's box in y,z) and x mask.  Warps then walk the staged batch; a warp whose 32 rows
-// miss the box skips the key.
+// brick-local coordinates and derives the brick-local row masks (which of the 64 rows lie inside
+// the Gaussian's box in y,z) and, for C = 1, the eight per-voxel weights w·[k inside the box in x],
+// so that full and x-partial keys run the same branch-free code.  Warps then walk the staged
+// batch; a warp whose 32 rows miss the box skips the key.
 //
 // Along a row the exponent of Eq. 4 is the parabola E(k) = Es - A (k - xs)^2 (base 2), with
 // xs, Es from the LDL^T form of the record (sum of squares, no cancellation).  For A <= 1 the
 // eight values are produced by a centre-out multiplicative recurrence from k = 3:
 //     G(k+1) = G(k) r(k),  r(k+1) = r(k) c,  c = 2^(-2A)      (exact identity for a parabola)
-// 3 MUFU.EX2 + 14 FMUL per row instead of 8 MUFU: the kernel is then FMA-pipe bound, not
+// 3 MUFU.EX2 + 14 FMUL per row instead of 8 MUFU: the kernel is then FMA/issue bound, not
 // MUFU bound (16 vs 128 lanes/clk/SM).  Narrow Gaussians (A > 1, under ~0.85 voxel along x)
 // take the direct path, one EX2 per voxel: the recurrence would lose accuracy and could
-// underflow there (error budget).
+// underflow there (error budget).  Direct keys are class 0 of the brick's
+// key range, so which path a staged key takes is known from bin_start, not from its data.
 #include "gsvox_internal.cuh"
 
 namespace gsvox {
@@ -30,9 +32,12 @@ __device__ __forceinline__ float ex2f(float x)
     return y;
 }
 
-template <int CH> struct FwdRec { static constexpr int kWords = (13 + CH + 3) & ~3; };
+// Shared-memory record of a staged key (floats):
+//   0 cx  1 cy  2 cz  3 -A | 4 -l01  5 -l02  6 l12  7 -D1 | 8 -D2  9 c  10 rowmask(z 0..3)  11 rowmask(z 4..7)
+//   CH == 1: 12..19  w * [k inside the box in x], k = 0..7
+//   CH  > 1: 12 xmask, 13..13+CH-1 weights
+template <int CH> struct FwdRec { static constexpr int kWords = (CH == 1) ? 20 : ((13 + CH + 3) & ~3); };
 
-// Stage key `k` of this brick into shared memory slot `dst`.
 template <int CH>
 __device__ __forceinline__ void stage_key(float* __restrict__ dst, const GsRec* __restrict__ rec,
                                           const float* __restrict__ weight, int wstride, int c0,
@@ -57,14 +62,72 @@ __device__ __forceinline__ void stage_key(float* __restrict__ dst, const GsRec* 
     uint32_t zh = zm >> 4;
     uint32_t sel1 = ((zh & 1u) ? 0xffu : 0u) | ((zh & 2u) ? 0xff00u : 0u) |
                     ((zh & 4u) ? 0xff0000u : 0u) | ((zh & 8u) ? 0xff000000u : 0u);
-    uint32_t flags = xm | ((-b.w > kRecurrenceMaxA) ? 0x100u : 0u);
     float4* o = reinterpret_cast<float4*>(dst);
     o[0] = make_float4((float)(cix - b0x) + a.x, (float)(ciy - b0y) + a.y, (float)(ciz - b0z) + a.z, b.w);
     o[1] = make_float4(c.x, c.y, c.z, c.w);
     o[2] = make_float4(d.x, a.w, __uint_as_float(rep & sel0), __uint_as_float(rep & sel1));
-    dst[12] = __uint_as_float(flags);
-    #pragma unroll
-    for (int ch = 0; ch < CH; ++ch) dst[13 + ch] = __ldg(weight + (size_t)gid * wstride + c0 + ch);
+    if (CH == 1) {
+        const float w = __ldg(weight + (size_t)gid * wstride + c0);
+        o[3] = make_float4((xm & 1u) ? w : 0.f, (xm & 2u) ? w : 0.f, (xm & 4u) ? w : 0.f, (xm & 8u) ? w : 0.f);
+        o[4] = make_float4((xm & 16u) ? w : 0.f, (xm & 32u) ? w : 0.f, (xm & 64u) ? w : 0.f, (xm & 128u) ? w : 0.f);
+    } else {
+        dst[12] = __uint_as_float(xm);
+        #pragma unroll
+        for (int ch = 0; ch < CH; ++ch) dst[13 + ch] = __ldg(weight + (size_t)gid * wstride + c0 + ch);
+    }
+}
+
+// One staged key against this thread's row.  DIRECT: one EX2 per voxel (narrow Gaussians).
+template <int CH, bool DIRECT>
+__device__ __forceinline__ void eval_key(const float* __restrict__ r, int wsel, uint32_t lanebit,
+                                         float fy, float fz, float (&acc)[CH][8])
+{
+    const uint32_t mrow = __float_as_uint(r[10 + wsel]);
+    if (mrow == 0u) return;                                         // none of this warp's 32 rows is in the box
+    const float4 r0 = *reinterpret_cast<const float4*>(r);
+    const float4 r1 = *reinterpret_cast<const float4*>(r + 4);
+    const float2 r2 = *reinterpret_cast<const float2*>(r + 8);
+    // row geometry: u2 = dz, u1 = dy + l12 dz, xs = cx - l01 dy - l02 dz
+    const float dy = fy - r0.y, dz = fz - r0.z;
+    const float u1 = fmaf(r1.z, dz, dy);
+    const float xs = fmaf(r1.y, dz, fmaf(r1.x, dy, r0.x));
+    float Es = fmaf(r2.x * dz, dz, (r1.w * u1) * u1);
+    Es = (mrow & lanebit) ? Es : -1.0e30f;                          // rows outside the box contribute exact zeros
+    const float negA = r0.w;
+    float G[8];
+    if (!DIRECT) {
+        // centre-out recurrence from k = 3
+        const float t3 = 3.0f - xs;
+        const float nAt = negA * t3;
+        const float Lf = fminf(fmaf(nAt, 2.0f, negA), 120.f);      // E(4) - E(3), clamped: 0 * inf would be NaN
+        const float Lb = fminf(fmaf(nAt, -2.0f, negA), 120.f);     // E(2) - E(3)
+        const float cc = r2.y;
+        G[3] = ex2f(fmaf(nAt, t3, Es));
+        float rf = ex2f(Lf), rb = ex2f(Lb);
+        G[4] = G[3] * rf; rf *= cc; G[5] = G[4] * rf; rf *= cc; G[6] = G[5] * rf; rf *= cc; G[7] = G[6] * rf;
+        G[2] = G[3] * rb; rb *= cc; G[1] = G[2] * rb; rb *= cc; G[0] = G[1] * rb;
+    } else {
+        #pragma unroll
+        for (int k = 0; k < 8; ++k) { const float t = (float)k - xs; G[k] = ex2f(fmaf(negA * t, t, Es)); }
+    }
+    if (CH == 1) {
+        const float4 wa = *reinterpret_cast<const float4*>(r + 12);
+        const float4 wb = *reinterpret_cast<const float4*>(r + 16);
+        acc[0][0] = fmaf(wa.x, G[0], acc[0][0]); acc[0][1] = fmaf(wa.y, G[1], acc[0][1]);
+        acc[0][2] = fmaf(wa.z, G[2], acc[0][2]); acc[0][3] = fmaf(wa.w, G[3], acc[0][3]);
+        acc[0][4] = fmaf(wb.x, G[4], acc[0][4]); acc[0][5] = fmaf(wb.y, G[5], acc[0][5]);
+        acc[0][6] = fmaf(wb.z, G[6], acc[0][6]); acc[0][7] = fmaf(wb.w, G[7], acc[0][7]);
+    } else {
+        const uint32_t xm = __float_as_uint(r[12]);
+        #pragma unroll
+        for (int k = 0; k < 8; ++k) G[k] = (xm & (1u << k)) ? G[k] : 0.f;
+        #pragma unroll
+        for (int ch = 0; ch < CH; ++ch) {
+            const float w = r[13 + ch];
+            #pragma unroll
+            for (int k = 0; k < 8; ++k) acc[ch][k] = fmaf(w, G[k], acc[ch][k]);
+        }
+    }
 }
 
 template <int CH, bool VEC>
@@ -83,7 +146,8 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
     const int b0x = bx * kBrick, b0y = by * kBrick, b0z = bz * kBrick;
     const int ry = tid & 7, rz = tid >> 3;
     const float fy = (float)ry, fz = (float)rz;
-    const int wsel = tid >> 5, lane = tid & 31;
+    const int wsel = tid >> 5;
+    const uint32_t lanebit = 1u << (tid & 31);
 
     float acc[CH][8];
     #pragma unroll
@@ -91,8 +155,11 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
         #pragma unroll
         for (int k = 0; k < 8; ++k) acc[ch][k] = 0.f;
 
-    uint32_t kbeg = 0, kend = 0;
-    if (!status->overflow) { kbeg = bin_start[b * kNumClasses]; kend = bin_start[(b + 1) * kNumClasses]; }
+    uint32_t kbeg = 0, kend = 0, kdirect = 0;
+    if (!status->overflow) {
+        kbeg = bin_start[b * kNumClasses]; kdirect = bin_start[b * kNumClasses + 1];
+        kend = bin_start[(b + 1) * kNumClasses];
+    }
 
     int buf = 0;
     for (uint32_t base = kbeg; base < kend; base += kFwdBatch, buf ^= 1) {
@@ -100,63 +167,12 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
         uint32_t k = base + tid;
         if (k < kend) stage_key<CH>(sb + tid * W, rec, weight, wstride, c0, keys[k], b0x, b0y, b0z);
         __syncthreads();
-        const int nb = min((uint32_t)kFwdBatch, kend - base);
-        for (int j = 0; j < nb; ++j) {
-            const float4* r = reinterpret_cast<const float4*>(sb + j * W);
-            const float4 r2 = r[2];
-            const uint32_t mrow = __float_as_uint(wsel ? r2.w : r2.z);
-            if (mrow == 0u) continue;                               // warp-uniform skip
-            const float4 r0 = r[0], r1 = r[1];
-            const uint32_t flags = __float_as_uint(sb[j * W + 12]);
-            const bool inside = (mrow >> lane) & 1u;
-            // row geometry: u2 = dz, u1 = dy + l12 dz, xs = cx - l01 dy - l02 dz
-            const float dy = fy - r0.y, dz = fz - r0.z;
-            const float u1 = fmaf(r1.z, dz, dy);
-            const float xs = fmaf(r1.y, dz, fmaf(r1.x, dy, r0.x));
-            const float Es = fmaf(r2.x * dz, dz, (r1.w * u1) * u1);
-            const float negA = r0.w;
-            float wv[CH];
-            #pragma unroll
-            for (int ch = 0; ch < CH; ++ch) wv[ch] = inside ? sb[j * W + 13 + ch] : 0.f;
-
-            if (!(flags & 0x100u)) {
-                // centre-out recurrence from k = 3
-                const float t3 = 3.0f - xs;
-                const float nAt = negA * t3;
-                const float E3 = fmaf(nAt, t3, Es);
-                const float Lf = fminf(fmaf(nAt, 2.0f, negA), 120.f);     // E(4) - E(3)
-                const float Lb = fminf(fmaf(nAt, -2.0f, negA), 120.f);    // E(2) - E(3)
-                const float cc = r2.y;
-                float G[8];
-                G[3] = ex2f(E3);
-                float rf = ex2f(Lf), rb = ex2f(Lb);
-                G[4] = G[3] * rf; rf *= cc; G[5] = G[4] * rf; rf *= cc; G[6] = G[5] * rf; rf *= cc; G[7] = G[6] * rf;
-                G[2] = G[3] * rb; rb *= cc; G[1] = G[2] * rb; rb *= cc; G[0] = G[1] * rb;
-                if ((flags & 0xffu) == 0xffu) {
-                    #pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2)
-                        #pragma unroll
-                        for (int ch = 0; ch < CH; ++ch) acc[ch][k2] = fmaf(wv[ch], G[k2], acc[ch][k2]);
-                } else {
-                    #pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2) {
-                        const float g = (flags & (1u << k2)) ? G[k2] : 0.f;
-                        #pragma unroll
-                        for (int ch = 0; ch < CH; ++ch) acc[ch][k2] = fmaf(wv[ch], g, acc[ch][k2]);
-                    }
-                }
-            } else {
-                // direct path: one EX2 per voxel
-                #pragma unroll
-                for (int k2 = 0; k2 < 8; ++k2) {
-                    const float t = (float)k2 - xs;
-                    float g = ex2f(fmaf(negA * t, t, Es));
-                    g = (flags & (1u << k2)) ? g : 0.f;
-                    #pragma unroll
-                    for (int ch = 0; ch < CH; ++ch) acc[ch][k2] = fmaf(wv[ch], g, acc[ch][k2]);
-                }
-            }
-        }
+        const int nb = (int)min((uint32_t)kFwdBatch, kend - base);
+        const int nd = (kdirect > base) ? (int)min((uint32_t)nb, kdirect - base) : 0;   // class 0 comes first
+        int j = 0;
+        for (; j < nd; ++j) eval_key<CH, true>(sb + j * W, wsel, lanebit, fy, fz, acc);
+        #pragma unroll 2
+        for (; j < nb; ++j) eval_key<CH, false>(sb + j * W, wsel, lanebit, fy, fz, acc);
     }
 
     // write the row once (zeros for empty bricks); x fastest, [C, nz, ny, nx]
@@ -188,10 +204,10 @@ static int launch_fwd_ch(gsvox_plan* p, const float* weight, int C, int c0, floa
     bool vec = (p->gd.dims[0] % 4 == 0) && (((uintptr_t)out & 15) == 0);
     if (vec)
         k_forward<CH, true><<<p->gd.nbricks, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
-                                                               weight, C, c0, out, p->gd);
+                                                                   weight, C, c0, out, p->gd);
     else
         k_forward<CH, false><<<p->gd.nbricks, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
-                                                                weight, C, c0, out, p->gd);
+                                                                    weight, C, c0, out, p->gd);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }
