@@ -36,6 +36,13 @@ __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float 
                  :: "l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
+__device__ __forceinline__ float4 lds_v4(uint32_t saddr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
+    return v;
+}
+
 // Geometry of one key, brick-local.
 struct KeyGeom {
     float cx, cy, cz, negA, nl01, nl02, l12, nD1, nD2, cc;
@@ -46,22 +53,23 @@ struct KeyGeom {
 
 struct Moments { float b0, bu0, bu1, bu2, b00, b01, b02, b11, b12, b22; };
 
-// Walk the rows of one key.  MASKED: some voxels of the row lie outside the box in x.
-template <int CH, bool SINGLE, bool MASKED>
-__device__ __forceinline__ void walk_rows(const KeyGeom& kg, const float* __restrict__ s_g, const float (&wv)[CH],
+// Walk the rows of one key.  DIRECT: one EX2 per voxel (narrow Gaussians, class 0).  sbase is the
+// shared-window byte address of the gradient tile.
+template <int CH, bool SINGLE, bool DIRECT>
+__device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, const float (&wv)[CH],
                                           Moments& m, float (&dw)[CH])
 {
     float dy = (float)kg.y0 - kg.cy, dz = (float)kg.z0 - kg.cz;
     const float dy0 = dy;
-    int goff = ((kg.z0 << 3) + kg.y0) << 3;                 // float offset of the row in the tile
-    const int wrapstep = (9 - kg.ny) << 3;                  // from the last y of a slice to y0 of the next
+    uint32_t gaddr = sbase + ((((kg.z0 << 3) + kg.y0) << 3) << 2);     // byte address of the row in the tile
+    const uint32_t wrapstep = (uint32_t)(9 - kg.ny) << 5;              // last y of a slice -> y0 of the next
     int yc = kg.ny;
     for (int r = kg.nrows; r > 0; --r) {
         const float u1 = fmaf(kg.l12, dz, dy);
         const float xs = fmaf(kg.nl02, dz, fmaf(kg.nl01, dy, kg.cx));
         const float Es = fmaf(kg.nD2 * dz, dz, (kg.nD1 * u1) * u1);
         float G[8];
-        if (!kg.direct) {
+        if (!DIRECT) {
             const float t3 = 3.0f - xs;
             const float nAt = kg.negA * t3;
             G[3] = ex2b(fmaf(nAt, t3, Es));
@@ -73,16 +81,12 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, const float* __rest
             #pragma unroll
             for (int k = 0; k < 8; ++k) { const float t = (float)k - xs; G[k] = ex2b(fmaf(kg.negA * t, t, Es)); }
         }
-        if (MASKED) {
-            #pragma unroll
-            for (int k = 0; k < 8; ++k) G[k] = (kg.xm & (1u << k)) ? G[k] : 0.f;
-        }
+        #pragma unroll
+        for (int k = 0; k < 8; ++k) G[k] = (kg.xm & (1u << k)) ? G[k] : 0.f;      // voxels outside the box in x
         // a_k = (sum_c g_c w_c) G_k  (w factored out when SINGLE)
-        const float* grow = s_g + goff;
         float av[8];
         if (SINGLE) {
-            const float4 g0 = *reinterpret_cast<const float4*>(grow);
-            const float4 g1 = *reinterpret_cast<const float4*>(grow + 4);
+            const float4 g0 = lds_v4(gaddr), g1 = lds_v4(gaddr + 16);
             av[0] = g0.x * G[0]; av[1] = g0.y * G[1]; av[2] = g0.z * G[2]; av[3] = g0.w * G[3];
             av[4] = g1.x * G[4]; av[5] = g1.y * G[5]; av[6] = g1.z * G[6]; av[7] = g1.w * G[7];
         } else {
@@ -90,8 +94,7 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, const float* __rest
             for (int k = 0; k < 8; ++k) av[k] = 0.f;
             #pragma unroll
             for (int ch = 0; ch < CH; ++ch) {
-                const float4 g0 = *reinterpret_cast<const float4*>(grow + ch * kBrickVox);
-                const float4 g1 = *reinterpret_cast<const float4*>(grow + ch * kBrickVox + 4);
+                const float4 g0 = lds_v4(gaddr + ch * kBrickVox * 4), g1 = lds_v4(gaddr + ch * kBrickVox * 4 + 16);
                 const float gv[8] = { g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w };
                 float d = 0.f;
                 #pragma unroll
@@ -103,7 +106,7 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, const float* __rest
         }
         // x-moments about xs
         float U0, U1, U2;
-        if (!kg.direct) {
+        if (!DIRECT) {
             // about the brick-local index, then shifted (wide profile: mild cancellation only)
             U0 = av[0]; float S1 = 0.f, S2 = 0.f;
             #pragma unroll
@@ -126,7 +129,7 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, const float* __rest
         const bool wrap = (yc == 0);
         dy = wrap ? dy0 : dy + 1.0f;
         dz = wrap ? dz + 1.0f : dz;
-        goff += wrap ? wrapstep : 8;
+        gaddr += wrap ? wrapstep : 32u;
         yc = wrap ? kg.ny : yc;
     }
 }
@@ -163,6 +166,7 @@ k_backward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start
 
     const uint32_t nkeys = kend - kbeg;
     const uint32_t lane = tid & 31u;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_g);
     for (uint32_t wbase = tid & ~31u; wbase < nkeys; wbase += kBwdThreads) {     // warp-uniform trip count
         const bool active = wbase + lane < nkeys;
         KeyGeom kg;
@@ -197,8 +201,9 @@ k_backward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start
         #pragma unroll
         for (int ch = 0; ch < CH; ++ch) dw[ch] = 0.f;
 
-        if (__any_sync(0xffffffffu, kg.xm != 0xffu)) walk_rows<CH, SINGLE, true>(kg, s_g, wv, m, dw);
-        else                                          walk_rows<CH, SINGLE, false>(kg, s_g, wv, m, dw);
+        // class 0 (direct) keys sit at the front of the brick's range: at most one warp mixes paths
+        if (kg.direct) walk_rows<CH, SINGLE, true>(kg, sbase, wv, m, dw);
+        else           walk_rows<CH, SINGLE, false>(kg, sbase, wv, m, dw);
 
         if (active) {
             float* dst = acc + (size_t)gid * astride;
