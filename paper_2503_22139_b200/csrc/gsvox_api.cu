@@ -74,10 +74,10 @@ static int make_layout(int64_t n_max, int32_t max_channels, const gsvox_grid* g,
     if (nbins > 0x7ffffff0LL) return GSVOX_ELIMIT;
     L->nbins = (int)nbins;
     size_t off = 0;
-    L->status = off;       off += up256(sizeof(DevStatus));
+    L->status = off;       off += up256(sizeof(DevStatus));          // status and bin_count are contiguous:
+    L->bin_count = off;    off += up256(sizeof(uint32_t) * (size_t)(nbins + 1));   // one memset clears both
     L->rec = off;          off += up256(sizeof(GsRec) * (size_t)n_max);
     L->aux = off;          off += up256(sizeof(GsAux) * (size_t)n_max);
-    L->bin_count = off;    off += up256(sizeof(uint32_t) * (size_t)(nbins + 1));
     L->bin_start = off;    off += up256(sizeof(uint32_t) * (size_t)(nbins + 1));
     size_t sblocks = (size_t)((nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock);
     L->scan_partial = off; off += up256(sizeof(uint32_t) * (sblocks + 1));

@@ -244,10 +244,9 @@ k_scan_apply(uint32_t* __restrict__ cnt, int nbins, const uint32_t* __restrict__
 int launch_preprocess(gsvox_plan* p, const float* pos, const float* scale, const float* quat,
                       int64_t n, cudaStream_t st)
 {
-    { LaunchScope ls(p, GSVOX_K_MEMSET, st);
-      GSVOX_CUDA(cudaMemsetAsync(p->status, 0, sizeof(DevStatus), st)); }
-    { LaunchScope ls(p, GSVOX_K_MEMSET, st);
-      GSVOX_CUDA(cudaMemsetAsync(p->bin_count, 0, sizeof(uint32_t) * (size_t)(p->nbins + 1), st)); }
+    { LaunchScope ls(p, GSVOX_K_MEMSET, st);        // status block + bin counters, contiguous in the workspace
+      size_t bytes = (size_t)((char*)p->bin_count - (char*)p->status) + sizeof(uint32_t) * (size_t)(p->nbins + 1);
+      GSVOX_CUDA(cudaMemsetAsync(p->status, 0, bytes, st)); }
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_PREPROCESS, st);
         int blocks = (int)((n + 255) / 256);

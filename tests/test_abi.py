@@ -49,8 +49,8 @@ def test_workspace_bytes_and_argument_checks(pkg):
     n = C.c_size_t(0)
     g = pkg.make_grid((0, 0, 0), (1, 1, 1), (256, 256, 256))
     assert L.gsvox_workspace_bytes(500000, 1, C.byref(g), 16_000_000, C.byref(n)) == 0
-    # records 64 B + aux 32 B + accumulators 48 B per Gaussian, 4 B per key, 8 B per brick
-    expect = 500000 * (64 + 32 + 48) + 16_000_000 * 4 + 32768 * 8
+    # records 64 B + aux 32 B + accumulators 48 B per Gaussian, 4 B per key, 8 B per (brick, class) bin
+    expect = 500000 * (64 + 32 + 48) + 16_000_000 * 4 + 32768 * 17 * 8
     assert expect <= n.value <= expect + 8192
     bad = pkg.make_grid((0, 0, 0), (1, 0, 1), (8, 8, 8))
     assert L.gsvox_workspace_bytes(10, 1, C.byref(bad), 10, C.byref(n)) == -1
