@@ -145,6 +145,15 @@ int gsvox_step_host(gsvox_plan* plan, void* staging, size_t staging_bytes,
                     float* grad_weight_host, float* grad_pos_host, float* grad_scale_host,
                     float* grad_quat_host, void* stream);
 
+/* Live ALU rooflines of the device the calling thread has current (the hot path is
+ * FP32-issue / MUFU bound, and MEASURED_PEAKS.json holds no FP32 figure).  Runs three register-only
+ * microbenchmarks on `stream` and SYNCHRONISES: scalar FFMA chains (fp32_tflops, 2 flops per lane
+ * instruction), packed fma.rn.f32x2 chains (fp32x2_tflops, 4 flops per lane instruction) and
+ * ex2.approx chains (ex2_tera_per_s, 1e12 results/s).  `scratch` = at least 4 bytes of DEVICE
+ * memory (never written in practice).  Any output pointer may be NULL.  HOST output pointers.  */
+int gsvox_probe_peaks(void* scratch, double* fp32_tflops, double* fp32x2_tflops,
+                      double* ex2_tera_per_s, int32_t* sm_count, void* stream);
+
 const char* gsvox_error_string(int code);
 /* Text of the last CUDA error seen by this thread inside the library ("" if none). */
 const char* gsvox_last_cuda_error(void);

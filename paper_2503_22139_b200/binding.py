@@ -19,7 +19,7 @@ EXPORTS = [
     "gsvox_forward", "gsvox_backward", "gsvox_plan_status", "gsvox_plan_geometry_host",
     "gsvox_plan_bins_host", "gsvox_plan_set_timing", "gsvox_plan_timings",
     "gsvox_host_staging_bytes", "gsvox_step_host", "gsvox_error_string",
-    "gsvox_last_cuda_error", "gsvox_version",
+    "gsvox_last_cuda_error", "gsvox_version", "gsvox_probe_peaks",
 ]
 
 
@@ -64,6 +64,8 @@ def lib():
     L.gsvox_plan_timings.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), i32, vp]
     L.gsvox_host_staging_bytes.argtypes = [i64, i32, gp, szp]
     L.gsvox_step_host.argtypes = [vp, vp, C.c_size_t, vp, vp, vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp]
+    dp = C.POINTER(C.c_double)
+    L.gsvox_probe_peaks.argtypes = [vp, dp, dp, dp, C.POINTER(i32), vp]
     L.gsvox_error_string.argtypes = [C.c_int]
     L.gsvox_error_string.restype = C.c_char_p
     L.gsvox_last_cuda_error.restype = C.c_char_p
@@ -105,6 +107,15 @@ def _host(t, name):
     if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
         raise GsvoxError("%s must be a contiguous float32 CPU tensor" % name)
     return C.c_void_p(t.data_ptr())
+
+
+def probe_peaks():
+    """Measured FP32 (scalar FFMA, packed FFMA2) and MUFU ex2 rates of the current device."""
+    scratch = torch.zeros(64, dtype=torch.float32, device="cuda")
+    a, b, c, sms = C.c_double(0), C.c_double(0), C.c_double(0), C.c_int32(0)
+    _check(lib().gsvox_probe_peaks(C.c_void_p(scratch.data_ptr()), C.byref(a), C.byref(b), C.byref(c),
+                                   C.byref(sms), _stream()))
+    return {"fp32_tflops": a.value, "fp32x2_tflops": b.value, "ex2_tera_per_s": c.value, "sm_count": sms.value}
 
 
 class Plan:

@@ -32,14 +32,17 @@ __device__ __forceinline__ float ex2f(float x)
     return y;
 }
 
-// Shared-memory record of a staged key (floats):
-//   0 cx  1 cy  2 cz  3 -A | 4 -l01  5 -l02  6 l12  7 -D1 | 8 -D2  9 c  10 rowmask(z 0..3)  11 rowmask(z 4..7)
-//   CH == 1: 12..19  w * [k inside the box in x], k = 0..7
-//   CH  > 1: 12 xmask, 13..13+CH-1 weights
+// Shared-memory record of a staged key (floats); pairs that feed packed (f32x2) instructions sit on
+// even word offsets so that one LDS.128 delivers them as aligned register pairs:
+//   0 cx  1 cy  2 cz  3 -A | 4 -l01  5 -l02  6 l12  7 -D1 | 8 -D2  9 (unused)  10 c  11 c
+//   CH == 1: 12..19  w * [k inside the box in x] in the order k = 3,4, 2,5 | 1,6, 0,7
+//   CH  > 1: 12 xmask, 13.. weights (scalar arithmetic: packed FFMA2 measured slower there)
+// The brick-local row masks (one word per warp) live in a separate array.
 template <int CH> struct FwdRec { static constexpr int kWords = (CH == 1) ? 20 : ((13 + CH + 3) & ~3); };
 
 template <int CH>
-__device__ __forceinline__ void stage_key(float* __restrict__ dst, const GsRec* __restrict__ rec,
+__device__ __forceinline__ void stage_key(float* __restrict__ dst, uint32_t* __restrict__ mask0,
+                                          uint32_t* __restrict__ mask1, const GsRec* __restrict__ rec,
                                           const float* __restrict__ weight, int wstride, int c0,
                                           uint32_t gid, int b0x, int b0y, int b0z)
 {
@@ -62,14 +65,16 @@ __device__ __forceinline__ void stage_key(float* __restrict__ dst, const GsRec* 
     uint32_t zh = zm >> 4;
     uint32_t sel1 = ((zh & 1u) ? 0xffu : 0u) | ((zh & 2u) ? 0xff00u : 0u) |
                     ((zh & 4u) ? 0xff0000u : 0u) | ((zh & 8u) ? 0xff000000u : 0u);
+    *mask0 = rep & sel0;
+    *mask1 = rep & sel1;
     float4* o = reinterpret_cast<float4*>(dst);
     o[0] = make_float4((float)(cix - b0x) + a.x, (float)(ciy - b0y) + a.y, (float)(ciz - b0z) + a.z, b.w);
     o[1] = make_float4(c.x, c.y, c.z, c.w);
-    o[2] = make_float4(d.x, a.w, __uint_as_float(rep & sel0), __uint_as_float(rep & sel1));
+    o[2] = make_float4(d.x, 0.f, a.w, a.w);
     if (CH == 1) {
         const float w = __ldg(weight + (size_t)gid * wstride + c0);
-        o[3] = make_float4((xm & 1u) ? w : 0.f, (xm & 2u) ? w : 0.f, (xm & 4u) ? w : 0.f, (xm & 8u) ? w : 0.f);
-        o[4] = make_float4((xm & 16u) ? w : 0.f, (xm & 32u) ? w : 0.f, (xm & 64u) ? w : 0.f, (xm & 128u) ? w : 0.f);
+        o[3] = make_float4((xm & 8u) ? w : 0.f, (xm & 16u) ? w : 0.f, (xm & 4u) ? w : 0.f, (xm & 32u) ? w : 0.f);
+        o[4] = make_float4((xm & 2u) ? w : 0.f, (xm & 64u) ? w : 0.f, (xm & 1u) ? w : 0.f, (xm & 128u) ? w : 0.f);
     } else {
         dst[12] = __uint_as_float(xm);
         #pragma unroll
@@ -78,15 +83,16 @@ __device__ __forceinline__ void stage_key(float* __restrict__ dst, const GsRec* 
 }
 
 // One staged key against this thread's row.  DIRECT: one EX2 per voxel (narrow Gaussians).
+// acc[ch][j] is the packed pair of voxels (3 - j, 4 + j): the two arms of the centre-out recurrence
+// advance together, one FMUL2 per step.
 template <int CH, bool DIRECT>
-__device__ __forceinline__ void eval_key(const float* __restrict__ r, int wsel, uint32_t lanebit,
+__device__ __forceinline__ void eval_key(const float* __restrict__ r, uint32_t mrow, uint32_t lanebit,
                                          float fy, float fz, float (&acc)[CH][8])
 {
-    const uint32_t mrow = __float_as_uint(r[10 + wsel]);
     if (mrow == 0u) return;                                         // none of this warp's 32 rows is in the box
     const float4 r0 = *reinterpret_cast<const float4*>(r);
     const float4 r1 = *reinterpret_cast<const float4*>(r + 4);
-    const float2 r2 = *reinterpret_cast<const float2*>(r + 8);
+    const float4 r2 = *reinterpret_cast<const float4*>(r + 8);
     // row geometry: u2 = dz, u1 = dy + l12 dz, xs = cx - l01 dy - l02 dz
     const float dy = fy - r0.y, dz = fz - r0.z;
     const float u1 = fmaf(r1.z, dz, dy);
@@ -94,30 +100,52 @@ __device__ __forceinline__ void eval_key(const float* __restrict__ r, int wsel, 
     float Es = fmaf(r2.x * dz, dz, (r1.w * u1) * u1);
     Es = (mrow & lanebit) ? Es : -1.0e30f;                          // rows outside the box contribute exact zeros
     const float negA = r0.w;
-    float G[8];
-    if (!DIRECT) {
-        // centre-out recurrence from k = 3
-        const float t3 = 3.0f - xs;
-        const float nAt = negA * t3;
-        const float Lf = fminf(fmaf(nAt, 2.0f, negA), 120.f);      // E(4) - E(3), clamped: 0 * inf would be NaN
-        const float Lb = fminf(fmaf(nAt, -2.0f, negA), 120.f);     // E(2) - E(3)
-        const float cc = r2.y;
-        G[3] = ex2f(fmaf(nAt, t3, Es));
-        float rf = ex2f(Lf), rb = ex2f(Lb);
-        G[4] = G[3] * rf; rf *= cc; G[5] = G[4] * rf; rf *= cc; G[6] = G[5] * rf; rf *= cc; G[7] = G[6] * rf;
-        G[2] = G[3] * rb; rb *= cc; G[1] = G[2] * rb; rb *= cc; G[0] = G[1] * rb;
-    } else {
-        #pragma unroll
-        for (int k = 0; k < 8; ++k) { const float t = (float)k - xs; G[k] = ex2f(fmaf(negA * t, t, Es)); }
-    }
     if (CH == 1) {
+        // packed pairs P[j] = (G[3-j], G[4+j]): the two arms of the centre-out recurrence advance together
+        f32x2 P[4];
+        if (!DIRECT) {
+            const float t3 = 3.0f - xs;
+            const float nAt = negA * t3;
+            const float Lf = fminf(fmaf(nAt, 2.0f, negA), 120.f);  // E(4) - E(3), clamped: 0 * inf would be NaN
+            const float Lb = fminf(fmaf(nAt, -2.0f, negA), 120.f); // E(2) - E(3)
+            const f32x2 cc2 = pk2(r2.z, r2.w);
+            const float G3 = ex2f(fmaf(nAt, t3, Es));
+            const float rf = ex2f(Lf), rb = ex2f(Lb);
+            const float G4 = G3 * rf;
+            f32x2 R = pk2(rb, rf * r2.z);                           // (G2/G3, G5/G4)
+            P[0] = pk2(G3, G4);
+            P[1] = mul2(P[0], R); R = mul2(R, cc2);
+            P[2] = mul2(P[1], R); R = mul2(R, cc2);
+            P[3] = mul2(P[2], R);
+        } else {
+            #pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float tl = (float)(3 - j) - xs, th = (float)(4 + j) - xs;
+                P[j] = pk2(ex2f(fmaf(negA * tl, tl, Es)), ex2f(fmaf(negA * th, th, Es)));
+            }
+        }
         const float4 wa = *reinterpret_cast<const float4*>(r + 12);
         const float4 wb = *reinterpret_cast<const float4*>(r + 16);
-        acc[0][0] = fmaf(wa.x, G[0], acc[0][0]); acc[0][1] = fmaf(wa.y, G[1], acc[0][1]);
-        acc[0][2] = fmaf(wa.z, G[2], acc[0][2]); acc[0][3] = fmaf(wa.w, G[3], acc[0][3]);
-        acc[0][4] = fmaf(wb.x, G[4], acc[0][4]); acc[0][5] = fmaf(wb.y, G[5], acc[0][5]);
-        acc[0][6] = fmaf(wb.z, G[6], acc[0][6]); acc[0][7] = fmaf(wb.w, G[7], acc[0][7]);
+        fma2_acc(acc[0][0], acc[0][1], P[0], pk2(wa.x, wa.y));
+        fma2_acc(acc[0][2], acc[0][3], P[1], pk2(wa.z, wa.w));
+        fma2_acc(acc[0][4], acc[0][5], P[2], pk2(wb.x, wb.y));
+        fma2_acc(acc[0][6], acc[0][7], P[3], pk2(wb.z, wb.w));
     } else {
+        float G[8];
+        if (!DIRECT) {
+            const float t3 = 3.0f - xs;
+            const float nAt = negA * t3;
+            const float Lf = fminf(fmaf(nAt, 2.0f, negA), 120.f);
+            const float Lb = fminf(fmaf(nAt, -2.0f, negA), 120.f);
+            const float cc = r2.z;
+            G[3] = ex2f(fmaf(nAt, t3, Es));
+            float rf = ex2f(Lf), rb = ex2f(Lb);
+            G[4] = G[3] * rf; rf *= cc; G[5] = G[4] * rf; rf *= cc; G[6] = G[5] * rf; rf *= cc; G[7] = G[6] * rf;
+            G[2] = G[3] * rb; rb *= cc; G[1] = G[2] * rb; rb *= cc; G[0] = G[1] * rb;
+        } else {
+            #pragma unroll
+            for (int k = 0; k < 8; ++k) { const float t = (float)k - xs; G[k] = ex2f(fmaf(negA * t, t, Es)); }
+        }
         const uint32_t xm = __float_as_uint(r[12]);
         #pragma unroll
         for (int k = 0; k < 8; ++k) G[k] = (xm & (1u << k)) ? G[k] : 0.f;
@@ -139,6 +167,7 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
 {
     constexpr int W = FwdRec<CH>::kWords;
     __shared__ __align__(16) float s_rec[2][kFwdBatch * W];
+    __shared__ uint32_t s_mask[2][2][kFwdBatch];                    // [buffer][warp][key]
 
     const int tid = threadIdx.x;
     const int b = blockIdx.x;
@@ -149,11 +178,11 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
     const int wsel = tid >> 5;
     const uint32_t lanebit = 1u << (tid & 31);
 
-    float acc[CH][8];
+    float acc[CH][8];       // CH == 1: acc[0][2j], acc[0][2j+1] = voxels 3 - j, 4 + j (packed pair j); else x order
     #pragma unroll
     for (int ch = 0; ch < CH; ++ch)
         #pragma unroll
-        for (int k = 0; k < 8; ++k) acc[ch][k] = 0.f;
+        for (int j = 0; j < 8; ++j) acc[ch][j] = 0.f;
 
     uint32_t kbeg = 0, kend = 0, kdirect = 0;
     if (!status->overflow) {
@@ -165,14 +194,16 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
     for (uint32_t base = kbeg; base < kend; base += kFwdBatch, buf ^= 1) {
         float* sb = s_rec[buf];
         uint32_t k = base + tid;
-        if (k < kend) stage_key<CH>(sb + tid * W, rec, weight, wstride, c0, keys[k], b0x, b0y, b0z);
+        if (k < kend) stage_key<CH>(sb + tid * W, &s_mask[buf][0][tid], &s_mask[buf][1][tid], rec, weight, wstride,
+                                    c0, keys[k], b0x, b0y, b0z);
         __syncthreads();
+        const uint32_t* mk = s_mask[buf][wsel];
         const int nb = (int)min((uint32_t)kFwdBatch, kend - base);
         const int nd = (kdirect > base) ? (int)min((uint32_t)nb, kdirect - base) : 0;   // class 0 comes first
         int j = 0;
-        for (; j < nd; ++j) eval_key<CH, true>(sb + j * W, wsel, lanebit, fy, fz, acc);
+        for (; j < nd; ++j) eval_key<CH, true>(sb + j * W, mk[j], lanebit, fy, fz, acc);
         #pragma unroll 2
-        for (; j < nb; ++j) eval_key<CH, false>(sb + j * W, wsel, lanebit, fy, fz, acc);
+        for (; j < nb; ++j) eval_key<CH, false>(sb + j * W, mk[j], lanebit, fy, fz, acc);
     }
 
     // write the row once (zeros for empty bricks); x fastest, [C, nz, ny, nx]
@@ -182,16 +213,22 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
         const size_t rowoff = ((size_t)gz * gd.dims[1] + gy) * gd.dims[0] + b0x;
         #pragma unroll
         for (int ch = 0; ch < CH; ++ch) {
+            float v[8];
+            #pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                v[3 - j] = (CH == 1) ? acc[ch][2 * j] : acc[ch][3 - j];
+                v[4 + j] = (CH == 1) ? acc[ch][2 * j + 1] : acc[ch][4 + j];
+            }
             float* o = out + (size_t)(c0 + ch) * plane + rowoff;
             if (VEC) {
                 if (b0x + 3 < gd.dims[0])
-                    __stcs(reinterpret_cast<float4*>(o), make_float4(acc[ch][0], acc[ch][1], acc[ch][2], acc[ch][3]));
+                    __stcs(reinterpret_cast<float4*>(o), make_float4(v[0], v[1], v[2], v[3]));
                 if (b0x + 7 < gd.dims[0])
-                    __stcs(reinterpret_cast<float4*>(o) + 1, make_float4(acc[ch][4], acc[ch][5], acc[ch][6], acc[ch][7]));
+                    __stcs(reinterpret_cast<float4*>(o) + 1, make_float4(v[4], v[5], v[6], v[7]));
             } else {
                 #pragma unroll
                 for (int k2 = 0; k2 < 8; ++k2)
-                    if (b0x + k2 < gd.dims[0]) o[k2] = acc[ch][k2];
+                    if (b0x + k2 < gd.dims[0]) o[k2] = v[k2];
             }
         }
     }

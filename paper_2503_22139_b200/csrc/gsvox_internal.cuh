@@ -79,6 +79,33 @@ __host__ __device__ __forceinline__ int key_class(bool direct, int x0, int x1, i
 
 inline __host__ __device__ int acc_stride(int channels) { return (9 + channels + 3) & ~3; }
 
+#ifdef __CUDACC__
+// Packed fp32 pairs (sm_100 family FFMA2/FMUL2/FADD2): one issue slot for two lanes of work.  a3/a4
+// are issue-bound (profiles/r1b), so halving the instruction count of the per-voxel arithmetic is
+// what the packed forms buy; the FP32 pipe rate itself is unchanged (gsvox_probe_peaks).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi)
+{ f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk2(f32x2 v, float& lo, float& hi)
+{ asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{ f32x2 r; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{ f32x2 r; asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{ f32x2 r; asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+// c += a * b in place: ties the accumulator to one register pair (the three-operand form lets
+// ptxas pick a fresh destination and copy back across the key loop's reconvergence points).
+__device__ __forceinline__ void fma2_acc(f32x2& c, f32x2 a, f32x2 b)
+{ asm("fma.rn.ftz.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b)); }
+// Same with the accumulator held as two scalar registers.
+__device__ __forceinline__ void fma2_acc(float& clo, float& chi, f32x2 a, f32x2 b)
+{
+    asm("{\n\t.reg .b64 c;\n\tmov.b64 c, {%0, %1};\n\tfma.rn.ftz.f32x2 c, %2, %3, c;\n\tmov.b64 {%0, %1}, c;\n\t}"
+        : "+f"(clo), "+f"(chi) : "l"(a), "l"(b));
+}
+#endif
+
 }  // namespace gsvox
 
 // The host-side plan (opaque in the public header).
