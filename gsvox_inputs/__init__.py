@@ -184,6 +184,79 @@ def subvolume_case(n=600, dims=(37, 29, 21), channels=3, seed=11,
                  origin=tuple(origin), spacing=tuple(spacing))
 
 
+@dataclass
+class DvfCase:
+    """Inputs of the fused MBC -> DVF op: the
+    three MBC levels as ONE Gaussian set with a level id per Gaussian, a 3-vector feature per
+    Gaussian (the Cartesian components k of e_{i,k}) and per-projection coefficients w_{i,k}(p)."""
+    name: str
+    dims: tuple
+    pos: np.ndarray             # [n,3]
+    scale: np.ndarray           # [n,3]
+    quat: np.ndarray            # [n,4]
+    feat: np.ndarray            # [n,3] fp32
+    level: np.ndarray           # [n] int32 in 0..L-1
+    coef: np.ndarray            # [B,L,3] fp32
+    origin: tuple = (0.0, 0.0, 0.0)
+    spacing: tuple = (1.0, 1.0, 1.0)
+    seed: object = 0
+
+    @property
+    def n(self):
+        return int(self.pos.shape[0])
+
+    @property
+    def batch(self):
+        return int(self.coef.shape[0])
+
+    @property
+    def nlevels(self):
+        return int(self.coef.shape[1])
+
+    @property
+    def grid(self):
+        return (np.asarray(self.origin, np.float32), np.asarray(self.spacing, np.float32),
+                np.asarray(self.dims, np.int32))
+
+    def levels(self):
+        """The same Gaussians split per level, as the oracle's (pos, scale, quat, feat) tuples,
+        plus the index arrays that map each level back into the concatenated set."""
+        out, ids = [], []
+        for i in range(self.nlevels):
+            sel = np.flatnonzero(self.level == i)
+            ids.append(sel)
+            out.append((self.pos[sel], self.scale[sel], self.quat[sel], self.feat[sel]))
+        return out, ids
+
+    def grad_dvf(self):
+        rng = np.random.default_rng([77, self.batch] + list(np.atleast_1d(self.seed)))
+        nx, ny, nz = self.dims
+        return rng.standard_normal((self.batch, 3, nz, ny, nx), dtype=np.float32)
+
+
+def dvf_case(batch=8, counts=(1_000, 8_000, 64_000), dims=(128, 128, 64), seed=5, shuffle=True,
+             scales=((16.0, 32.0), (6.0, 12.0), (2.0, 5.0))):
+    """Config 3's three MBC levels (same counts and scale ranges) as one set for the fused op:
+    features N(0,1) per Cartesian component, coefficients w_{i,k}(p) ~ N(0,1) for `batch`
+    projections (N_batch = 8 in Stage 3, 32 in Stage 2).  Level membership is
+    interleaved (shuffle) so that the level id really is per Gaussian."""
+    rng = np.random.default_rng(seed)
+    pos, scale, quat, feat, level = [], [], [], [], []
+    for i, (n, (a, b)) in enumerate(zip(counts, scales)):
+        pos.append(_uniform_in_grid(rng, n, dims))
+        scale.append(_log_uniform(rng, a, b, (n, 3)))
+        quat.append(_unit_quats(rng, n))
+        feat.append(rng.standard_normal((n, 3)))
+        level.append(np.full(n, i, dtype=np.int32))
+    pos, scale, quat, feat, level = (np.concatenate(x) for x in (pos, scale, quat, feat, level))
+    if shuffle:
+        perm = rng.permutation(pos.shape[0])
+        pos, scale, quat, feat, level = pos[perm], scale[perm], quat[perm], feat[perm], level[perm]
+    coef = rng.standard_normal((batch, len(counts), 3))
+    return DvfCase("dvf_fused_b%d" % batch, tuple(dims), _f32(pos), _f32(scale), _f32(quat), _f32(feat),
+                   np.ascontiguousarray(level, dtype=np.int32), _f32(coef), seed=seed)
+
+
 FULL = {
     "config1": lambda: [config1()],
     "config2": lambda: [config2()],

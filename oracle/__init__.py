@@ -150,3 +150,64 @@ def backward_for(pos, scale, quat, weight, grid, grad_out, ids, kappa=KAPPA):
                                            _p(gw, C.c_double), _p(gp, C.c_double),
                                            _p(gs, C.c_double), _p(gq, C.c_double)))
     return gw, gp, gs, gq
+
+
+# --------------------------------------------------------------------------------------------
+# motion-basis components -> deformation vector fields.
+#   PAPER.md:106   "three spatial levels (i = 1, 2, 3) are employed for e_i(x) along each Cartesian
+#                   direction (x, y, z), resulting in a total of nine MBC volumes"
+#   PAPER.md:58-61 Eq. 3:  d(x,p) = sum_i w_i(p) e_i(x);  PAPER.md:141: w_{i,k}(p), i = level, k = axis
+# The oracle follows the paper's order literally: voxelize every level into its three MBC volumes
+# e_{i,k} (Eq. 5 with the level's feature column k as the weight), THEN combine them with the
+# per-projection coefficients.  (The CUDA path never forms the nine volumes; it folds the
+# coefficients into per-Gaussian weights.  Nothing of that is used here.)
+# --------------------------------------------------------------------------------------------
+def mbc_volumes(levels, grid, kappa=KAPPA):
+    """levels = [(pos, scale, quat, feat[n_i,3]), ...]  ->  e [L, 3, nz, ny, nx] fp64."""
+    return np.stack([forward(p, s, q, f, grid, kappa) for (p, s, q, f) in levels])
+
+
+def dvf_forward(levels, coef, grid, kappa=KAPPA):
+    """coef [B, L, 3] (w_{i,k}(p) of PAPER.md:141)  ->  d [B, 3, nz, ny, nx] fp64 (Eq. 3)."""
+    coef = np.asarray(_f32(coef), dtype=np.float64)
+    e = mbc_volumes(levels, grid, kappa)
+    B, L = coef.shape[0], coef.shape[1]
+    d = np.zeros((B, 3) + e.shape[2:])
+    for b in range(B):
+        for i in range(L):
+            for k in range(3):
+                d[b, k] += coef[b, i, k] * e[i, k]
+    return d
+
+
+def _split_f32(a):
+    """fp64 array -> (hi, lo) fp32 arrays with hi + lo == a to ~1e-15 relative."""
+    hi = a.astype(np.float32)
+    lo = (a - hi.astype(np.float64)).astype(np.float32)
+    return hi, lo
+
+
+def dvf_backward(levels, coef, grid, grad_dvf, kappa=KAPPA):
+    """Chain rule of dvf_forward.  grad_dvf [B,3,nz,ny,nx] (fp32 as handed to the CUDA path) ->
+    (grad_coef [B,L,3], [(grad_feat [n_i,3], grad_pos, grad_scale, grad_quat) per level]).
+      dL/dcoef[b,i,k] = <grad_dvf[b,k], e_{i,k}>
+      dL/de_{i,k}     = sum_b coef[b,i,k] grad_dvf[b,k]      then the voxelizer's analytic backward.
+    The C oracle takes fp32 upstream gradients; dL/de is handed over as an exact hi+lo fp32 split
+    (the backward is linear in the upstream gradient)."""
+    coef = np.asarray(_f32(coef), dtype=np.float64)
+    g = np.asarray(_f32(grad_dvf), dtype=np.float64)
+    e = mbc_volumes(levels, grid, kappa)
+    B, L = coef.shape[0], coef.shape[1]
+    grad_coef = np.zeros((B, L, 3))
+    per_level = []
+    for i, (p, s, q, f) in enumerate(levels):
+        ge = np.zeros((3,) + e.shape[2:])
+        for b in range(B):
+            for k in range(3):
+                grad_coef[b, i, k] = float(np.sum(g[b, k] * e[i, k]))
+                ge[k] += coef[b, i, k] * g[b, k]
+        hi, lo = _split_f32(ge)
+        a = backward(p, s, q, f, grid, hi, kappa)
+        c = backward(p, s, q, f, grid, lo, kappa)
+        per_level.append(tuple(x + y for x, y in zip(a, c)))
+    return grad_coef, per_level
