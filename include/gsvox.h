@@ -45,8 +45,9 @@ extern "C" {
 #define GSVOX_ENOTREADY    -4   /* forward/backward before preprocess                         */
 #define GSVOX_ELIMIT       -5   /* size beyond the library limits below                       */
 
-#define GSVOX_MAX_CHANNELS  16          /* 1 <= C <= 16                                       */
+#define GSVOX_MAX_CHANNELS  96          /* 1 <= C <= 96 (3 axes x 32 projections) */
 #define GSVOX_MAX_DIM       32760       /* per-axis voxel count                               */
+#define GSVOX_MAX_LEVELS    4           /* MBC levels of the two-stage combine (the paper uses 3) */
 #define GSVOX_BRICK         8           /* bricks are 8x8x8 voxels                            */
 #define GSVOX_SIGMA_CUTOFF  3.0         /* fixed (north_star)                                 */
 
@@ -126,6 +127,7 @@ enum {
     GSVOX_K_BACKWARD,         /* a4                                               */
     GSVOX_K_EPILOGUE,         /* a5  chain rule to scale/quat/pos                 */
     GSVOX_K_MEMSET,           /* zero-fills issued by the library                 */
+    GSVOX_K_DVF,              /* 8(f)-1 coefficient mixing / un-mixing            */
     GSVOX_K_COUNT_KINDS
 };
 int gsvox_plan_set_timing(gsvox_plan* plan, int32_t enabled);
@@ -144,6 +146,45 @@ int gsvox_step_host(gsvox_plan* plan, void* staging, size_t staging_bytes,
                     const float* grad_out_host, float* out_host,
                     float* grad_weight_host, float* grad_pos_host, float* grad_scale_host,
                     float* grad_quat_host, void* stream);
+
+/* ---- motion-basis components -> deformation vector fields, fused ----
+ * PAPER.md:58-61 (Eq. 3)  d(x,p) = sum_i w_i(p) e_i(x);  PAPER.md:106: three spatial levels i, each
+ * with one MBC volume per Cartesian direction k (nine volumes), each level its own Gaussian set;
+ * the motion encoder yields nine coefficients w_{i,k}(p) per projection p.
+ *   e_{i,k}(x) = sum_{j in level i} feat[j,k] G_j(x)   (Eq. 5, signed values)
+ *   dvf[b,k,x] = sum_i coef[b,i,k] e_{i,k}(x)           for the B projections of a batch.
+ * The plan holds the geometry of ALL levels as one Gaussian set (gsvox_preprocess once per step);
+ * level[j] in 0..L-1 names the level of Gaussian j (other values: the Gaussian contributes
+ * nothing).  The nine MBC volumes are never materialised: the coefficients are folded into
+ * per-Gaussian weights mixed[j, 3b+k] = coef[b,level[j],k] feat[j,k] and the set is voxelized once
+ * with C = 3B channels (the plan needs max_channels >= 3B).
+ *   feat [n,3], level [n] int32, coef [B,L,3], mixed [n,3B] (caller-owned scratch, overwritten),
+ *   dvf [B,3,nz,ny,nx] OVERWRITTEN.  All DEVICE pointers.  No host synchronisation.            */
+int gsvox_dvf_forward(gsvox_plan* plan, const float* feat, const int32_t* level, const float* coef,
+                      int32_t B, int32_t L, float* mixed, float* dvf, void* stream);
+/* Backward of the above for grad_dvf = dL/ddvf [B,3,nz,ny,nx]: writes dL/dfeat [n,3],
+ * dL/dcoef [B,L,3], dL/dpos [n,3], dL/dscale [n,3], dL/dquat [n,4] (all OVERWRITTEN).
+ * grad_mixed [n,3B] is caller-owned scratch (overwritten); mixed is recomputed from coef.       */
+int gsvox_dvf_backward(gsvox_plan* plan, const float* feat, const int32_t* level, const float* coef,
+                       int32_t B, int32_t L, float* mixed, const float* grad_dvf, float* grad_mixed,
+                       float* grad_feat, float* grad_coef, float* grad_pos, float* grad_scale,
+                       float* grad_quat, void* stream);
+
+/* Two-stage form of the same map for batches of projections (BASELINE config 3: "each level
+ * voxelized separately"): e [L,3,V] are the MBC volumes (gsvox_forward with C = 3 on one plan per
+ * level, V = nx*ny*nz), coef [B,L,3]:
+ *     dvf[b,k,v] = sum_i coef[b,i,k] e[i,k,v]                                    (Eq. 3)
+ * HBM-bound: 4 V (3L + 3B) algorithmic bytes.  The voxelizer is ALU-bound, so for B > 1 this form
+ * (exponentials evaluated once per level) is the fast one; gsvox_dvf_forward re-evaluates them per
+ * group of 9 channels and is the single-projection path (measured).
+ * 1 <= B <= 32, 1 <= L <= GSVOX_MAX_LEVELS.  All DEVICE pointers; outputs OVERWRITTEN.          */
+int gsvox_mbc_combine_forward(const float* e, const float* coef, int32_t B, int32_t L, int64_t V,
+                              float* dvf, void* stream);
+/* Backward: grad_e[i,k,v] = sum_b coef[b,i,k] grad_dvf[b,k,v] (feed it to gsvox_backward of level
+ * i) and grad_coef[b,i,k] = sum_v grad_dvf[b,k,v] e[i,k,v], in one pass over grad_dvf and e:
+ * 4 V (3B + 6L) algorithmic bytes.                                                              */
+int gsvox_mbc_combine_backward(const float* e, const float* coef, const float* grad_dvf, int32_t B,
+                               int32_t L, int64_t V, float* grad_e, float* grad_coef, void* stream);
 
 /* Live ALU rooflines of the device the calling thread has current (the hot path is
  * FP32-issue / MUFU bound, and MEASURED_PEAKS.json holds no FP32 figure).  Runs three register-only

@@ -167,10 +167,10 @@ def mbc_volumes(levels, grid, kappa=KAPPA):
     return np.stack([forward(p, s, q, f, grid, kappa) for (p, s, q, f) in levels])
 
 
-def dvf_forward(levels, coef, grid, kappa=KAPPA):
-    """coef [B, L, 3] (w_{i,k}(p) of PAPER.md:141)  ->  d [B, 3, nz, ny, nx] fp64 (Eq. 3)."""
+def mbc_combine(e, coef):
+    """Eq. 3 on given MBC volumes: e [L,3,...] , coef [B,L,3] -> d [B,3,...] fp64."""
     coef = np.asarray(_f32(coef), dtype=np.float64)
-    e = mbc_volumes(levels, grid, kappa)
+    e = np.asarray(e, dtype=np.float64)
     B, L = coef.shape[0], coef.shape[1]
     d = np.zeros((B, 3) + e.shape[2:])
     for b in range(B):
@@ -178,6 +178,27 @@ def dvf_forward(levels, coef, grid, kappa=KAPPA):
             for k in range(3):
                 d[b, k] += coef[b, i, k] * e[i, k]
     return d
+
+
+def mbc_combine_backward(e, coef, grad_dvf):
+    """-> (dL/de [L,3,...], dL/dcoef [B,L,3]) of mbc_combine, fp64."""
+    coef = np.asarray(_f32(coef), dtype=np.float64)
+    e = np.asarray(e, dtype=np.float64)
+    g = np.asarray(grad_dvf, dtype=np.float64)
+    B, L = coef.shape[0], coef.shape[1]
+    ge = np.zeros_like(e)
+    gc = np.zeros((B, L, 3))
+    for b in range(B):
+        for i in range(L):
+            for k in range(3):
+                ge[i, k] += coef[b, i, k] * g[b, k]
+                gc[b, i, k] = float(np.sum(g[b, k] * e[i, k]))
+    return ge, gc
+
+
+def dvf_forward(levels, coef, grid, kappa=KAPPA):
+    """coef [B, L, 3] (w_{i,k}(p) of PAPER.md:141)  ->  d [B, 3, nz, ny, nx] fp64 (Eq. 3)."""
+    return mbc_combine(mbc_volumes(levels, grid, kappa), coef)
 
 
 def _split_f32(a):

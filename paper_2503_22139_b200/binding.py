@@ -12,14 +12,15 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgsvox.so")
 
-K_NAMES = ["preprocess", "count", "scan", "scatter", "forward", "backward", "epilogue", "memset"]
+K_NAMES = ["preprocess", "count", "scan", "scatter", "forward", "backward", "epilogue", "memset", "dvf"]
 
 EXPORTS = [
     "gsvox_workspace_bytes", "gsvox_plan_create", "gsvox_plan_destroy", "gsvox_preprocess",
     "gsvox_forward", "gsvox_backward", "gsvox_plan_status", "gsvox_plan_geometry_host",
     "gsvox_plan_bins_host", "gsvox_plan_set_timing", "gsvox_plan_timings",
     "gsvox_host_staging_bytes", "gsvox_step_host", "gsvox_error_string",
-    "gsvox_last_cuda_error", "gsvox_version", "gsvox_probe_peaks",
+    "gsvox_last_cuda_error", "gsvox_version", "gsvox_probe_peaks", "gsvox_dvf_forward", "gsvox_dvf_backward",
+    "gsvox_mbc_combine_forward", "gsvox_mbc_combine_backward",
 ]
 
 
@@ -64,6 +65,10 @@ def lib():
     L.gsvox_plan_timings.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), i32, vp]
     L.gsvox_host_staging_bytes.argtypes = [i64, i32, gp, szp]
     L.gsvox_step_host.argtypes = [vp, vp, C.c_size_t, vp, vp, vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp]
+    L.gsvox_dvf_forward.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, vp]
+    L.gsvox_dvf_backward.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.gsvox_mbc_combine_forward.argtypes = [vp, vp, i32, i32, i64, vp, vp]
+    L.gsvox_mbc_combine_backward.argtypes = [vp, vp, vp, i32, i32, i64, vp, vp, vp]
     dp = C.POINTER(C.c_double)
     L.gsvox_probe_peaks.argtypes = [vp, dp, dp, dp, C.POINTER(i32), vp]
     L.gsvox_error_string.argtypes = [C.c_int]
@@ -116,6 +121,28 @@ def probe_peaks():
     _check(lib().gsvox_probe_peaks(C.c_void_p(scratch.data_ptr()), C.byref(a), C.byref(b), C.byref(c),
                                    C.byref(sms), _stream()))
     return {"fp32_tflops": a.value, "fp32x2_tflops": b.value, "ex2_tera_per_s": c.value, "sm_count": sms.value}
+
+
+def mbc_combine_forward(e, coef, out=None):
+    """e [L,3,nz,ny,nx], coef [B,L,3] -> dvf [B,3,nz,ny,nx] (Eq. 3), HBM-bound combine."""
+    L_, B = int(e.shape[0]), int(coef.shape[0])
+    V = int(e[0, 0].numel())
+    if out is None:
+        out = torch.empty((B, 3) + tuple(e.shape[2:]), dtype=torch.float32, device=e.device)
+    _check(lib().gsvox_mbc_combine_forward(_dev(e, "e"), _dev(coef, "coef"), B, L_, V, _dev(out, "dvf"), _stream()))
+    return out
+
+
+def mbc_combine_backward(e, coef, grad_dvf, grads=None):
+    """-> (grad_e [L,3,nz,ny,nx], grad_coef [B,L,3])."""
+    L_, B = int(e.shape[0]), int(coef.shape[0])
+    V = int(e[0, 0].numel())
+    if grads is None:
+        grads = (torch.empty_like(e), torch.empty((B, L_, 3), dtype=torch.float32, device=e.device))
+    ge, gc = grads
+    _check(lib().gsvox_mbc_combine_backward(_dev(e, "e"), _dev(coef, "coef"), _dev(grad_dvf, "grad_dvf"), B, L_, V,
+                                            _dev(ge, "grad_e"), _dev(gc, "grad_coef"), _stream()))
+    return grads
 
 
 class Plan:
@@ -178,6 +205,44 @@ class Plan:
         _check(lib().gsvox_backward(self._h, _dev(weight, "weight"), ch, _dev(grad_out, "grad_out"),
                                     _dev(gw, "grad_weight"), _dev(gp, "grad_pos"), _dev(gs, "grad_scale"),
                                     _dev(gq, "grad_quat"), _stream()))
+        return grads
+
+    # --- 8(f) rank 1: fused MBC -> DVF ------------------------------------------------
+    def _dvf_scratch(self, n, ch):
+        key = (n, ch)
+        if getattr(self, "_dvf_key", None) != key:
+            self._dvf_mixed = torch.empty((n, ch), dtype=torch.float32, device=self.device)
+            self._dvf_gmixed = torch.empty((n, ch), dtype=torch.float32, device=self.device)
+            self._dvf_key = key
+        return self._dvf_mixed, self._dvf_gmixed
+
+    @staticmethod
+    def _dev_i32(t, name):
+        if not (t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()):
+            raise GsvoxError("%s must be a contiguous int32 CUDA tensor" % name)
+        return C.c_void_p(t.data_ptr())
+
+    def dvf_forward(self, feat, level, coef, out=None):
+        n, B, L = int(feat.shape[0]), int(coef.shape[0]), int(coef.shape[1])
+        nx, ny, nz = self.dims
+        if out is None:
+            out = torch.empty((B, 3, nz, ny, nx), dtype=torch.float32, device=self.device)
+        mixed, _ = self._dvf_scratch(n, 3 * B)
+        _check(lib().gsvox_dvf_forward(self._h, _dev(feat, "feat"), self._dev_i32(level, "level"), _dev(coef, "coef"),
+                                       B, L, _dev(mixed, "mixed"), _dev(out, "dvf"), _stream()))
+        return out
+
+    def dvf_backward(self, feat, level, coef, grad_dvf, grads=None):
+        n, B, L = int(feat.shape[0]), int(coef.shape[0]), int(coef.shape[1])
+        if grads is None:
+            mk = lambda *shape: torch.empty(shape, dtype=torch.float32, device=self.device)
+            grads = (mk(n, 3), mk(B, L, 3), mk(n, 3), mk(n, 3), mk(n, 4))
+        gf, gc, gp, gs, gq = grads
+        mixed, gmixed = self._dvf_scratch(n, 3 * B)
+        _check(lib().gsvox_dvf_backward(self._h, _dev(feat, "feat"), self._dev_i32(level, "level"), _dev(coef, "coef"),
+                                        B, L, _dev(mixed, "mixed"), _dev(grad_dvf, "grad_dvf"), _dev(gmixed, "grad_mixed"),
+                                        _dev(gf, "grad_feat"), _dev(gc, "grad_coef"), _dev(gp, "grad_pos"),
+                                        _dev(gs, "grad_scale"), _dev(gq, "grad_quat"), _stream()))
         return grads
 
     # --- synchronising helpers --------------------------------------------------------

@@ -56,7 +56,7 @@ def test_workspace_bytes_and_argument_checks(pkg):
     assert L.gsvox_workspace_bytes(10, 1, C.byref(bad), 10, C.byref(n)) == -1
     bad = pkg.make_grid((0, 0, 0), (1, 1, 1), (8, 0, 8))
     assert L.gsvox_workspace_bytes(10, 1, C.byref(bad), 10, C.byref(n)) == -1
-    assert L.gsvox_workspace_bytes(10, 17, C.byref(g), 10, C.byref(n)) == -1
+    assert L.gsvox_workspace_bytes(10, 97, C.byref(g), 10, C.byref(n)) == -1      # GSVOX_MAX_CHANNELS = 96
     assert L.gsvox_workspace_bytes(-1, 1, C.byref(g), 10, C.byref(n)) == -1
     big = pkg.make_grid((0, 0, 0), (1, 1, 1), (40000, 8, 8))
     assert L.gsvox_workspace_bytes(10, 1, C.byref(big), 10, C.byref(n)) == -5
