@@ -232,3 +232,82 @@ def dvf_backward(levels, coef, grid, grad_dvf, kappa=KAPPA):
         c = backward(p, s, q, f, grid, lo, kappa)
         per_level.append(tuple(x + y for x, y in zip(a, c)))
     return grad_coef, per_level
+
+
+# --------------------------------------------------------------------------------------------
+# the warp  I(x,p) = I_ref(x + d(x,p))   (PAPER.md:55, Eq. 2; :136).
+# The paper does not say how I_ref is evaluated between voxel centres or outside the volume.
+# Readings (W1-W4): trilinear interpolation of the voxel-centre samples; a corner
+# outside the grid contributes 0 (zero padding, corner by corner); d is in world units like
+# origin/spacing, so the sample position in index units is u_k = i_k + d_k / h_k; the cell index
+# floor(u_k) is decided on t_k = fp32(d_k) / fp32(h_k) ROUNDED TO fp32 (the kernel's precision:
+# both sides take the integer decision in the same precision), everything after that is fp64;
+# a non-finite displacement yields 0 and zero gradients.  Backward is the exact derivative of the
+# piecewise-trilinear interpolant (kinks at integer u have measure zero).
+# --------------------------------------------------------------------------------------------
+def _warp_cells(dvf, spacing, dims):
+    """-> integer base corner i0 [B,3,nz,ny,nx] (int64), fraction f [B,3,nz,ny,nx] fp64, finite mask."""
+    nx, ny, nz = (int(v) for v in dims)
+    d32 = _f32(dvf).reshape(-1, 3, nz, ny, nx)
+    h32 = _f32(spacing).reshape(3)
+    with np.errstate(invalid="ignore", over="ignore"):
+        t = d32 / h32[None, :, None, None, None]              # fp32 IEEE division, as on the device
+    finite = np.all(np.isfinite(t), axis=1) & np.all(np.abs(t) < 1.0e9, axis=1)
+    t = np.where(finite[:, None], t, np.float32(0))
+    tf = np.floor(t)
+    frac = (t - tf).astype(np.float64)                         # exact in fp32
+    idx = np.stack(np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij"))   # z,y,x
+    base = np.empty(t.shape, dtype=np.int64)
+    base[:, 0] = idx[2][None] + tf[:, 0].astype(np.int64)      # x
+    base[:, 1] = idx[1][None] + tf[:, 1].astype(np.int64)      # y
+    base[:, 2] = idx[0][None] + tf[:, 2].astype(np.int64)      # z
+    return base, frac, finite
+
+
+def warp_forward(iref, dvf, grid):
+    """iref [nz,ny,nx], dvf [B,3,nz,ny,nx] (components x,y,z, world units) -> out [B,nz,ny,nx] fp64."""
+    _, h, dims = _grid(grid)
+    nx, ny, nz = (int(v) for v in dims)
+    I = np.asarray(_f32(iref), dtype=np.float64).reshape(nz, ny, nx)
+    base, f, finite = _warp_cells(dvf, h, dims)
+    B = base.shape[0]
+    out = np.zeros((B, nz, ny, nx))
+    for az in (0, 1):
+        for ay in (0, 1):
+            for ax in (0, 1):
+                cx, cy, cz = base[:, 0] + ax, base[:, 1] + ay, base[:, 2] + az
+                w = (f[:, 0] if ax else 1.0 - f[:, 0]) * (f[:, 1] if ay else 1.0 - f[:, 1]) * \
+                    (f[:, 2] if az else 1.0 - f[:, 2])
+                ok = (cx >= 0) & (cx < nx) & (cy >= 0) & (cy < ny) & (cz >= 0) & (cz < nz) & finite
+                val = I[np.clip(cz, 0, nz - 1), np.clip(cy, 0, ny - 1), np.clip(cx, 0, nx - 1)]
+                out += np.where(ok, w * val, 0.0)
+    return out
+
+
+def warp_backward(iref, dvf, grid, grad_out):
+    """-> (dL/dI_ref [nz,ny,nx], dL/ddvf [B,3,nz,ny,nx]) fp64."""
+    _, h, dims = _grid(grid)
+    nx, ny, nz = (int(v) for v in dims)
+    I = np.asarray(_f32(iref), dtype=np.float64).reshape(nz, ny, nx)
+    base, f, finite = _warp_cells(dvf, h, dims)
+    B = base.shape[0]
+    g = np.asarray(_f32(grad_out), dtype=np.float64).reshape(B, nz, ny, nx)
+    gI = np.zeros(nz * ny * nx)
+    gd = np.zeros((B, 3, nz, ny, nx))
+    h64 = np.asarray(h, dtype=np.float64)
+    for az in (0, 1):
+        for ay in (0, 1):
+            for ax in (0, 1):
+                cx, cy, cz = base[:, 0] + ax, base[:, 1] + ay, base[:, 2] + az
+                wx = f[:, 0] if ax else 1.0 - f[:, 0]
+                wy = f[:, 1] if ay else 1.0 - f[:, 1]
+                wz = f[:, 2] if az else 1.0 - f[:, 2]
+                ok = (cx >= 0) & (cx < nx) & (cy >= 0) & (cy < ny) & (cz >= 0) & (cz < nz) & finite
+                lin = (np.clip(cz, 0, nz - 1) * ny + np.clip(cy, 0, ny - 1)) * nx + np.clip(cx, 0, nx - 1)
+                np.add.at(gI, lin[ok], (g * wx * wy * wz)[ok])
+                val = np.where(ok, I.reshape(-1)[lin], 0.0)
+                sx, sy, sz = (1.0 if ax else -1.0), (1.0 if ay else -1.0), (1.0 if az else -1.0)
+                gd[:, 0] += g * val * sx * wy * wz / h64[0]
+                gd[:, 1] += g * val * wx * sy * wz / h64[1]
+                gd[:, 2] += g * val * wx * wy * sz / h64[2]
+    return gI.reshape(nz, ny, nx), gd
