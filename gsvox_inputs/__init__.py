@@ -257,6 +257,64 @@ def dvf_case(batch=8, counts=(1_000, 8_000, 64_000), dims=(128, 128, 64), seed=5
                    np.ascontiguousarray(level, dtype=np.int32), _f32(coef), seed=seed)
 
 
+@dataclass
+class WarpCase:
+    """Inputs of the warp I(x,p) = I_ref(x + d(x,p)) (Eq. 2)."""
+    name: str
+    dims: tuple
+    iref: np.ndarray            # [nz,ny,nx] fp32
+    dvf: np.ndarray             # [B,3,nz,ny,nx] fp32, world units, components x,y,z
+    origin: tuple = (0.0, 0.0, 0.0)
+    spacing: tuple = (2.0, 2.0, 2.0)
+    seed: object = 0
+
+    @property
+    def batch(self):
+        return int(self.dvf.shape[0])
+
+    @property
+    def grid(self):
+        return (np.asarray(self.origin, np.float32), np.asarray(self.spacing, np.float32),
+                np.asarray(self.dims, np.int32))
+
+    def grad_out(self):
+        rng = np.random.default_rng([78, self.batch] + list(np.atleast_1d(self.seed)))
+        nx, ny, nz = self.dims
+        return rng.standard_normal((self.batch, nz, ny, nx), dtype=np.float32)
+
+
+def warp_case(batch=8, dims=(256, 256, 128), spacing=(2.0, 2.0, 2.0), amp_vox=4.0, seed=6, rough=0.15):
+    """Stand-in for a reference CBCT and a batch of breathing DVFs (2 mm voxels):
+    I_ref = an ellipsoidal body (0.45/0.35/0.48 of the grid, as config 2) of attenuation 0.2 with a
+    few low-frequency cosine modulations plus N(0, 0.01) noise, 0 outside; d = per-projection
+    amplitude U(-amp, amp) voxels per axis times a smooth cosine field, plus `rough` voxels of
+    white noise (so neighbouring samples do not share cells exactly); world units = voxels x spacing.
+    A thin shell of samples leaves the grid (zero padding is exercised)."""
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = dims
+    z, y, x = np.meshgrid(np.arange(nz, dtype=np.float32), np.arange(ny, dtype=np.float32),
+                          np.arange(nx, dtype=np.float32), indexing="ij")
+    c = (np.array([nx, ny, nz], np.float32) - 1) / 2
+    semi = np.array([0.45 * nx, 0.35 * ny, 0.48 * nz], np.float32)
+    r2 = ((x - c[0]) / semi[0]) ** 2 + ((y - c[1]) / semi[1]) ** 2 + ((z - c[2]) / semi[2]) ** 2
+    body = (r2 <= 1.0).astype(np.float32)
+    tex = np.zeros_like(body)
+    for _ in range(4):
+        k = rng.uniform(0.5, 4.0, size=3) * 2 * np.pi / np.array([nx, ny, nz])
+        ph = rng.uniform(0, 2 * np.pi)
+        tex += np.cos(k[0] * x + k[1] * y + k[2] * z + ph).astype(np.float32)
+    iref = body * (0.2 + 0.05 * tex) + rng.normal(0.0, 0.01, size=body.shape).astype(np.float32) * body
+    dvf = np.empty((batch, 3, nz, ny, nx), np.float32)
+    for b in range(batch):
+        for a in range(3):
+            k = rng.uniform(0.3, 1.5, size=3) * 2 * np.pi / np.array([nx, ny, nz])
+            ph = rng.uniform(0, 2 * np.pi)
+            field = np.cos(k[0] * x + k[1] * y + k[2] * z + ph)
+            field = rng.uniform(-amp_vox, amp_vox) * field + rough * rng.standard_normal(field.shape, dtype=np.float32)
+            dvf[b, a] = (field * spacing[a]).astype(np.float32)
+    return WarpCase("warp_b%d" % batch, tuple(dims), _f32(iref), dvf, spacing=tuple(spacing), seed=seed)
+
+
 FULL = {
     "config1": lambda: [config1()],
     "config2": lambda: [config2()],

@@ -186,6 +186,20 @@ int gsvox_mbc_combine_forward(const float* e, const float* coef, int32_t B, int3
 int gsvox_mbc_combine_backward(const float* e, const float* coef, const float* grad_dvf, int32_t B,
                                int32_t L, int64_t V, float* grad_e, float* grad_coef, void* stream);
 
+/* ---- the warp (Eq. 2) -------------------------------------
+ *     out[b, v] = I_ref(x_v + d[b, :, v]),   b = 0..B-1 projections of a batch
+ * iref [nz,ny,nx]; dvf [B,3,nz,ny,nx] with components in the order x,y,z and in WORLD units (the
+ * unit of grid->spacing; grid->origin cancels); out [B,nz,ny,nx] OVERWRITTEN.  Trilinear
+ * interpolation of the voxel-centre samples, corners outside the grid read 0, a non-finite
+ * displacement yields 0 (readings W1-W4).  All DEVICE pointers, no host sync.        */
+int gsvox_warp_forward(const float* iref, const float* dvf, const gsvox_grid* grid, int32_t B,
+                       float* out, void* stream);
+/* Backward for grad_out = dL/dout [B,nz,ny,nx]: grad_iref [nz,ny,nx] (OVERWRITTEN; summed over the
+ * batch with fp32 atomics, so run-to-run dependent in the last bits) and grad_dvf [B,3,nz,ny,nx]
+ * (OVERWRITTEN), the exact derivative of the piecewise-trilinear interpolant.                   */
+int gsvox_warp_backward(const float* iref, const float* dvf, const gsvox_grid* grid, int32_t B,
+                        const float* grad_out, float* grad_iref, float* grad_dvf, void* stream);
+
 /* Live ALU rooflines of the device the calling thread has current (the hot path is
  * FP32-issue / MUFU bound, and MEASURED_PEAKS.json holds no FP32 figure).  Runs three register-only
  * microbenchmarks on `stream` and SYNCHRONISES: scalar FFMA chains (fp32_tflops, 2 flops per lane

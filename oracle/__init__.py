@@ -304,7 +304,7 @@ def warp_backward(iref, dvf, grid, grad_out):
                 wz = f[:, 2] if az else 1.0 - f[:, 2]
                 ok = (cx >= 0) & (cx < nx) & (cy >= 0) & (cy < ny) & (cz >= 0) & (cz < nz) & finite
                 lin = (np.clip(cz, 0, nz - 1) * ny + np.clip(cy, 0, ny - 1)) * nx + np.clip(cx, 0, nx - 1)
-                np.add.at(gI, lin[ok], (g * wx * wy * wz)[ok])
+                gI += np.bincount(lin[ok], weights=(g * wx * wy * wz)[ok], minlength=gI.size)   # scatter-add
                 val = np.where(ok, I.reshape(-1)[lin], 0.0)
                 sx, sy, sz = (1.0 if ax else -1.0), (1.0 if ay else -1.0), (1.0 if az else -1.0)
                 gd[:, 0] += g * val * sx * wy * wz / h64[0]

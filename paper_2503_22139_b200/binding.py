@@ -20,7 +20,7 @@ EXPORTS = [
     "gsvox_plan_bins_host", "gsvox_plan_set_timing", "gsvox_plan_timings",
     "gsvox_host_staging_bytes", "gsvox_step_host", "gsvox_error_string",
     "gsvox_last_cuda_error", "gsvox_version", "gsvox_probe_peaks", "gsvox_dvf_forward", "gsvox_dvf_backward",
-    "gsvox_mbc_combine_forward", "gsvox_mbc_combine_backward",
+    "gsvox_mbc_combine_forward", "gsvox_mbc_combine_backward", "gsvox_warp_forward", "gsvox_warp_backward",
 ]
 
 
@@ -69,6 +69,8 @@ def lib():
     L.gsvox_dvf_backward.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.gsvox_mbc_combine_forward.argtypes = [vp, vp, i32, i32, i64, vp, vp]
     L.gsvox_mbc_combine_backward.argtypes = [vp, vp, vp, i32, i32, i64, vp, vp, vp]
+    L.gsvox_warp_forward.argtypes = [vp, vp, gp, i32, vp, vp]
+    L.gsvox_warp_backward.argtypes = [vp, vp, gp, i32, vp, vp, vp, vp]
     dp = C.POINTER(C.c_double)
     L.gsvox_probe_peaks.argtypes = [vp, dp, dp, dp, C.POINTER(i32), vp]
     L.gsvox_error_string.argtypes = [C.c_int]
@@ -142,6 +144,28 @@ def mbc_combine_backward(e, coef, grad_dvf, grads=None):
     ge, gc = grads
     _check(lib().gsvox_mbc_combine_backward(_dev(e, "e"), _dev(coef, "coef"), _dev(grad_dvf, "grad_dvf"), B, L_, V,
                                             _dev(ge, "grad_e"), _dev(gc, "grad_coef"), _stream()))
+    return grads
+
+
+def warp_forward(iref, dvf, grid, out=None):
+    """iref [nz,ny,nx], dvf [B,3,nz,ny,nx] (world units), grid = (origin, spacing, dims) -> [B,nz,ny,nx]."""
+    g = make_grid(*grid)
+    B = int(dvf.shape[0])
+    if out is None:
+        out = torch.empty((B,) + tuple(iref.shape), dtype=torch.float32, device=iref.device)
+    _check(lib().gsvox_warp_forward(_dev(iref, "iref"), _dev(dvf, "dvf"), C.byref(g), B, _dev(out, "out"), _stream()))
+    return out
+
+
+def warp_backward(iref, dvf, grid, grad_out, grads=None):
+    """-> (grad_iref [nz,ny,nx], grad_dvf [B,3,nz,ny,nx])."""
+    g = make_grid(*grid)
+    B = int(dvf.shape[0])
+    if grads is None:
+        grads = (torch.empty_like(iref), torch.empty_like(dvf))
+    gi, gd = grads
+    _check(lib().gsvox_warp_backward(_dev(iref, "iref"), _dev(dvf, "dvf"), C.byref(g), B, _dev(grad_out, "grad_out"),
+                                     _dev(gi, "grad_iref"), _dev(gd, "grad_dvf"), _stream()))
     return grads
 
 

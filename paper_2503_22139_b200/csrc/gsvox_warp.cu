@@ -1,0 +1,215 @@
+// gsvox_warp.cu — SURVEY.md 8(f) rank 2: the warp  I(x,p) = I_ref(x + d(x,p))  (Eq. 2;
+// :136 "we applied DVFs derived from the MBC motion model to yield time-resolved dynamic CBCTs"),
+// batched over the B projections of a training batch, forward and backward.
+//
+// Readings W1-W4: trilinear interpolation of the voxel-centre samples; a corner outside
+// the grid contributes 0; d is in world units, the sample sits at index u_k = i_k + d_k / h_k; the
+// cell index is decided on t_k = d_k / h_k in fp32 (IEEE division, floor; the fraction t - floor t
+// is exact), so positions far from the origin lose nothing to the magnitude of i_k; a non-finite
+// displacement yields 0 and zero gradients.
+//
+// HBM/L2-bound gather.  One thread per output voxel, x fastest: the three d loads, the g load and
+// the store are coalesced; the eight corner reads hit L1/L2 (I_ref is 33 MB at 256x256x128, inside
+// the 126 MB L2, and neighbouring threads read neighbouring cells).  Algorithmic bytes per output
+// voxel: forward 12 (d) + 4 (out) + 4/B (I_ref once per batch); backward 4 (g) + 12 (d) + 12
+// (grad d) + 8/B (I_ref read, grad I_ref written) — the eight `red.global.add.f32` per voxel land
+// in L2.
+#include "gsvox_internal.cuh"
+
+namespace gsvox {
+
+constexpr int kWarpThreads = 256;
+
+struct WarpGrid { int nx, ny, nz; float inv_hx, inv_hy, inv_hz; float hx, hy, hz; };
+
+// Cell of one sample: base corner (may be outside the grid) and fractions; false if non-finite.
+__device__ __forceinline__ bool warp_cell(float dx, float dy, float dz, const WarpGrid& wg, int x, int y, int z,
+                                          int& cx, int& cy, int& cz, float& fx, float& fy, float& fz)
+{
+    const float tx = __fdiv_rn(dx, wg.hx), ty = __fdiv_rn(dy, wg.hy), tz = __fdiv_rn(dz, wg.hz);
+    // |t| < 1e9 also rejects NaN (comparison false) and inf
+    const bool ok = (fabsf(tx) < 1.0e9f) && (fabsf(ty) < 1.0e9f) && (fabsf(tz) < 1.0e9f);
+    const float flx = floorf(tx), fly = floorf(ty), flz = floorf(tz);
+    fx = ok ? tx - flx : 0.f; fy = ok ? ty - fly : 0.f; fz = ok ? tz - flz : 0.f;
+    cx = ok ? x + (int)flx : x; cy = ok ? y + (int)fly : y; cz = ok ? z + (int)flz : z;
+    return ok;
+}
+
+// Eight-corner gather of one sample; corners outside the grid read 0.
+__device__ __forceinline__ float warp_sample(const float* __restrict__ iref, const WarpGrid& wg,
+                                             int cx, int cy, int cz, float fx, float fy, float fz)
+{
+    float acc = 0.f;
+    #pragma unroll
+    for (int az = 0; az < 2; ++az) {
+        const int zz = cz + az;
+        const float wz = az ? fz : 1.f - fz;
+        #pragma unroll
+        for (int ay = 0; ay < 2; ++ay) {
+            const int yy = cy + ay;
+            const float wyz = wz * (ay ? fy : 1.f - fy);
+            const bool rowok = ((unsigned)zz < (unsigned)wg.nz) && ((unsigned)yy < (unsigned)wg.ny);
+            const float* row = iref + ((size_t)(rowok ? zz : 0) * wg.ny + (rowok ? yy : 0)) * wg.nx;
+            const float v0 = (rowok && (unsigned)cx < (unsigned)wg.nx) ? __ldg(row + cx) : 0.f;
+            const float v1 = (rowok && (unsigned)(cx + 1) < (unsigned)wg.nx) ? __ldg(row + cx + 1) : 0.f;
+            acc = fmaf(wyz, fmaf(fx, v1 - v0, v0), acc);
+        }
+    }
+    return acc;
+}
+
+// VPT consecutive x per thread (4: 128-bit loads of d and a 128-bit store; needs nx % 4 == 0).
+// 32-bit index arithmetic: V < 2^31 is checked on the host.
+template <int VPT>
+__global__ void __launch_bounds__(kWarpThreads)
+k_warp_forward(const float* __restrict__ iref, const float* __restrict__ dvf, WarpGrid wg, int B,
+               float* __restrict__ out)
+{
+    const unsigned V = (unsigned)wg.nx * wg.ny * wg.nz;
+    const unsigned v = (blockIdx.x * kWarpThreads + threadIdx.x) * VPT;
+    const int b = blockIdx.y;
+    if (v >= V) return;
+    const unsigned row = v / (unsigned)wg.nx;
+    const int x = (int)(v - row * wg.nx), z = (int)(row / (unsigned)wg.ny), y = (int)(row - (unsigned)z * wg.ny);
+    const float* d = dvf + (size_t)b * 3 * V;
+    float dx[VPT], dy[VPT], dz[VPT], res[VPT];
+    if (VPT == 4) {
+        const float4 a = __ldcs(reinterpret_cast<const float4*>(d + v));
+        const float4 c = __ldcs(reinterpret_cast<const float4*>(d + V + v));
+        const float4 e = __ldcs(reinterpret_cast<const float4*>(d + 2 * (size_t)V + v));
+        dx[0] = a.x; dx[VPT - 1] = a.w; dy[0] = c.x; dy[VPT - 1] = c.w; dz[0] = e.x; dz[VPT - 1] = e.w;
+        if (VPT > 2) { dx[1] = a.y; dx[2] = a.z; dy[1] = c.y; dy[2] = c.z; dz[1] = e.y; dz[2] = e.z; }
+    } else {
+        dx[0] = __ldcs(d + v); dy[0] = __ldcs(d + V + v); dz[0] = __ldcs(d + 2 * (size_t)V + v);
+    }
+    #pragma unroll
+    for (int j = 0; j < VPT; ++j) {
+        int cx, cy, cz; float fx, fy, fz;
+        const bool ok = warp_cell(dx[j], dy[j], dz[j], wg, x + j, y, z, cx, cy, cz, fx, fy, fz);
+        res[j] = ok ? warp_sample(iref, wg, cx, cy, cz, fx, fy, fz) : 0.f;
+    }
+    float* o = out + (size_t)b * V + v;
+    if (VPT == 4) __stcs(reinterpret_cast<float4*>(o), make_float4(res[0], res[1 % VPT], res[2 % VPT], res[3 % VPT]));
+    else __stcs(o, res[0]);
+}
+
+__device__ __forceinline__ void red_add(float* addr, float v)
+{
+    asm volatile("red.global.add.f32 [%0], %1;" :: "l"(addr), "f"(v) : "memory");
+}
+
+// One thread per voxel, lanes along x, so the atomics of a warp are contiguous.  Neighbouring samples
+// of a smooth DVF sit in neighbouring cells: lane l's right-hand corner is lane l+1's left-hand one.
+// Those two contributions are merged with a shuffle before they leave the SM, which halves the
+// `red.global.add.f32` count (8 -> ~4 per voxel); a lane keeps its own left-hand add only when its
+// left neighbour did not take it.  (Four x per thread, as in the forward kernel, strides the
+// atomics and measured 40 % slower.)
+__global__ void __launch_bounds__(kWarpThreads)
+k_warp_backward(const float* __restrict__ iref, const float* __restrict__ dvf, const float* __restrict__ gout,
+                WarpGrid wg, int B, float* __restrict__ giref, float* __restrict__ gdvf)
+{
+    const unsigned V = (unsigned)wg.nx * wg.ny * wg.nz;
+    const unsigned v = blockIdx.x * kWarpThreads + threadIdx.x;
+    const int b = blockIdx.y;
+    const bool live = v < V;
+    const unsigned vv = live ? v : 0u;
+    const unsigned row = vv / (unsigned)wg.nx;
+    const int x = (int)(vv - row * wg.nx), z = (int)(row / (unsigned)wg.ny), y = (int)(row - (unsigned)z * wg.ny);
+    const float* d = dvf + (size_t)b * 3 * V;
+    float dx = 0.f, dy = 0.f, dz = 0.f, g = 0.f;
+    if (live) {
+        dx = __ldcs(d + v); dy = __ldcs(d + V + v); dz = __ldcs(d + 2 * (size_t)V + v);
+        g = __ldcs(gout + (size_t)b * V + v);
+    }
+    int cx, cy, cz; float fx, fy, fz;
+    const bool ok = warp_cell(dx, dy, dz, wg, x, y, z, cx, cy, cz, fx, fy, fz) && live;
+    // does lane+1 continue my cell row?  (same y,z cell, x cell one further, both valid)
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const int ncx = __shfl_down_sync(full, cx, 1), ncy = __shfl_down_sync(full, cy, 1), ncz = __shfl_down_sync(full, cz, 1);
+    const int nok = __shfl_down_sync(full, (int)ok, 1);
+    const bool take_next = ok && nok && (lane < 31) && (ncx == cx + 1) && (ncy == cy) && (ncz == cz);
+    const bool taken = __shfl_up_sync(full, (int)take_next, 1) && (lane > 0);       // my left add is done by lane-1
+    if (!ok) g = 0.f;                                               // non-finite displacement: zero gradients
+    float gx = 0.f, gy = 0.f, gz = 0.f;
+    #pragma unroll
+    for (int az = 0; az < 2; ++az) {
+        const int zz = cz + az;
+        const float wz = az ? fz : 1.f - fz, sz = az ? 1.f : -1.f;
+        #pragma unroll
+        for (int ay = 0; ay < 2; ++ay) {
+            const int yy = cy + ay;
+            const float wy = ay ? fy : 1.f - fy, sy = ay ? 1.f : -1.f;
+            const bool rowok = ok && ((unsigned)zz < (unsigned)wg.nz) && ((unsigned)yy < (unsigned)wg.ny);
+            const size_t rowoff = ((size_t)(rowok ? zz : 0) * wg.ny + (rowok ? yy : 0)) * wg.nx;
+            const bool ok0 = rowok && (unsigned)cx < (unsigned)wg.nx, ok1 = rowok && (unsigned)(cx + 1) < (unsigned)wg.nx;
+            const float v0 = ok0 ? __ldg(iref + rowoff + cx) : 0.f;
+            const float v1 = ok1 ? __ldg(iref + rowoff + cx + 1) : 0.f;
+            const float gwyz = g * wy * wz;
+            const float a0 = gwyz * (1.f - fx);
+            float a1 = gwyz * fx;
+            const float na0 = __shfl_down_sync(full, a0, 1);          // lane+1's left-hand contribution, same address
+            if (take_next) a1 += na0;
+            if (ok0 && !taken) red_add(giref + rowoff + cx, a0);
+            if (ok1) red_add(giref + rowoff + cx + 1, a1);
+            const float lin = fmaf(fx, v1 - v0, v0);                  // interpolated along x
+            gx = fmaf(wy * wz, v1 - v0, gx);
+            gy = fmaf(sy * wz, lin, gy);
+            gz = fmaf(wy * sz, lin, gz);
+        }
+    }
+    if (live) {
+        float* gd = gdvf + (size_t)b * 3 * V;
+        __stcs(gd + v, g * gx * wg.inv_hx); __stcs(gd + V + v, g * gy * wg.inv_hy);
+        __stcs(gd + 2 * (size_t)V + v, g * gz * wg.inv_hz);
+    }
+}
+
+}  // namespace gsvox
+
+using namespace gsvox;
+
+static int warp_grid(const gsvox_grid* g, int32_t B, WarpGrid* wg)
+{
+    if (!g || B < 1 || B > 65535) return GSVOX_EINVAL;
+    for (int k = 0; k < 3; ++k)
+        if (!(g->spacing[k] > 0.f) || g->dims[k] < 1 || g->dims[k] > GSVOX_MAX_DIM) return GSVOX_EINVAL;
+    wg->nx = g->dims[0]; wg->ny = g->dims[1]; wg->nz = g->dims[2];
+    wg->hx = g->spacing[0]; wg->hy = g->spacing[1]; wg->hz = g->spacing[2];
+    wg->inv_hx = 1.f / g->spacing[0]; wg->inv_hy = 1.f / g->spacing[1]; wg->inv_hz = 1.f / g->spacing[2];
+    if ((long long)wg->nx * wg->ny * wg->nz >= (1LL << 31)) return GSVOX_ELIMIT;     // 32-bit voxel indices
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_warp_forward(const float* iref, const float* dvf, const gsvox_grid* grid, int32_t B,
+                                  float* out, void* stream)
+{
+    WarpGrid wg;
+    int rc = warp_grid(grid, B, &wg);
+    if (rc != GSVOX_OK) return rc;
+    if (!iref || !dvf || !out) return GSVOX_EINVAL;
+    const long long V = (long long)wg.nx * wg.ny * wg.nz;
+    const bool vec = (wg.nx % 4 == 0) && ((((uintptr_t)dvf | (uintptr_t)out) & 15) == 0);
+    const long long items = vec ? V / 4 : V;
+    dim3 gridDim((unsigned)((items + kWarpThreads - 1) / kWarpThreads), (unsigned)B);
+    if (vec) k_warp_forward<4><<<gridDim, kWarpThreads, 0, (cudaStream_t)stream>>>(iref, dvf, wg, B, out);
+    else     k_warp_forward<1><<<gridDim, kWarpThreads, 0, (cudaStream_t)stream>>>(iref, dvf, wg, B, out);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_warp_backward(const float* iref, const float* dvf, const gsvox_grid* grid, int32_t B,
+                                   const float* grad_out, float* grad_iref, float* grad_dvf, void* stream)
+{
+    WarpGrid wg;
+    int rc = warp_grid(grid, B, &wg);
+    if (rc != GSVOX_OK) return rc;
+    if (!iref || !dvf || !grad_out || !grad_iref || !grad_dvf) return GSVOX_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long V = (long long)wg.nx * wg.ny * wg.nz;
+    GSVOX_CUDA(cudaMemsetAsync(grad_iref, 0, sizeof(float) * (size_t)V, st));
+    dim3 gridDim((unsigned)((V + kWarpThreads - 1) / kWarpThreads), (unsigned)B);
+    k_warp_backward<<<gridDim, kWarpThreads, 0, st>>>(iref, dvf, grad_out, wg, B, grad_iref, grad_dvf);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
