@@ -178,6 +178,107 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------- rows of SURVEY 8(f) built so far
+def _time_ms(torch, fn, iters, warm=3):
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(iters):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / iters
+
+
+def next_rows(torch, pkg, hbm_peak_gbs, quick=False):
+    """8(f) rank 1 (MBC -> DVF, two-stage) and rank 2 (warp) at their full sizes: ms and, for the
+    HBM-bound kernels, algorithmic GB/s against the measured copy bandwidth (DESIGN.md sections 10-11)."""
+    import gsvox_inputs
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    res = {}
+    if quick:                      # one launch of everything (ncu captures of the 8(f) kernels)
+        global _time_ms
+        full_time = _time_ms
+        _time_ms = lambda torch_, fn, iters, warm=3: full_time(torch_, fn, 1, warm=0)
+    # ---- rank 1: three config-3 levels voxelized separately (C = 3) + combine, B = 8 projections
+    case = gsvox_inputs.dvf_case(batch=8)
+    lv, _ = case.levels()
+    nx, ny, nz = case.dims
+    V, L, B = nx * ny * nz, case.nlevels, case.batch
+    e = torch.empty((L, 3, nz, ny, nx), dtype=torch.float32, device="cuda")
+    plans, P, pairs = [], [], 0
+    for i, (p, s, q, f) in enumerate(lv):
+        t = (dev(p), dev(s), dev(q), dev(f))
+        plan = pkg.Plan(len(p), case.grid, max_channels=3)
+        plan.preprocess(*t[:3])
+        st = plan.status()
+        if st["overflow"]:
+            plan = pkg.Plan(len(p), case.grid, max_channels=3, key_capacity=int(1.05 * st["keys_needed"]))
+            plan.preprocess(*t[:3])
+            st = plan.status()
+        pairs += st["pairs"]
+        plans.append(plan); P.append(t)
+    coef, g = dev(case.coef), dev(case.grad_dvf())
+    d = torch.empty((B, 3, nz, ny, nx), dtype=torch.float32, device="cuda")
+    ge, gc = torch.empty_like(e), torch.empty((B, L, 3), dtype=torch.float32, device="cuda")
+    gr = [None] * L
+
+    def dvf_step():
+        for i in range(L):
+            plans[i].preprocess(*P[i][:3])
+            plans[i].forward(P[i][3], out=e[i])
+        pkg.mbc_combine_forward(e, coef, out=d)
+        pkg.mbc_combine_backward(e, coef, g, grads=(ge, gc))
+        for i in range(L):
+            gr[i] = plans[i].backward(P[i][3], ge[i], grads=gr[i])
+    ms = _time_ms(torch, dvf_step, 10)
+    mf = _time_ms(torch, lambda: pkg.mbc_combine_forward(e, coef, out=d), 50)
+    mb = _time_ms(torch, lambda: pkg.mbc_combine_backward(e, coef, g, grads=(ge, gc)), 50)
+    bf, bb = 4 * V * (3 * L + 3 * B), 4 * V * (3 * B + 6 * L)
+    res["dvf_two_stage"] = {
+        "workload": "3 MBC levels (1k/8k/64k Gaussians, C=3 each) on 128x128x64 + Eq. 3 combine, B=8, fwd+bwd",
+        "ms_per_step": ms, "pairs_P_def": pairs, "pair_channels_per_s": 3 * pairs / (ms * 1e-3),
+        "combine_forward": {"ms": mf, "bytes": bf, "GBps": bf / mf / 1e6, "frac_of_hbm_peak": bf / mf / 1e6 / hbm_peak_gbs,
+                            "note": "38 MB working set: L2-resident at this size"},
+        "combine_backward": {"ms": mb, "bytes": bb, "GBps": bb / mb / 1e6, "frac_of_hbm_peak": bb / mb / 1e6 / hbm_peak_gbs}}
+    # the same combine beyond L2 (256^3 volumes, 1.6 GB working set): the HBM roofline proper
+    shape = (256, 256, 256)
+    Vb = shape[0] * shape[1] * shape[2]
+    eb = torch.randn((L, 3) + shape, device="cuda"); gb = torch.randn((B, 3) + shape, device="cuda")
+    db = torch.empty((B, 3) + shape, device="cuda"); geb = torch.empty_like(eb)
+    mf = _time_ms(torch, lambda: pkg.mbc_combine_forward(eb, coef, out=db), 20)
+    mb = _time_ms(torch, lambda: pkg.mbc_combine_backward(eb, coef, gb, grads=(geb, gc)), 20)
+    bf, bb = 4 * Vb * (3 * L + 3 * B), 4 * Vb * (3 * B + 6 * L)
+    res["mbc_combine_256cubed_b8"] = {
+        "forward": {"ms": mf, "bytes": bf, "GBps": bf / mf / 1e6, "frac_of_hbm_peak": bf / mf / 1e6 / hbm_peak_gbs},
+        "backward": {"ms": mb, "bytes": bb, "GBps": bb / mb / 1e6, "frac_of_hbm_peak": bb / mb / 1e6 / hbm_peak_gbs}}
+    del eb, gb, db, geb
+    # ---- rank 2: warp of a 256x256x128 reference volume by B = 8 DVFs
+    wc = gsvox_inputs.warp_case(batch=8)
+    nx, ny, nz = wc.dims
+    Vw = nx * ny * nz
+    iref, dvf, gw = dev(wc.iref), dev(wc.dvf), dev(wc.grad_out())
+    out = torch.empty((8, nz, ny, nx), dtype=torch.float32, device="cuda")
+    gi, gd = torch.empty_like(iref), torch.empty_like(dvf)
+    mf = _time_ms(torch, lambda: pkg.warp_forward(iref, dvf, wc.grid, out=out), 20)
+    mb = _time_ms(torch, lambda: pkg.warp_backward(iref, dvf, wc.grid, gw, grads=(gi, gd)), 20)
+    bf, bb = 4 * Vw * (4 * 8 + 1), 4 * Vw * (7 * 8 + 2)
+    res["warp_256x256x128_b8"] = {
+        "forward": {"ms": mf, "bytes": bf, "GBps": bf / mf / 1e6, "frac_of_hbm_peak": bf / mf / 1e6 / hbm_peak_gbs},
+        "backward": {"ms": mb, "bytes": bb, "GBps": bb / mb / 1e6, "frac_of_hbm_peak": bb / mb / 1e6 / hbm_peak_gbs,
+                     "note": "8 fp32 atomics per voxel into grad I_ref (L2), merged pairwise by shuffle"}}
+    return res
+
+
+def hbm_peak():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6545.0, "fallback (B200_PROFILING.md measured copy bandwidth)"
+
+
 # ------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import torch
@@ -188,6 +289,12 @@ def run_ours(args):
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     pkg.lib()
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    if args.only_next_rows:
+        pk, src = hbm_peak()
+        extra = next_rows(torch, pkg, pk, quick=True)
+        extra["hbm_peak_GBps"] = pk
+        print(json.dumps({"next_rows": extra, "note": "single launches (profiling mode), not a benchmark"}), flush=True)
+        return
     ranks = Ranks(backend="nccl")
     rank, world, local = ranks.rank, ranks.world, ranks.local
     barrier = ranks.barrier
@@ -299,11 +406,19 @@ def run_ours(args):
                    "seconds": dt, "sample": "every %d-th Gaussian of %s (%d pairs), full grid, forward+backward, fp64"
                    % (stride, case.name, cp)}
 
+        extra = None
+        if not args.no_next_rows and args.config == 4:
+            pk, src = hbm_peak()
+            extra = next_rows(torch, pkg, pk)
+            extra["hbm_peak_GBps"] = pk
+            extra["hbm_peak_source"] = src
+
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": workload_config(case, {"pairs_P_def": pairs, "keys": keys}),
-                "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu}
+                "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
+                "next_rows": extra}
     ranks.close()
     if line is not None:
         print(json.dumps(line), flush=True)
@@ -317,6 +432,9 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=4, help="4 (headline), 1, 2, 5, or 31/32/33 for config 3 levels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the SURVEY 8(f) rows (DVF combine, warp)")
+    ap.add_argument("--only-next-rows", action="store_true",
+                    help="launch every 8(f) kernel once and exit (for ncu captures; prints no benchmark line)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
