@@ -23,7 +23,8 @@
 namespace gsvox {
 
 constexpr int kFwdThreads = 64;
-constexpr int kFwdBatch = 64;
+constexpr int kFwdBatch = 64;      // keys staged per __syncthreads.  Measured on config 4: batch 32/48 and forcing
+                                   // 24-32 resident CTAs (<= 40 / 32 registers) are 2-25 % slower than this.
 
 __device__ __forceinline__ float ex2f(float x)
 {
@@ -194,7 +195,7 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
     for (uint32_t base = kbeg; base < kend; base += kFwdBatch, buf ^= 1) {
         float* sb = s_rec[buf];
         uint32_t k = base + tid;
-        if (k < kend) stage_key<CH>(sb + tid * W, &s_mask[buf][0][tid], &s_mask[buf][1][tid], rec, weight, wstride,
+        if (tid < kFwdBatch && k < kend) stage_key<CH>(sb + tid * W, &s_mask[buf][0][tid], &s_mask[buf][1][tid], rec, weight, wstride,
                                     c0, keys[k], b0x, b0y, b0z);
         __syncthreads();
         const uint32_t* mk = s_mask[buf][wsel];
