@@ -283,7 +283,7 @@ def hbm_peak():
 def run_ours(args):
     import torch
     import paper_2503_22139_b200 as pkg
-    from paper_2503_22139_b200.dist import Ranks, whole_job_rate
+    from paper_2503_22139_b200.dist import Ranks, sharded_backward, slab_bounds, whole_job_rate
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
@@ -307,11 +307,18 @@ def run_ours(args):
     grad = dev(grad_np)
     nx, ny, nz = case.dims
 
+    slab = None
+    if args.shard == "slab":                     # z-slabs of bricks per rank + one all-reduce in backward
+        slab = slab_bounds((nz + 7) // 8, rank, world)
     plan = pkg.Plan(case.n, case.grid, max_channels=C)
+    if slab:
+        plan.set_slab(*slab)
     plan.preprocess(pos, scale, quat)
     st = plan.status()
     if st["overflow"]:
         plan = pkg.Plan(case.n, case.grid, max_channels=C, key_capacity=int(1.05 * st["keys_needed"]))
+        if slab:
+            plan.set_slab(*slab)
         plan.preprocess(pos, scale, quat)
         st = plan.status()
     assert not st["overflow"]
@@ -322,7 +329,10 @@ def run_ours(args):
     def step():
         plan.preprocess(pos, scale, quat)
         plan.forward(w, out=out)
-        plan.backward(w, grad, grads=grads)
+        if slab:
+            sharded_backward(plan, w, grad, ranks, grads=grads)
+        else:
+            plan.backward(w, grad, grads=grads)
 
     for _ in range(max(3, args.warmup)):
         step()
@@ -344,7 +354,11 @@ def run_ours(args):
     ms_total = ev0.elapsed_time(ev1)
     _, launches = plan.timings(reset=True)
     n_launch = sum(launches.values())
-    value, ms_step = whole_job_rate(pairs, ranks, ms_total, args.steps)
+    if slab:                                     # strong scaling: the job is ONE 256^3 step split over the ranks
+        ms_step = ranks.max_over_ranks(ms_total) / args.steps
+        value = pairs / (ms_step * 1e-3)
+    else:
+        value, ms_step = whole_job_rate(pairs, ranks, ms_total, args.steps)
 
     line = None
     if rank == 0:
@@ -415,8 +429,9 @@ def run_ours(args):
 
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": workload_config(case, {"pairs_P_def": pairs, "keys": keys}),
+                "scaling": "strong" if slab else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": workload_config(case, {"pairs_P_def": pairs, "keys": keys,
+                                                 "parallelism": "z-slabs + all-reduce" if slab else "replicas"}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
                 "next_rows": extra}
     ranks.close()
@@ -431,6 +446,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=4, help="4 (headline), 1, 2, 5, or 31/32/33 for config 3 levels")
+    ap.add_argument("--shard", choices=["replicas", "slab"], default="replicas",
+                    help="N > 1: independent replicas (default, weak scaling) or z-slabs of bricks per rank with one "
+                         "NCCL all-reduce of the per-Gaussian accumulators in backward (strong scaling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the SURVEY 8(f) rows (DVF combine, warp)")
     ap.add_argument("--only-next-rows", action="store_true",

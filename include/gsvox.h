@@ -147,6 +147,25 @@ int gsvox_step_host(gsvox_plan* plan, void* staging, size_t staging_bytes,
                     float* grad_weight_host, float* grad_pos_host, float* grad_scale_host,
                     float* grad_quat_host, void* stream);
 
+/* ---- Multi-GPU z-slabs ------------------------------------
+ * One process per GPU; every rank holds all Gaussian parameters and owns a contiguous range of
+ * brick layers along z.  gsvox_plan_set_slab restricts a2/a3/a4 of this plan to brick layers
+ * [bz_begin, bz_end) (0 <= bz_begin <= bz_end <= ceil(nz/8); an empty range is allowed); call it
+ * before gsvox_preprocess.  Forward then writes only the voxels of its slab (no collective: the
+ * slabs are disjoint).  Backward is split so that the caller can sum the per-Gaussian accumulators
+ * over ranks (NCCL all-reduce on the buffer gsvox_plan_accumulators returns) between the two halves:
+ *     gsvox_backward_accumulate  ->  all-reduce(acc, count floats, sum)  ->  gsvox_backward_finish
+ * gsvox_backward = accumulate + finish on one GPU.  status.pairs stays the whole-grid P_def;
+ * status.keys_needed counts the slab's keys.                                                    */
+int gsvox_plan_set_slab(gsvox_plan* plan, int32_t bz_begin, int32_t bz_end);
+int gsvox_backward_accumulate(gsvox_plan* plan, const float* weight, int32_t channels,
+                              const float* grad_out, void* stream);
+int gsvox_backward_finish(gsvox_plan* plan, int32_t channels, float* grad_weight, float* grad_pos,
+                          float* grad_scale, float* grad_quat, void* stream);
+/* DEVICE pointer to the [n, round4(9 + C)] fp32 accumulators of the latest preprocess and their
+ * number (the all-reduce payload: 24 MB at config 4).  HOST output pointers.                     */
+int gsvox_plan_accumulators(gsvox_plan* plan, int32_t channels, float** acc, int64_t* count);
+
 /* ---- motion-basis components -> deformation vector fields, fused ----
  * PAPER.md:58-61 (Eq. 3)  d(x,p) = sum_i w_i(p) e_i(x);  PAPER.md:106: three spatial levels i, each
  * with one MBC volume per Cartesian direction k (nine volumes), each level its own Gaussian set;

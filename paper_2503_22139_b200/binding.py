@@ -21,6 +21,7 @@ EXPORTS = [
     "gsvox_host_staging_bytes", "gsvox_step_host", "gsvox_error_string",
     "gsvox_last_cuda_error", "gsvox_version", "gsvox_probe_peaks", "gsvox_dvf_forward", "gsvox_dvf_backward",
     "gsvox_mbc_combine_forward", "gsvox_mbc_combine_backward", "gsvox_warp_forward", "gsvox_warp_backward",
+    "gsvox_plan_set_slab", "gsvox_backward_accumulate", "gsvox_backward_finish", "gsvox_plan_accumulators",
 ]
 
 
@@ -71,6 +72,10 @@ def lib():
     L.gsvox_mbc_combine_backward.argtypes = [vp, vp, vp, i32, i32, i64, vp, vp, vp]
     L.gsvox_warp_forward.argtypes = [vp, vp, gp, i32, vp, vp]
     L.gsvox_warp_backward.argtypes = [vp, vp, gp, i32, vp, vp, vp, vp]
+    L.gsvox_plan_set_slab.argtypes = [vp, i32, i32]
+    L.gsvox_backward_accumulate.argtypes = [vp, vp, i32, vp, vp]
+    L.gsvox_backward_finish.argtypes = [vp, i32, vp, vp, vp, vp, vp]
+    L.gsvox_plan_accumulators.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(i64)]
     dp = C.POINTER(C.c_double)
     L.gsvox_probe_peaks.argtypes = [vp, dp, dp, dp, C.POINTER(i32), vp]
     L.gsvox_error_string.argtypes = [C.c_int]
@@ -229,6 +234,32 @@ class Plan:
         _check(lib().gsvox_backward(self._h, _dev(weight, "weight"), ch, _dev(grad_out, "grad_out"),
                                     _dev(gw, "grad_weight"), _dev(gp, "grad_pos"), _dev(gs, "grad_scale"),
                                     _dev(gq, "grad_quat"), _stream()))
+        return grads
+
+    # --- multi-GPU z-slabs --------------------------------------
+    def set_slab(self, bz_begin, bz_end):
+        _check(lib().gsvox_plan_set_slab(self._h, int(bz_begin), int(bz_end)))
+        self.n = None
+
+    def backward_accumulate(self, weight, grad_out):
+        ch = int(weight.shape[1])
+        _check(lib().gsvox_backward_accumulate(self._h, _dev(weight, "weight"), ch, _dev(grad_out, "grad_out"), _stream()))
+
+    def accumulators(self, channels):
+        """torch view (no copy) of the [n, round4(9 + C)] accumulators: the all-reduce payload."""
+        ptr, cnt = C.c_void_p(None), C.c_int64(0)
+        _check(lib().gsvox_plan_accumulators(self._h, int(channels), C.byref(ptr), C.byref(cnt)))
+        off = int(ptr.value) - self.workspace.data_ptr()
+        return self.workspace[off:off + 4 * int(cnt.value)].view(torch.float32)
+
+    def backward_finish(self, channels, grads=None):
+        n = self.n
+        if grads is None:
+            mk = lambda k: torch.empty((n, k), dtype=torch.float32, device=self.device)
+            grads = (mk(channels), mk(3), mk(3), mk(4))
+        gw, gp, gs, gq = grads
+        _check(lib().gsvox_backward_finish(self._h, int(channels), _dev(gw, "grad_weight"), _dev(gp, "grad_pos"),
+                                           _dev(gs, "grad_scale"), _dev(gq, "grad_quat"), _stream()))
         return grads
 
     # --- 8(f) rank 1: fused MBC -> DVF ------------------------------------------------

@@ -117,6 +117,7 @@ extern "C" int gsvox_plan_create(int64_t n_max, int32_t max_channels, const gsvo
         p->gd.dims[k] = grid->dims[k]; p->gd.nb[k] = L.nb[k];
     }
     p->gd.nbricks = L.nbricks;
+    p->gd.slab0 = 0; p->gd.slab1 = L.nb[2];
     p->n_max = n_max; p->max_channels = max_channels; p->key_capacity = key_capacity; p->n = -1;
     char* w = (char*)workspace;
     p->status = (DevStatus*)(w + L.status); p->rec = (GsRec*)(w + L.rec); p->aux = (GsAux*)(w + L.aux);
@@ -167,4 +168,42 @@ extern "C" int gsvox_backward(gsvox_plan* p, const float* weight, int32_t channe
     if (p->n == 0) return GSVOX_OK;
     if (!weight || !grad_out || !gw || !gp || !gs || !gq) return GSVOX_EINVAL;
     return launch_backward(p, weight, channels, grad_out, gw, gp, gs, gq, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------ multi-GPU z-slabs
+extern "C" int gsvox_plan_set_slab(gsvox_plan* p, int32_t bz_begin, int32_t bz_end)
+{
+    if (!p || bz_begin < 0 || bz_end < bz_begin || bz_end > p->gd.nb[2]) return GSVOX_EINVAL;
+    p->gd.slab0 = bz_begin; p->gd.slab1 = bz_end;
+    p->n = -1;                                   // the binning of the previous slab is stale
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_backward_accumulate(gsvox_plan* p, const float* weight, int32_t channels,
+                                         const float* grad_out, void* stream)
+{
+    if (!p || channels < 1 || channels > p->max_channels) return GSVOX_EINVAL;
+    if (p->n < 0) return GSVOX_ENOTREADY;
+    if (p->n == 0) return GSVOX_OK;
+    if (!weight || !grad_out) return GSVOX_EINVAL;
+    return launch_backward_accumulate(p, weight, channels, grad_out, (cudaStream_t)stream);
+}
+
+extern "C" int gsvox_backward_finish(gsvox_plan* p, int32_t channels, float* gw, float* gp, float* gs,
+                                     float* gq, void* stream)
+{
+    if (!p || channels < 1 || channels > p->max_channels) return GSVOX_EINVAL;
+    if (p->n < 0) return GSVOX_ENOTREADY;
+    if (p->n == 0) return GSVOX_OK;
+    if (!gw || !gp || !gs || !gq) return GSVOX_EINVAL;
+    return launch_epilogue(p, channels, gw, gp, gs, gq, (cudaStream_t)stream);
+}
+
+extern "C" int gsvox_plan_accumulators(gsvox_plan* p, int32_t channels, float** acc, int64_t* count)
+{
+    if (!p || !acc || !count || channels < 1 || channels > p->max_channels) return GSVOX_EINVAL;
+    if (p->n < 0) return GSVOX_ENOTREADY;
+    *acc = p->acc;
+    *count = p->n * (int64_t)acc_stride(channels);
+    return GSVOX_OK;
 }

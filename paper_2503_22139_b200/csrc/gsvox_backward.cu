@@ -143,7 +143,7 @@ k_backward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start
 {
     __shared__ __align__(16) float s_g[CH * kBrickVox];
     if (status->overflow) return;
-    const int b = blockIdx.x;
+    const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];      // z-slab of this plan
     const uint32_t kbeg = bin_start[b * kNumClasses], kend = bin_start[(b + 1) * kNumClasses];
     if (kbeg == kend) return;
     const int tid = threadIdx.x;
@@ -228,15 +228,17 @@ template <int CH, bool SINGLE>
 static int launch_bwd_ch(gsvox_plan* p, const float* weight, int C, int c0, const float* grad_out,
                          int astride, cudaStream_t st)
 {
+    const int nblocks = (p->gd.slab1 - p->gd.slab0) * p->gd.nb[0] * p->gd.nb[1];
+    if (nblocks <= 0) return GSVOX_OK;
     LaunchScope ls(p, GSVOX_K_BACKWARD, st);
-    k_backward<CH, SINGLE><<<p->gd.nbricks, kBwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight,
+    k_backward<CH, SINGLE><<<nblocks, kBwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight,
                                                                   C, c0, grad_out, p->acc, astride, p->gd);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }
 
-int launch_backward(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
-                    float* gw, float* gp, float* gs, float* gq, cudaStream_t st)
+int launch_backward_accumulate(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
+                               cudaStream_t st)
 {
     const int astride = acc_stride(channels);
     { LaunchScope ls(p, GSVOX_K_MEMSET, st);
@@ -252,6 +254,13 @@ int launch_backward(gsvox_plan* p, const float* weight, int channels, const floa
             else                { rc = launch_bwd_ch<1, false>(p, weight, channels, c0, grad_out, astride, st); c0 += 1; }
         }
     }
+    return rc;
+}
+
+int launch_backward(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
+                    float* gw, float* gp, float* gs, float* gq, cudaStream_t st)
+{
+    int rc = launch_backward_accumulate(p, weight, channels, grad_out, st);
     if (rc != GSVOX_OK) return rc;
     return launch_epilogue(p, channels, gw, gp, gs, gq, st);
 }

@@ -171,7 +171,7 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
     __shared__ uint32_t s_mask[2][2][kFwdBatch];                    // [buffer][warp][key]
 
     const int tid = threadIdx.x;
-    const int b = blockIdx.x;
+    const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];      // bricks are z-major: a z-slab is a contiguous id range
     const int bx = b % gd.nb[0], by = (b / gd.nb[0]) % gd.nb[1], bz = b / (gd.nb[0] * gd.nb[1]);
     const int b0x = bx * kBrick, b0y = by * kBrick, b0z = bz * kBrick;
     const int ry = tid & 7, rz = tid >> 3;
@@ -240,11 +240,13 @@ static int launch_fwd_ch(gsvox_plan* p, const float* weight, int C, int c0, floa
 {
     LaunchScope ls(p, GSVOX_K_FORWARD, st);
     bool vec = (p->gd.dims[0] % 4 == 0) && (((uintptr_t)out & 15) == 0);
+    const int nblocks = (p->gd.slab1 - p->gd.slab0) * p->gd.nb[0] * p->gd.nb[1];
+    if (nblocks <= 0) return GSVOX_OK;
     if (vec)
-        k_forward<CH, true><<<p->gd.nbricks, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
+        k_forward<CH, true><<<nblocks, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
                                                                    weight, C, c0, out, p->gd);
     else
-        k_forward<CH, false><<<p->gd.nbricks, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
+        k_forward<CH, false><<<nblocks, kFwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
                                                                     weight, C, c0, out, p->gd);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;

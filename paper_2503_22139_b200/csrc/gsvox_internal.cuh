@@ -56,6 +56,7 @@ struct GridDev {
     int dims[3];
     int nb[3];          // bricks per axis
     int nbricks;
+    int slab0, slab1;   // brick layers [slab0, slab1) along z this plan works on (multi-GPU z-slabs; default all)
 };
 
 constexpr int kBrick = GSVOX_BRICK;
@@ -155,6 +156,8 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st);
 int launch_forward(gsvox_plan* p, const float* weight, int channels, float* out, cudaStream_t st);
 int launch_backward(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
                     float* gw, float* gp, float* gs, float* gq, cudaStream_t st);
+int launch_backward_accumulate(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
+                               cudaStream_t st);
 int launch_epilogue(gsvox_plan* p, int channels, float* gw, float* gp, float* gs, float* gq, cudaStream_t st);
 
 }  // namespace gsvox

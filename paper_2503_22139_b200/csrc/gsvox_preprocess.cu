@@ -153,8 +153,9 @@ k_keys(const GsRec* __restrict__ rec, int n, GridDev gd, uint32_t* __restrict__ 
     int loz = (int16_t)(w3.z & 0xffff), hix = (int16_t)(w3.z >> 16);
     int hiy = (int16_t)(w3.w & 0xffff), hiz = (int16_t)(w3.w >> 16);
     if (hix < lox) return;
-    int bx0 = lox >> 3, by0 = loy >> 3, bz0 = loz >> 3;
-    int ex = (hix >> 3) - bx0 + 1, ey = (hiy >> 3) - by0 + 1, ez = (hiz >> 3) - bz0 + 1;
+    int bx0 = lox >> 3, by0 = loy >> 3, bz0 = max(loz >> 3, gd.slab0);          // z-slab of this plan only
+    int ex = (hix >> 3) - bx0 + 1, ey = (hiy >> 3) - by0 + 1, ez = min(hiz >> 3, gd.slab1 - 1) - bz0 + 1;
+    if (ez <= 0) return;
     int total = ex * ey * ez;
     for (int t = sub; t < total; t += 8) {
         int tx = t % ex, r = t / ex, ty = r % ey, tz = r / ey;

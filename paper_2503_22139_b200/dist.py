@@ -1,6 +1,8 @@
-"""Multi-GPU plumbing of bench.py: one process per GPU, "replicas only" (section
-multi-GPU): every rank runs an independent replica of the step on its own GPU, there is no
-data-path collective.  torch.distributed is used for the rendezvous, the barriers around the timed
+"""Multi-GPU plumbing: one process per GPU.  Two modes:
+  replicas  every rank runs an independent replica of the step, no data-path collective (bench.py default);
+  z-slabs   every rank owns a contiguous range of brick layers (slab_bounds), forward is
+            collective-free, backward sums the per-Gaussian accumulators with ONE all-reduce
+            (sharded_backward) between gsvox_backward_accumulate and gsvox_backward_finish.  torch.distributed is used for the rendezvous, the barriers around the timed
 region and the max-over-ranks reduction of the device time.  Backend nccl on GPUs, gloo in the CPU
 tests (tests/test_dist_gloo.py, world_size 2)."""
 import os
@@ -55,3 +57,23 @@ def whole_job_rate(units_per_rank, ranks, ms_total, steps):
     ms_step = ranks.max_over_ranks(ms_total) / steps
     total_units = ranks.sum_over_ranks(units_per_rank)
     return total_units / (ms_step * 1e-3), ms_step
+
+
+def slab_bounds(nbz, rank, world):
+    """Balanced contiguous split of the nbz brick layers (8 voxels each) along z: rank r owns layers
+    [lo, hi).  Covers 0..nbz exactly once; ranks beyond nbz get an empty slab."""
+    if not (0 <= rank < world) or nbz < 0:
+        raise ValueError("slab_bounds(nbz=%r, rank=%r, world=%r)" % (nbz, rank, world))
+    base, extra = divmod(nbz, world)
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)
+
+
+def sharded_backward(plan, weight, grad_out, ranks, grads=None, all_reduce=None):
+    """a4 on this rank's slab -> sum of the [n, 9 + C] accumulators over ranks -> a5.  `all_reduce`
+    defaults to torch.distributed.all_reduce (NCCL over NVLink/NVSwitch: 24 MB at config 4)."""
+    ch = int(weight.shape[1])
+    plan.backward_accumulate(weight, grad_out)
+    if ranks.on:
+        (all_reduce or dist.all_reduce)(plan.accumulators(ch))
+    return plan.backward_finish(ch, grads=grads)

@@ -59,3 +59,64 @@ def test_single_process_needs_no_process_group():
     assert out.returncode == 0, out.stderr[-2000:]
     v, ms = out.stdout.split()
     assert float(ms) == 10.0 and abs(float(v) - 50000.0) < 1e-9
+
+
+# ------------------------------------------------------------------ z-slab sharding
+def test_slab_bounds_partition_every_layer_exactly_once():
+    sys.path.insert(0, ROOT)
+    from paper_2503_22139_b200.dist import slab_bounds
+    for nbz in (0, 1, 3, 8, 16, 32, 33):
+        for world in (1, 2, 3, 4, 8, 16):
+            cover = []
+            sizes = []
+            for r in range(world):
+                lo, hi = slab_bounds(nbz, r, world)
+                assert 0 <= lo <= hi <= nbz
+                cover += list(range(lo, hi)); sizes.append(hi - lo)
+            assert cover == list(range(nbz))                 # contiguous, ordered, no gap, no overlap
+            assert max(sizes) - min(sizes) <= 1              # balanced
+    import pytest
+    with pytest.raises(ValueError):
+        slab_bounds(4, 2, 2)
+
+
+SLAB_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import torch
+from paper_2503_22139_b200.dist import Ranks, slab_bounds, sharded_backward
+
+class FakePlan:                       # host-side stand-in: the accumulate / all-reduce / finish protocol
+    def __init__(self, rank): self.acc = torch.full((6, 12), float(rank + 1)); self.calls = []
+    def backward_accumulate(self, w, g): self.calls.append("acc")
+    def accumulators(self, ch): self.calls.append("view%%d" %% ch); return self.acc.view(-1)
+    def backward_finish(self, ch, grads=None): self.calls.append("fin"); return self.acc.clone()
+
+r = Ranks(backend="gloo")
+lo, hi = slab_bounds(5, r.rank, r.world)
+plan = FakePlan(r.rank)
+out = sharded_backward(plan, torch.zeros(6, 1), None, r)
+r.close()
+print(json.dumps({"rank": r.rank, "slab": [lo, hi], "calls": plan.calls, "sum": float(out[0, 0])}))
+"""
+
+
+def test_two_rank_gloo_sharded_backward_all_reduces_between_the_halves():
+    import json
+    port = free_port()
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", LOCAL_RANK=str(rank),
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, "-c", SLAB_WORKER % ROOT], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = []
+    for p in procs:
+        o, e = p.communicate(timeout=120)
+        assert p.returncode == 0, e[-2000:]
+        outs.append(json.loads(o.strip().splitlines()[-1]))
+    outs.sort(key=lambda o: o["rank"])
+    assert outs[0]["slab"] == [0, 3] and outs[1]["slab"] == [3, 5]
+    for o in outs:
+        assert o["calls"] == ["acc", "view1", "fin"]
+        assert o["sum"] == 3.0                               # 1 + 2: summed over both ranks before a5
