@@ -94,12 +94,18 @@ int gsvox_backward(gsvox_plan* plan, const float* weight, int32_t channels,
  *   keys_needed        number of (brick, Gaussian) keys the input produces
  *   overflow           1 if keys_needed > key_capacity (forward/backward wrote zeros)
  *   skipped_gaussians  degenerate inputs that were skipped
- *   pairs              P_def: (Gaussian, voxel) pairs inside the cutoff = sum of box volumes  */
+ *   pairs              P_def: (Gaussian, voxel) pairs inside the cutoff = sum of box volumes
+ *   culled_keys        (brick, Gaussian) keys of the boxes that were NOT emitted because a conservative
+ *                      lower bound of the exponent over the brick shows every term of the key below
+ *                      w e^-32 (reading A15; thin rotated Gaussians); keys_needed excludes them
+ *   pairs_exec         P_exec: pairs of the emitted keys (what forward/backward evaluate), this slab */
 typedef struct {
     int64_t keys_needed;
     int64_t pairs;
     int32_t skipped_gaussians;
     int32_t overflow;
+    int64_t culled_keys;
+    int64_t pairs_exec;
 } gsvox_status;
 int gsvox_plan_status(gsvox_plan* plan, gsvox_status* status, void* stream);
 

@@ -31,7 +31,8 @@ class GsvoxGrid(C.Structure):
 
 class GsvoxStatus(C.Structure):
     _fields_ = [("keys_needed", C.c_int64), ("pairs", C.c_int64),
-                ("skipped_gaussians", C.c_int32), ("overflow", C.c_int32)]
+                ("skipped_gaussians", C.c_int32), ("overflow", C.c_int32),
+                ("culled_keys", C.c_int64), ("pairs_exec", C.c_int64)]
 
 
 class GsvoxError(RuntimeError):
@@ -305,7 +306,8 @@ class Plan:
         s = GsvoxStatus()
         _check(lib().gsvox_plan_status(self._h, C.byref(s), _stream()))
         return {"keys_needed": int(s.keys_needed), "pairs": int(s.pairs),
-                "skipped_gaussians": int(s.skipped_gaussians), "overflow": bool(s.overflow)}
+                "skipped_gaussians": int(s.skipped_gaussians), "overflow": bool(s.overflow),
+                "culled_keys": int(s.culled_keys), "pairs_exec": int(s.pairs_exec)}
 
     def geometry(self):
         box = torch.empty((self.n, 6), dtype=torch.int32)

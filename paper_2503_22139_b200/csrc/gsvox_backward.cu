@@ -190,7 +190,7 @@ k_backward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start
             kg.cx = (float)(__float_as_int(rb4.x) - b0x) + ra.x;
             kg.cy = (float)(__float_as_int(rb4.y) - b0y) + ra.y;
             kg.cz = (float)(__float_as_int(rb4.z) - b0z) + ra.z;
-            kg.negA = rb4.w; kg.nl01 = rc.x; kg.nl02 = rc.y; kg.l12 = rc.z; kg.nD1 = rc.w; kg.nD2 = rd.x; kg.cc = ra.w;
+            kg.negA = rb4.w; kg.nl01 = rc.x; kg.nl02 = rc.y; kg.l12 = rc.z; kg.nD1 = rc.w; kg.nD2 = rd.x; kg.cc = fabsf(ra.w);
             kg.direct = (-kg.negA > kRecurrenceMaxA);
             kg.y0 = y0; kg.z0 = z0; kg.ny = y1 - y0 + 1; kg.nrows = kg.ny * (z1 - z0 + 1);
             #pragma unroll

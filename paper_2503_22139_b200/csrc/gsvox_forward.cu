@@ -71,7 +71,8 @@ __device__ __forceinline__ void stage_key(float* __restrict__ dst, uint32_t* __r
     float4* o = reinterpret_cast<float4*>(dst);
     o[0] = make_float4((float)(cix - b0x) + a.x, (float)(ciy - b0y) + a.y, (float)(ciz - b0z) + a.z, b.w);
     o[1] = make_float4(c.x, c.y, c.z, c.w);
-    o[2] = make_float4(d.x, 0.f, a.w, a.w);
+    const float cc = fabsf(a.w);                                    // the sign bit is a2's cull flag
+    o[2] = make_float4(d.x, 0.f, cc, cc);
     if (CH == 1) {
         const float w = __ldg(weight + (size_t)gid * wstride + c0);
         o[3] = make_float4((xm & 8u) ? w : 0.f, (xm & 16u) ? w : 0.f, (xm & 4u) ? w : 0.f, (xm & 32u) ? w : 0.f);

@@ -31,6 +31,8 @@ extern "C" int gsvox_plan_status(gsvox_plan* p, gsvox_status* status, void* stre
     status->pairs = (int64_t)h.pairs;
     status->skipped_gaussians = (int32_t)h.skipped;
     status->overflow = (int32_t)h.overflow;
+    status->culled_keys = (int64_t)h.culled;
+    status->pairs_exec = (int64_t)h.pairs_exec;
     return GSVOX_OK;
 }
 

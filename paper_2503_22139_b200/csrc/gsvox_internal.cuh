@@ -16,7 +16,8 @@ namespace gsvox {
 //              E = -( A u0^2 + D1 u1^2 + D2 u2^2 ),  u2 = dz, u1 = dy + l12 dz,
 //              u0 = dx + l01 dy + l02 dz,  A = kappa2*M00, kappa2 = log2(e)/2
 //            a sum of squares: no cancellation for needle-like Gaussians (kernels)
-//   cexp     = 2^(-2A), rounded from fp64: ratio of successive ratios along an x-row
+//   cexp     = 2^(-2A), rounded from fp64: ratio of successive ratios along an x-row; its SIGN BIT is
+//              a2's cull flag (thin rotated Gaussian: run the per-brick negligibility test); use fabsf
 //   box      = inclusive voxel box (reading A5), int16; empty <=> hi[0] < lo[0]
 // ------------------------------------------------------------------------------------------
 struct __align__(16) GsRec {
@@ -47,7 +48,8 @@ struct DevStatus {
     unsigned long long pairs;
     unsigned int skipped;
     unsigned int overflow;
-    unsigned int pad[2];
+    unsigned long long culled;        // keys dropped by the conservative q_min > 64 test (reading A15)
+    unsigned long long pairs_exec;    // P_exec: pairs of the kept keys
 };
 
 struct GridDev {

@@ -11,6 +11,9 @@
 
 namespace gsvox {
 
+constexpr float kCullQ = 64.0f;
+constexpr double kCullBoxRatio = 8.0;     // config 4's 6:1 Gaussians stay below 7.6: the test costs them nothing
+
 __device__ __forceinline__ bool finite_d(double v) { return isfinite(v); }
 
 __global__ void __launch_bounds__(256)
@@ -64,12 +67,14 @@ k_preprocess(const float* __restrict__ pos, const float* __restrict__ scale,
             // steps 4-5: r_k = 3 sqrt(Sigma_kk), integer box clipped to the grid
             double s0 = MUL(s[0], s[0]), s1 = MUL(s[1], s[1]), s2 = MUL(s[2], s[2]);
             bool empty = false; int lo[3], hi[3];
+            double rprod = 1.0;
             #pragma unroll
             for (int k = 0; k < 3; ++k) {
                 double Skk = ADD(ADD(MUL(MUL(R[3 * k], R[3 * k]), s0),
                                      MUL(MUL(R[3 * k + 1], R[3 * k + 1]), s1)),
                                  MUL(MUL(R[3 * k + 2], R[3 * k + 2]), s2));
                 double rk = MUL(GSVOX_SIGMA_CUTOFF, __dsqrt_rn(Skk));
+                rprod *= rk;
                 double l = ceil(__ddiv_rn(SUB(SUB(p[k], rk), gd.origin[k]), gd.spacing[k]));
                 double h = floor(__ddiv_rn(SUB(ADD(p[k], rk), gd.origin[k]), gd.spacing[k]));
                 double top = (double)(gd.dims[k] - 1);
@@ -104,6 +109,10 @@ k_preprocess(const float* __restrict__ pos, const float* __restrict__ scale,
                 r.negA = (float)(-k2 * D0); r.nl01 = (float)(-l01); r.nl02 = (float)(-l02);
                 r.l12 = (float)l12; r.nD1 = (float)(-k2 * D1); r.nD2 = (float)(-k2 * D2);
                 r.cexp = (float)exp2(-2.0 * k2 * D0);
+                // a2 cull flag in the sign bit of cexp (readers take fabsf): the box holds > 8x the volume of
+                // the box of the unrotated 3-sigma ellipsoid, i.e. it is mostly empty space (thin and rotated)
+                const double kap3 = GSVOX_SIGMA_CUTOFF * GSVOX_SIGMA_CUTOFF * GSVOX_SIGMA_CUTOFF;
+                if (rprod > kCullBoxRatio * kap3 * s[0] * s[1] * s[2]) r.cexp = -r.cexp;
                 for (int k = 0; k < 3; ++k) {
                     double c = (p[k] - gd.origin[k]) / gd.spacing[k];
                     double ci = rint(c);
@@ -136,35 +145,108 @@ k_preprocess(const float* __restrict__ pos, const float* __restrict__ scale,
 // ------------------------------------------------------------------------------------------
 // a2: keys.  Eight lanes cooperate on one Gaussian and stride over the bricks of its box.
 // MODE 0: count keys per brick.  MODE 1: claim a slot per key and write the Gaussian id.
+//
+// Negligible keys are dropped (reading A15; SURVEY.md section 7 hard part 7): the axis-aligned box
+// of a thin rotated Gaussian is mostly empty space (config 5's needles: 91 % of all pairs, 0.8 % of
+// them with q < 9).  For a brick, in the Gaussian's principal frame t = S^-1 R^T (x - p), each t_k is
+// linear in x, so over the brick it spans centre_k +- half_k with half_k = sum_j |R_jk| h_j 3.5 / s_k,
+// and q = |t|^2 >= sum_k max(|centre_k| - half_k, 0)^2.  A key is kept unless that lower bound
+// exceeds kCullQ = 64: every dropped term is below w e^-32 = 1.3e-14 w, far inside the forward
+// tolerance even with 1e5 keys per brick.  Both passes take the decision with the same code on the
+// same data.  Dropped keys and the pairs of kept keys (P_exec) are counted in DevStatus.  Only Gaussians
+// flagged by a1 (box volume > 8x the unrotated ellipsoid box: thin AND rotated) run the test, the rest
+// pay nothing (unflagged: 0.23 ms of binning at config 4; testing every key cost 0.31 ms).
 // ------------------------------------------------------------------------------------------
+
+// The brick test of one flagged Gaussian (everything recomputed per brick: only needles get here).
+__device__ __forceinline__ bool key_negligible(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int g,
+                                            float h0, float h1, float h2, int bx, int by, int bz)
+{
+    const int4* rp = reinterpret_cast<const int4*>(rec + g);
+    const int4 w0 = __ldg(rp), w1 = __ldg(rp + 1);                        // cf, cexp | ci, negA
+    const float4 qa = __ldg(reinterpret_cast<const float4*>(aux + g));
+    const float4 sa = __ldg(reinterpret_cast<const float4*>(aux + g) + 1);
+    const float qn = rsqrtf(qa.x * qa.x + qa.y * qa.y + qa.z * qa.z + qa.w * qa.w);
+    const float r = qa.x * qn, x = qa.y * qn, y = qa.z * qn, z = qa.w * qn;
+    // rows of R scaled by the spacing: t_k = (1/s_k) sum_j R_jk h_j (x_j - c_j) in index units
+    const float Rm[9] = { (1.f - 2.f * (y * y + z * z)) * h0, 2.f * (x * y - r * z) * h0, 2.f * (x * z + r * y) * h0,
+                          2.f * (x * y + r * z) * h1, (1.f - 2.f * (x * x + z * z)) * h1, 2.f * (y * z - r * x) * h1,
+                          2.f * (x * z - r * y) * h2, 2.f * (y * z + r * x) * h2, (1.f - 2.f * (x * x + y * y)) * h2 };
+    const float is[3] = { 1.f / sa.x, 1.f / sa.y, 1.f / sa.z };
+    const float d0 = (float)(8 * bx - w1.x) + (3.5f - __int_as_float(w0.x));
+    const float d1 = (float)(8 * by - w1.y) + (3.5f - __int_as_float(w0.y));
+    const float d2 = (float)(8 * bz - w1.z) + (3.5f - __int_as_float(w0.z));
+    float qmin = 0.f;
+    #pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const float c = (Rm[k] * d0 + Rm[3 + k] * d1 + Rm[6 + k] * d2) * is[k];
+        const float half = 3.5f * (fabsf(Rm[k]) + fabsf(Rm[3 + k]) + fabsf(Rm[6 + k])) * is[k];
+        const float dist = fmaxf(fabsf(c) - half, 0.f);
+        qmin = fmaf(dist, dist, qmin);
+    }
+    return qmin > kCullQ;
+}
+
 template <int MODE>
-__global__ void __launch_bounds__(256)
-k_keys(const GsRec* __restrict__ rec, int n, GridDev gd, uint32_t* __restrict__ bin_count,
-       uint32_t* __restrict__ keys, const DevStatus* __restrict__ status)
+__global__ void __launch_bounds__(256, 6)       // <= 40 registers: the kernel lives on atomics in flight, i.e. on resident warps
+k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, GridDev gd,
+       uint32_t* __restrict__ bin_count, uint32_t* __restrict__ keys, DevStatus* __restrict__ status)
 {
     if (MODE == 1 && status->overflow) return;
-    int g = (blockIdx.x * blockDim.x + threadIdx.x) >> 3;
-    int sub = threadIdx.x & 7;
-    if (g >= n) return;
-    const int4* rp = reinterpret_cast<const int4*>(rec + g);
-    int4 w3 = __ldg(rp + 3);                      // bytes 48..63: nD2, lo[3], hi[3]
-    const bool direct = -__int_as_float(__ldg(rp + 1).w) > kRecurrenceMaxA;      // negA at byte 28
-    int lox = (int16_t)(w3.y & 0xffff), loy = (int16_t)(w3.y >> 16);
-    int loz = (int16_t)(w3.z & 0xffff), hix = (int16_t)(w3.z >> 16);
-    int hiy = (int16_t)(w3.w & 0xffff), hiz = (int16_t)(w3.w >> 16);
-    if (hix < lox) return;
-    int bx0 = lox >> 3, by0 = loy >> 3, bz0 = max(loz >> 3, gd.slab0);          // z-slab of this plan only
-    int ex = (hix >> 3) - bx0 + 1, ey = (hiy >> 3) - by0 + 1, ez = min(hiz >> 3, gd.slab1 - 1) - bz0 + 1;
-    if (ez <= 0) return;
-    int total = ex * ey * ez;
+    __shared__ unsigned long long s_pairs;
+    __shared__ unsigned int s_culled;
+    if (MODE == 0) {
+        if (threadIdx.x == 0) { s_pairs = 0ull; s_culled = 0u; }
+        __syncthreads();
+    }
+    const int g = (blockIdx.x * blockDim.x + threadIdx.x) >> 3;
+    const int sub = threadIdx.x & 7;
+    unsigned int my_pairs = 0u, my_culled = 0u;                // per thread: < 2^32 (<= 4096^3/8 bricks x 512)
+    int total = 0, lox = 0, loy = 0, loz = 0, hix = -1, hiy = -1, hiz = -1, bx0 = 0, by0 = 0, bz0 = 0, ex = 1, ey = 1;
+    bool direct = false, cullable = false;
+    if (g < n) {
+        const int4* rp = reinterpret_cast<const int4*>(rec + g);
+        const int4 w3 = __ldg(rp + 3);                      // bytes 48..63: nD2, lo[3], hi[3]
+        direct = -__int_as_float(__ldg(rp + 1).w) > kRecurrenceMaxA;      // negA at byte 28
+        lox = (int16_t)(w3.y & 0xffff); loy = (int16_t)(w3.y >> 16);
+        loz = (int16_t)(w3.z & 0xffff); hix = (int16_t)(w3.z >> 16);
+        hiy = (int16_t)(w3.w & 0xffff); hiz = (int16_t)(w3.w >> 16);
+        if (hix >= lox) {
+            bx0 = lox >> 3; by0 = loy >> 3; bz0 = max(loz >> 3, gd.slab0);          // z-slab of this plan only
+            ex = (hix >> 3) - bx0 + 1; ey = (hiy >> 3) - by0 + 1;
+            const int ez = min(hiz >> 3, gd.slab1 - 1) - bz0 + 1;
+            total = (ez > 0) ? ex * ey * ez : 0;
+        }
+        cullable = (total > 1) && (__ldg(reinterpret_cast<const int*>(rec + g) + 3) < 0);   // sign bit of cexp
+    }
     for (int t = sub; t < total; t += 8) {
         int tx = t % ex, r = t / ex, ty = r % ey, tz = r / ey;
         const int bx = bx0 + tx, by = by0 + ty, bz = bz0 + tz;
-        const int cls = key_class(direct, max(lox - 8 * bx, 0), min(hix - 8 * bx, 7), max(loy - 8 * by, 0),
-                                  min(hiy - 8 * by, 7), max(loz - 8 * bz, 0), min(hiz - 8 * bz, 7));
+        if (cullable && key_negligible(rec, aux, g, (float)gd.spacing[0], (float)gd.spacing[1], (float)gd.spacing[2],
+                                       bx, by, bz)) { my_culled += 1u; continue; }
+        const int x0 = max(lox - 8 * bx, 0), x1 = min(hix - 8 * bx, 7), y0 = max(loy - 8 * by, 0), y1 = min(hiy - 8 * by, 7);
+        const int z0 = max(loz - 8 * bz, 0), z1 = min(hiz - 8 * bz, 7);
+        const int cls = key_class(direct, x0, x1, y0, y1, z0, z1);
         int b = ((bz * gd.nb[1] + by) * gd.nb[0] + bx) * kNumClasses + cls;
-        if (MODE == 0) atomicAdd(&bin_count[b], 1u);
+        if (MODE == 0) { atomicAdd(&bin_count[b], 1u); my_pairs += (unsigned)((x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1)); }
         else { uint32_t slot = atomicAdd(&bin_count[b], 1u); keys[slot] = (uint32_t)g; }
+    }
+    if (MODE == 0) {
+        // P_exec and the culled count: warp -> CTA (shared) -> ONE global atomic pair per CTA
+        unsigned long long wp = my_pairs;
+        for (int o = 16; o > 0; o >>= 1) {
+            wp += __shfl_xor_sync(0xffffffffu, wp, o);
+            my_culled += __shfl_xor_sync(0xffffffffu, my_culled, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            if (wp) atomicAdd(&s_pairs, wp);
+            if (my_culled) atomicAdd(&s_culled, my_culled);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            if (s_pairs) atomicAdd(&status->pairs_exec, s_pairs);
+            if (s_culled) atomicAdd(&status->culled, (unsigned long long)s_culled);
+        }
     }
 }
 
@@ -262,7 +344,7 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
     int kblocks = (int)((n * 8 + 255) / 256);
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_COUNT, st);
-        k_keys<0><<<kblocks, 256, 0, st>>>(p->rec, (int)n, p->gd, p->bin_count, p->keys, p->status);
+        k_keys<0><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status);
         GSVOX_CUDA(cudaGetLastError());
     }
     int sblocks = (p->nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock;
@@ -278,7 +360,7 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
       GSVOX_CUDA(cudaGetLastError()); }
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_SCATTER, st);
-        k_keys<1><<<kblocks, 256, 0, st>>>(p->rec, (int)n, p->gd, p->bin_count, p->keys, p->status);
+        k_keys<1><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status);
         GSVOX_CUDA(cudaGetLastError());
     }
     return GSVOX_OK;
