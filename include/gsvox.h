@@ -144,7 +144,9 @@ int gsvox_plan_timings(gsvox_plan* plan, double* ms /*[GSVOX_K_COUNT_KINDS]*/,
  * host->device, runs preprocess + forward + backward, copies out and the four gradients
  * device->host, all on `stream`, then SYNCHRONISES.  `staging` is caller-owned device memory of
  * at least gsvox_host_staging_bytes(); host buffers should be pinned.  out_host may be NULL
- * (skip the volume read-back) and grad_out_host may be NULL (forward only).                   */
+ * (skip the volume read-back) and grad_out_host may be NULL (forward only).  The upstream gradient
+ * is uploaded and the volume downloaded on two copy streams owned by the plan, overlapped with the
+ * kernels (both ordered after work already enqueued on `stream`).                              */
 int gsvox_host_staging_bytes(int64_t n_max, int32_t max_channels, const gsvox_grid* grid, size_t* bytes);
 int gsvox_step_host(gsvox_plan* plan, void* staging, size_t staging_bytes,
                     const float* pos_host, const float* scale_host, const float* quat_host,

@@ -134,6 +134,10 @@ extern "C" void gsvox_plan_destroy(gsvox_plan* p)
     if (!p) return;
     for (int i = 0; i < p->n_pending; ++i) { cudaEventDestroy(p->pending[i].a); cudaEventDestroy(p->pending[i].b); }
     free(p->pending);
+    if (p->side_ready) {
+        for (int i = 0; i < 2; ++i) cudaStreamDestroy(p->side[i]);
+        for (int i = 0; i < 4; ++i) cudaEventDestroy(p->side_ev[i]);
+    }
     delete p;
 }
 

@@ -162,18 +162,38 @@ extern "C" int gsvox_step_host(gsvox_plan* p, void* staging, size_t staging_byte
     size_t V = (size_t)p->grid.dims[0] * p->grid.dims[1] * p->grid.dims[2];
     size_t nn = (size_t)n;
     const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
+    // Two copy streams keep both DMA engines busy beside the kernels: the upstream gradient (the
+    // large H2D) travels while a1-a3 run, the volume (the large D2H) while a4-a5 run.
+    if (!p->side_ready) {
+        for (int i = 0; i < 2; ++i) GSVOX_CUDA(cudaStreamCreateWithFlags(&p->side[i], cudaStreamNonBlocking));
+        for (int i = 0; i < 4; ++i) GSVOX_CUDA(cudaEventCreateWithFlags(&p->side_ev[i], cudaEventDisableTiming));
+        p->side_ready = 1;
+    }
+    cudaStream_t up = p->side[0], down = p->side[1];
+    cudaEvent_t ev_begin = p->side_ev[0], ev_grad = p->side_ev[1], ev_fwd = p->side_ev[2], ev_out = p->side_ev[3];
+    GSVOX_CUDA(cudaEventRecord(ev_begin, st));                 // the copy streams start after the caller's earlier work
     if (nn) {
         GSVOX_CUDA(cudaMemcpyAsync(d + S.pos, pos_h, nn * 12, H2D, st));
         GSVOX_CUDA(cudaMemcpyAsync(d + S.scale, scale_h, nn * 12, H2D, st));
         GSVOX_CUDA(cudaMemcpyAsync(d + S.quat, quat_h, nn * 16, H2D, st));
         GSVOX_CUDA(cudaMemcpyAsync(d + S.weight, weight_h, nn * C * 4, H2D, st));
     }
-    if (grad_out_h) GSVOX_CUDA(cudaMemcpyAsync(d + S.vol_grad, grad_out_h, V * C * 4, H2D, st));
+    if (grad_out_h) {
+        GSVOX_CUDA(cudaStreamWaitEvent(up, ev_begin, 0));
+        GSVOX_CUDA(cudaMemcpyAsync(d + S.vol_grad, grad_out_h, V * C * 4, H2D, up));
+        GSVOX_CUDA(cudaEventRecord(ev_grad, up));
+    }
     rc = gsvox_preprocess(p, (float*)(d + S.pos), (float*)(d + S.scale), (float*)(d + S.quat), n, stream);
     if (rc != GSVOX_OK) return rc;
     rc = gsvox_forward(p, (float*)(d + S.weight), C, (float*)(d + S.vol_out), stream);
     if (rc != GSVOX_OK) return rc;
-    if (out_h) GSVOX_CUDA(cudaMemcpyAsync(out_h, d + S.vol_out, V * C * 4, D2H, st));
+    if (out_h) {
+        GSVOX_CUDA(cudaEventRecord(ev_fwd, st));
+        GSVOX_CUDA(cudaStreamWaitEvent(down, ev_fwd, 0));
+        GSVOX_CUDA(cudaMemcpyAsync(out_h, d + S.vol_out, V * C * 4, D2H, down));
+        GSVOX_CUDA(cudaEventRecord(ev_out, down));
+    }
+    if (grad_out_h) GSVOX_CUDA(cudaStreamWaitEvent(st, ev_grad, 0));
     if (grad_out_h && nn) {
         rc = gsvox_backward(p, (float*)(d + S.weight), C, (float*)(d + S.vol_grad), (float*)(d + S.gw),
                             (float*)(d + S.gp), (float*)(d + S.gs), (float*)(d + S.gq), stream);
@@ -183,6 +203,7 @@ extern "C" int gsvox_step_host(gsvox_plan* p, void* staging, size_t staging_byte
         GSVOX_CUDA(cudaMemcpyAsync(gs_h, d + S.gs, nn * 12, D2H, st));
         GSVOX_CUDA(cudaMemcpyAsync(gq_h, d + S.gq, nn * 16, D2H, st));
     }
+    if (out_h) GSVOX_CUDA(cudaStreamWaitEvent(st, ev_out, 0));
     GSVOX_CUDA(cudaStreamSynchronize(st));
     return GSVOX_OK;
 }

@@ -136,6 +136,10 @@ struct gsvox_plan {
     struct Pending { cudaEvent_t a, b; int kind; };
     Pending* pending;
     int n_pending, cap_pending;
+    // gsvox_step_host: copy streams (H2D of the upstream gradient, D2H of the volume) and their events, created lazily
+    cudaStream_t side[2];
+    cudaEvent_t side_ev[4];
+    int side_ready;
 };
 
 namespace gsvox {
