@@ -35,10 +35,23 @@ __device__ __forceinline__ bool warp_cell(float dx, float dy, float dz, const Wa
     return ok;
 }
 
-// Eight-corner gather of one sample; corners outside the grid read 0.
+// Eight-corner gather of one sample; corners outside the grid read 0.  Cells wholly inside the grid
+// (all but a boundary shell) take the path without bounds tests.
 __device__ __forceinline__ float warp_sample(const float* __restrict__ iref, const WarpGrid& wg,
                                              int cx, int cy, int cz, float fx, float fy, float fz)
 {
+    if ((unsigned)cx < (unsigned)(wg.nx - 1) && (unsigned)cy < (unsigned)(wg.ny - 1) && (unsigned)cz < (unsigned)(wg.nz - 1)) {
+        const float* p00 = iref + ((size_t)cz * wg.ny + cy) * wg.nx + cx;
+        const float* p10 = p00 + wg.nx;
+        const float* p01 = p00 + (size_t)wg.nx * wg.ny;
+        const float* p11 = p01 + wg.nx;
+        const float a0 = __ldg(p00), a1 = __ldg(p00 + 1), b0 = __ldg(p10), b1 = __ldg(p10 + 1);
+        const float c0 = __ldg(p01), c1 = __ldg(p01 + 1), e0 = __ldg(p11), e1 = __ldg(p11 + 1);
+        const float la = fmaf(fx, a1 - a0, a0), lb = fmaf(fx, b1 - b0, b0);
+        const float lc = fmaf(fx, c1 - c0, c0), le = fmaf(fx, e1 - e0, e0);
+        const float lo = fmaf(fy, lb - la, la), hi = fmaf(fy, le - lc, lc);
+        return fmaf(fz, hi - lo, lo);
+    }
     float acc = 0.f;
     #pragma unroll
     for (int az = 0; az < 2; ++az) {
