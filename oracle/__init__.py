@@ -240,9 +240,10 @@ def dvf_backward(levels, coef, grid, grad_dvf, kappa=KAPPA):
 # Readings (W1-W4): trilinear interpolation of the voxel-centre samples; a corner
 # outside the grid contributes 0 (zero padding, corner by corner); d is in world units like
 # origin/spacing, so the sample position in index units is u_k = i_k + d_k / h_k; the cell index
-# floor(u_k) is decided on t_k = fp32(d_k) / fp32(h_k) ROUNDED TO fp32 (the kernel's precision:
-# both sides take the integer decision in the same precision), everything after that is fp64;
-# a non-finite displacement yields 0 and zero gradients.  Backward is the exact derivative of the
+# floor(u_k) is decided on t_k = fp32(fp32(d_k) * fp32(1 / h_k)) — one fp32 reciprocal of the spacing, one
+# fp32 multiply (the kernel's precision and operation order: both sides take the integer decision in
+# the same precision), everything after that is fp64; a non-finite displacement, or one of 2^22 voxels
+# or more, yields 0 and zero gradients.  Backward is the exact derivative of the
 # piecewise-trilinear interpolant (kinks at integer u have measure zero).
 # --------------------------------------------------------------------------------------------
 def _warp_cells(dvf, spacing, dims):
@@ -250,9 +251,10 @@ def _warp_cells(dvf, spacing, dims):
     nx, ny, nz = (int(v) for v in dims)
     d32 = _f32(dvf).reshape(-1, 3, nz, ny, nx)
     h32 = _f32(spacing).reshape(3)
+    inv_h32 = (np.float32(1.0) / h32).astype(np.float32)      # 1/h rounded once to fp32 ...
     with np.errstate(invalid="ignore", over="ignore"):
-        t = d32 / h32[None, :, None, None, None]              # fp32 IEEE division, as on the device
-    finite = np.all(np.isfinite(t), axis=1) & np.all(np.abs(t) < 1.0e9, axis=1)
+        t = (d32 * inv_h32[None, :, None, None, None]).astype(np.float32)   # ... then ONE fp32 multiply, as on the device
+    finite = np.all(np.isfinite(t), axis=1) & np.all(np.abs(t) < 4194304.0, axis=1)   # |t| < 2^22 voxels
     t = np.where(finite[:, None], t, np.float32(0))
     tf = np.floor(t)
     frac = (t - tf).astype(np.float64)                         # exact in fp32

@@ -4,8 +4,8 @@
 //
 // Readings W1-W4: trilinear interpolation of the voxel-centre samples; a corner outside
 // the grid contributes 0; d is in world units, the sample sits at index u_k = i_k + d_k / h_k; the
-// cell index is decided on t_k = d_k / h_k in fp32 (IEEE division, floor; the fraction t - floor t
-// is exact), so positions far from the origin lose nothing to the magnitude of i_k; a non-finite
+// cell index is decided on t_k = d_k * (1 / h_k) in fp32 (reciprocal rounded once, one multiply, floor;
+// the fraction t - floor t is exact), so positions far from the origin lose nothing to the magnitude of i_k; a non-finite
 // displacement yields 0 and zero gradients.
 //
 // HBM/L2-bound gather.  One thread per output voxel, x fastest: the three d loads, the g load and
@@ -22,16 +22,21 @@ constexpr int kWarpThreads = 256;
 
 struct WarpGrid { int nx, ny, nz; float inv_hx, inv_hy, inv_hz; float hx, hy, hz; };
 
-// Cell of one sample: base corner (may be outside the grid) and fractions; false if non-finite.
+// Cell of one sample: base corner (may be outside the grid) and fractions; false if non-finite or
+// |t| >= 2^22 voxels.  t = d * (1/h): one fp32 multiply by the reciprocal the host rounded once (reading
+// W3; the oracle does the same two roundings).  floor -> int without a second conversion instruction:
+// for |fl| < 2^22, fl + 1.5 * 2^23 holds the integer in its low mantissa bits.
 __device__ __forceinline__ bool warp_cell(float dx, float dy, float dz, const WarpGrid& wg, int x, int y, int z,
                                           int& cx, int& cy, int& cz, float& fx, float& fy, float& fz)
 {
-    const float tx = __fdiv_rn(dx, wg.hx), ty = __fdiv_rn(dy, wg.hy), tz = __fdiv_rn(dz, wg.hz);
-    // |t| < 1e9 also rejects NaN (comparison false) and inf
-    const bool ok = (fabsf(tx) < 1.0e9f) && (fabsf(ty) < 1.0e9f) && (fabsf(tz) < 1.0e9f);
+    const float tx = __fmul_rn(dx, wg.inv_hx), ty = __fmul_rn(dy, wg.inv_hy), tz = __fmul_rn(dz, wg.inv_hz);
+    // the comparison is false for NaN, so it rejects NaN and inf as well
+    const bool ok = (fabsf(tx) < 4194304.f) && (fabsf(ty) < 4194304.f) && (fabsf(tz) < 4194304.f);
     const float flx = floorf(tx), fly = floorf(ty), flz = floorf(tz);
     fx = ok ? tx - flx : 0.f; fy = ok ? ty - fly : 0.f; fz = ok ? tz - flz : 0.f;
-    cx = ok ? x + (int)flx : x; cy = ok ? y + (int)fly : y; cz = ok ? z + (int)flz : z;
+    const int ix = __float_as_int(flx + 12582912.f) - 0x4B400000, iy = __float_as_int(fly + 12582912.f) - 0x4B400000;
+    const int iz = __float_as_int(flz + 12582912.f) - 0x4B400000;
+    cx = ok ? x + ix : x; cy = ok ? y + iy : y; cz = ok ? z + iz : z;
     return ok;
 }
 
