@@ -315,6 +315,60 @@ def warp_case(batch=8, dims=(256, 256, 128), spacing=(2.0, 2.0, 2.0), amp_vox=4.
     return WarpCase("warp_b%d" % batch, tuple(dims), _f32(iref), dvf, spacing=tuple(spacing), seed=seed)
 
 
+@dataclass
+class ProjectCase:
+    """Inputs of the batched cone-beam projector (Table I)."""
+    name: str
+    dims: tuple
+    vol: np.ndarray             # [B,nz,ny,nx] fp32: one dynamic CBCT per gantry angle
+    angles: np.ndarray          # [B] fp32 radians
+    geom: dict                  # sad, sdd, nu, nv, du, dv, off_u, off_v, iso[3]
+    origin: tuple = (0.0, 0.0, 0.0)
+    spacing: tuple = (2.0, 2.0, 2.0)
+    seed: object = 0
+
+    @property
+    def batch(self):
+        return int(self.vol.shape[0])
+
+    @property
+    def grid(self):
+        return (np.asarray(self.origin, np.float32), np.asarray(self.spacing, np.float32),
+                np.asarray(self.dims, np.int32))
+
+    def grad_drr(self):
+        rng = np.random.default_rng([79, self.batch] + list(np.atleast_1d(self.seed)))
+        return rng.standard_normal((self.batch, self.geom["nv"], self.geom["nu"]), dtype=np.float32)
+
+
+def project_case(batch=8, dims=(200, 200, 100), spacing=(2.0, 2.0, 2.0), nu=512, nv=384, du=0.776, dv=0.776,
+                 sad=1000.0, sdd=1500.0, off_u=0.0, off_v=0.0, seed=7, angles=None):
+    """The paper's acquisition geometry (Table I: 512x384 pixels of 0.776 mm, SAD 1000 / SDD 1500 mm;
+    200x200x100 voxels of 2 mm) with the isocentre at the grid centre.  Volumes: the
+    ellipsoidal body of warp_case with a different low-frequency modulation per projection (stand-ins
+    for the dynamic CBCTs); gantry angles uniform over a full turn unless given."""
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = dims
+    origin = tuple(-(n - 1) / 2.0 * h for n, h in zip(dims, spacing))
+    z, y, x = np.meshgrid(np.arange(nz, dtype=np.float32), np.arange(ny, dtype=np.float32),
+                          np.arange(nx, dtype=np.float32), indexing="ij")
+    c = (np.array([nx, ny, nz], np.float32) - 1) / 2
+    semi = np.array([0.45 * nx, 0.35 * ny, 0.48 * nz], np.float32)
+    body = ((((x - c[0]) / semi[0]) ** 2 + ((y - c[1]) / semi[1]) ** 2 + ((z - c[2]) / semi[2]) ** 2) <= 1.0)
+    body = body.astype(np.float32)
+    vol = np.empty((batch, nz, ny, nx), np.float32)
+    for b in range(batch):
+        k = rng.uniform(0.5, 4.0, size=3) * 2 * np.pi / np.array([nx, ny, nz])
+        tex = np.cos(k[0] * x + k[1] * y + k[2] * z + rng.uniform(0, 2 * np.pi)).astype(np.float32)
+        vol[b] = body * (0.02 + 0.005 * tex) + body * rng.normal(0.0, 0.001, size=body.shape).astype(np.float32)
+    if angles is None:
+        angles = rng.uniform(0.0, 2 * np.pi, size=batch)
+    geom = dict(sad=float(sad), sdd=float(sdd), nu=int(nu), nv=int(nv), du=float(du), dv=float(dv),
+                off_u=float(off_u), off_v=float(off_v), iso=[0.0, 0.0, 0.0])
+    return ProjectCase("project_b%d" % batch, tuple(dims), vol, np.asarray(angles, np.float32), geom,
+                       origin=origin, spacing=tuple(spacing), seed=seed)
+
+
 FULL = {
     "config1": lambda: [config1()],
     "config2": lambda: [config2()],

@@ -227,6 +227,35 @@ int gsvox_warp_forward(const float* iref, const float* dvf, const gsvox_grid* gr
 int gsvox_warp_backward(const float* iref, const float* dvf, const gsvox_grid* grid, int32_t B,
                         const float* grad_out, float* grad_iref, float* grad_dvf, void* stream);
 
+/* ---- batched cone-beam projector, one distinct volume per gantry angle ----
+ * PAPER.md:141 (Eq. 12) P[I(x,p)]; "PMF-STGR requires a distinct DRR for each dynamic
+ * CBCT at each gantry angle ... future work could implement GPU-based parallelization to compute DRRs
+ * from multiple dynamic CBCTs simultaneously"; Eq. 6: I(r) = int sigma(r(t)) dt; Table I: SAD, SDD,
+ * detector size and pixel pitch.  Geometry (reading P1): circular orbit about the axis through `iso`
+ * parallel to z; at gantry angle a the source sits at iso + sad (cos a, sin a, 0); flat detector
+ * perpendicular to the central ray at distance sdd from the source; u = (-sin a, cos a, 0),
+ * v = (0, 0, 1); pixel (iu, iv) centre at det_centre + ((iu - (nu-1)/2) du + off_u) u
+ * + ((iv - (nv-1)/2) dv + off_v) v.  Line integral by Joseph's method (reading P2).              */
+typedef struct {
+    float   sad, sdd;        /* source-to-axis and source-to-detector distance, world units          */
+    int32_t nu, nv;          /* detector pixels along u (in the orbit plane) and v (along the axis)   */
+    float   du, dv;          /* pixel pitch                                                            */
+    float   off_u, off_v;    /* detector offset (half-fan acquisitions)                                */
+    float   iso[3];          /* a point of the rotation axis, world units                              */
+} gsvox_cone_geometry;
+/* scratch: caller-owned DEVICE memory of gsvox_project_scratch_bytes() (a y-fastest copy of the B
+ * volumes, so that rays running mostly along x read contiguously).  1 <= B <= 64 per call.          */
+int gsvox_project_scratch_bytes(const gsvox_grid* grid, int32_t B, size_t* bytes);
+/* drr[b, iv, iu] = line integral of volume b along the ray source(angles_host[b]) -> pixel (iu, iv).
+ * vol [B,nz,ny,nx] with vol_stride = nx*ny*nz, or ONE volume shared by all angles with vol_stride =
+ * 0 (the conventional case); angles_host [B] radians, a HOST pointer; drr [B,nv,nu] OVERWRITTEN.    */
+int gsvox_project_forward(const float* vol, int64_t vol_stride, const gsvox_grid* grid,
+                          const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                          void* scratch, float* drr, void* stream);
+/* Exact transpose: grad_vol[b] = P_b^T grad_drr[b], grad_vol [B,nz,ny,nx] OVERWRITTEN (fp32 atomics). */
+int gsvox_project_backward(const float* grad_drr, const gsvox_grid* grid, const gsvox_cone_geometry* geom,
+                           const float* angles_host, int32_t B, void* scratch, float* grad_vol, void* stream);
+
 /* Live ALU rooflines of the device the calling thread has current (the hot path is
  * FP32-issue / MUFU bound, and MEASURED_PEAKS.json holds no FP32 figure).  Runs three register-only
  * microbenchmarks on `stream` and SYNCHRONISES: scalar FFMA chains (fp32_tflops, 2 flops per lane

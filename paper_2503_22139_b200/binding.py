@@ -22,6 +22,7 @@ EXPORTS = [
     "gsvox_last_cuda_error", "gsvox_version", "gsvox_probe_peaks", "gsvox_dvf_forward", "gsvox_dvf_backward",
     "gsvox_mbc_combine_forward", "gsvox_mbc_combine_backward", "gsvox_warp_forward", "gsvox_warp_backward",
     "gsvox_plan_set_slab", "gsvox_backward_accumulate", "gsvox_backward_finish", "gsvox_plan_accumulators",
+    "gsvox_project_scratch_bytes", "gsvox_project_forward", "gsvox_project_backward",
 ]
 
 
@@ -33,6 +34,12 @@ class GsvoxStatus(C.Structure):
     _fields_ = [("keys_needed", C.c_int64), ("pairs", C.c_int64),
                 ("skipped_gaussians", C.c_int32), ("overflow", C.c_int32),
                 ("culled_keys", C.c_int64), ("pairs_exec", C.c_int64)]
+
+
+class GsvoxConeGeometry(C.Structure):
+    _fields_ = [("sad", C.c_float), ("sdd", C.c_float), ("nu", C.c_int32), ("nv", C.c_int32),
+                ("du", C.c_float), ("dv", C.c_float), ("off_u", C.c_float), ("off_v", C.c_float),
+                ("iso", C.c_float * 3)]
 
 
 class GsvoxError(RuntimeError):
@@ -77,6 +84,10 @@ def lib():
     L.gsvox_backward_accumulate.argtypes = [vp, vp, i32, vp, vp]
     L.gsvox_backward_finish.argtypes = [vp, i32, vp, vp, vp, vp, vp]
     L.gsvox_plan_accumulators.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(i64)]
+    cgp = C.POINTER(GsvoxConeGeometry)
+    L.gsvox_project_scratch_bytes.argtypes = [gp, i32, szp]
+    L.gsvox_project_forward.argtypes = [vp, i64, gp, cgp, vp, i32, vp, vp, vp]
+    L.gsvox_project_backward.argtypes = [vp, gp, cgp, vp, i32, vp, vp, vp]
     dp = C.POINTER(C.c_double)
     L.gsvox_probe_peaks.argtypes = [vp, dp, dp, dp, C.POINTER(i32), vp]
     L.gsvox_error_string.argtypes = [C.c_int]
@@ -173,6 +184,52 @@ def warp_backward(iref, dvf, grid, grad_out, grads=None):
     _check(lib().gsvox_warp_backward(_dev(iref, "iref"), _dev(dvf, "dvf"), C.byref(g), B, _dev(grad_out, "grad_out"),
                                      _dev(gi, "grad_iref"), _dev(gd, "grad_dvf"), _stream()))
     return grads
+
+
+def make_cone_geometry(geom):
+    g = GsvoxConeGeometry()
+    g.sad, g.sdd, g.nu, g.nv = float(geom["sad"]), float(geom["sdd"]), int(geom["nu"]), int(geom["nv"])
+    g.du, g.dv, g.off_u, g.off_v = float(geom["du"]), float(geom["dv"]), float(geom["off_u"]), float(geom["off_v"])
+    for k in range(3):
+        g.iso[k] = float(geom["iso"][k])
+    return g
+
+
+def _project_scratch(grid, B, device):
+    nb = C.c_size_t(0)
+    _check(lib().gsvox_project_scratch_bytes(C.byref(grid), B, C.byref(nb)))
+    return torch.empty(int(nb.value) // 4, dtype=torch.float32, device=device)
+
+
+def project_forward(vol, grid, geom, angles, out=None, scratch=None):
+    """vol [B,nz,ny,nx] (or [nz,ny,nx] shared by all angles), angles: sequence of B radians (host)
+    -> drr [B,nv,nu] (cone-beam line integrals, Joseph's method)."""
+    g, cg = make_grid(*grid), make_cone_geometry(geom)
+    ang = (C.c_float * len(angles))(*[float(a) for a in angles])
+    B = len(angles)
+    shared = vol.dim() == 3
+    if out is None:
+        out = torch.empty((B, cg.nv, cg.nu), dtype=torch.float32, device=vol.device)
+    if scratch is None:
+        scratch = _project_scratch(g, B, vol.device)
+    V = int(vol[0].numel()) if not shared else int(vol.numel())
+    _check(lib().gsvox_project_forward(_dev(vol, "vol"), 0 if shared else V, C.byref(g), C.byref(cg), ang, B,
+                                       _dev(scratch, "scratch"), _dev(out, "drr"), _stream()))
+    return out
+
+
+def project_backward(grad_drr, grid, geom, angles, out=None, scratch=None):
+    """grad_drr [B,nv,nu] -> grad_vol [B,nz,ny,nx] (exact transpose of project_forward)."""
+    g, cg = make_grid(*grid), make_cone_geometry(geom)
+    ang = (C.c_float * len(angles))(*[float(a) for a in angles])
+    B = len(angles)
+    if out is None:
+        out = torch.empty((B, g.dims[2], g.dims[1], g.dims[0]), dtype=torch.float32, device=grad_drr.device)
+    if scratch is None:
+        scratch = _project_scratch(g, B, grad_drr.device)
+    _check(lib().gsvox_project_backward(_dev(grad_drr, "grad_drr"), C.byref(g), C.byref(cg), ang, B,
+                                        _dev(scratch, "scratch"), _dev(out, "grad_vol"), _stream()))
+    return out
 
 
 class Plan:

@@ -1,0 +1,254 @@
+// gsvox_project.cu — SURVEY.md 8(f) rank 4: batched cone-beam forward projector and its transpose,
+// ONE DISTINCT VOLUME PER GANTRY ANGLE (Eq. 12: P[I(x,p)]; "PMF-STGR
+// requires a distinct DRR for each dynamic CBCT at each gantry angle, necessitating sequential
+// projections across views ... future work could implement GPU-based parallelization to compute
+// DRRs from multiple dynamic CBCTs simultaneously").  Eq. 6: I(r) = int sigma(r(t)) dt.
+//
+// Readings P1-P4: circular orbit about the axis through `iso` parallel to z,
+// flat detector; Joseph's method — along the axis on which the ray direction is largest, one sample
+// per voxel-centre plane, bilinear in the plane, zero outside, weight h_a |D| / |D_a|; per-ray
+// constants in fp64 rounded to fp32, sample position fp32(u0 + fp32(m su)) without FMA (the oracle
+// takes the same two roundings); backward = exact transpose.
+//
+// One thread per detector pixel, lanes along u.  Neighbouring rays hit neighbouring in-plane cells,
+// so the four corner reads of a warp are contiguous when the in-plane fast axis is the memory-fast
+// axis: true for y-dominant rays on the x-fastest volume, false for x-dominant rays (lanes then
+// differ in y, one cache line each).  x-dominant rays therefore read a y-fastest copy of the volume
+// (k_transpose_xy, 2 x 4V bytes per volume, < 10 % of the projector's time) — no texture units: point
+// sampling must be exact and hardware filtering has 8-bit weights.  L1/L2-bound gather: per sample 4
+// loads, algorithmic HBM bytes = 4V per volume + 4 per DRR pixel.
+#include <cmath>
+#include "gsvox_internal.cuh"
+
+namespace gsvox {
+
+constexpr int kProjMaxBatch = 64;
+constexpr int kProjThreads = 128;
+
+struct ProjParams {
+    int n[3];                 // nx, ny, nz
+    int nu, nv, B;
+    double o[3], h[3];        // grid origin, spacing
+    double iso[3];
+    double sad, sdd, du, dv, off_u, off_v;
+    double ca[kProjMaxBatch], sa[kProjMaxBatch];
+    long long vol_stride;     // 0: one volume shared by all projections
+};
+
+struct Ray { int axis; float p0, ps, q0, qs, w; int m0, m1; };
+
+// Per-ray constants, fp64 -> fp32 (reading P3).  In-plane axes (b, c) = the two other axes, ascending.
+__device__ __forceinline__ Ray make_ray(const ProjParams& P, int b_, int iu, int iv)
+{
+    const double ca = P.ca[b_], sa = P.sa[b_];
+    const double src[3] = { P.iso[0] + P.sad * ca, P.iso[1] + P.sad * sa, P.iso[2] };
+    const double u = ((double)iu - (P.nu - 1) / 2.0) * P.du + P.off_u;
+    const double v = ((double)iv - (P.nv - 1) / 2.0) * P.dv + P.off_v;
+    const double D[3] = { -P.sdd * ca - u * sa, -P.sdd * sa + u * ca, v };
+    const double ax = fabs(D[0]), ay = fabs(D[1]), az = fabs(D[2]);
+    Ray r;
+    r.axis = (ax >= ay && ax >= az) ? 0 : ((ay >= az) ? 1 : 2);
+    const int a = r.axis, b = (a == 0) ? 1 : 0, c = (a == 2) ? 1 : 2;
+    const double Da = D[a], rb = D[b] / Da, rc = D[c] / Da;
+    const double norm = sqrt(D[0] * D[0] + D[1] * D[1] + D[2] * D[2]);
+    r.p0 = (float)((src[b] - P.o[b] + (P.o[a] - src[a]) * rb) / P.h[b]);
+    r.q0 = (float)((src[c] - P.o[c] + (P.o[a] - src[a]) * rc) / P.h[c]);
+    r.ps = (float)((P.h[a] / P.h[b]) * rb);
+    r.qs = (float)((P.h[a] / P.h[c]) * rc);
+    r.w = (float)(P.h[a] * norm / fabs(Da));
+    // planes on which the sample can touch the grid: -1 < p < n_b and -1 < q < n_c (superset, +-1 plane)
+    float lo = 0.f, hi = (float)(P.n[a] - 1);
+    const float p0[2] = { r.p0, r.q0 }, ps[2] = { r.ps, r.qs }, nn[2] = { (float)P.n[b], (float)P.n[c] };
+    #pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        if (fabsf(ps[k]) > 1e-12f) {
+            const float t0 = (-1.f - p0[k]) / ps[k], t1 = (nn[k] - p0[k]) / ps[k];
+            lo = fmaxf(lo, fminf(t0, t1) - 1.f); hi = fminf(hi, fmaxf(t0, t1) + 1.f);
+        } else if (!(p0[k] > -1.f && p0[k] < nn[k])) hi = -1.f;
+    }
+    r.m0 = (lo <= hi) ? (int)floorf(lo) : 0;
+    r.m1 = (lo <= hi) ? (int)ceilf(hi) : -1;
+    r.m0 = max(r.m0, 0); r.m1 = min(r.m1, P.n[a] - 1);
+    return r;
+}
+
+// Layout of the array a ray samples: x-dominant rays use the y-fastest copy.
+struct Lay { long long sa, sb, sc; int nb, nc; };
+__device__ __forceinline__ Lay make_lay(const ProjParams& P, int axis)
+{
+    const long long nx = P.n[0], ny = P.n[1];
+    Lay L;
+    if (axis == 0)      { L.sa = ny; L.sb = 1;  L.sc = nx * ny; L.nb = P.n[1]; L.nc = P.n[2]; }   // volT[z][x][y]: a = x, b = y, c = z
+    else if (axis == 1) { L.sa = nx; L.sb = 1;  L.sc = nx * ny; L.nb = P.n[0]; L.nc = P.n[2]; }   // vol [z][y][x]: a = y, b = x, c = z
+    else                { L.sa = nx * ny; L.sb = 1; L.sc = nx;  L.nb = P.n[0]; L.nc = P.n[1]; }   // vol: a = z, b = x, c = y
+    return L;
+}
+
+__device__ __forceinline__ bool sample_cell(const Ray& r, int m, int& ib, int& ic, float& fb, float& fc)
+{
+    const float fm = (float)m;
+    const float p = __fadd_rn(r.p0, __fmul_rn(fm, r.ps)), q = __fadd_rn(r.q0, __fmul_rn(fm, r.qs));
+    const bool good = (fabsf(p) < 4194304.f) && (fabsf(q) < 4194304.f);
+    const float pf = floorf(p), qf = floorf(q);
+    fb = p - pf; fc = q - qf;
+    ib = __float_as_int(pf + 12582912.f) - 0x4B400000; ic = __float_as_int(qf + 12582912.f) - 0x4B400000;
+    return good;
+}
+
+__global__ void __launch_bounds__(kProjThreads)
+k_project_forward(const float* __restrict__ vol, const float* __restrict__ volT, ProjParams P, float* __restrict__ drr)
+{
+    const int iu = blockIdx.x * kProjThreads + threadIdx.x, iv = blockIdx.y, b_ = blockIdx.z;
+    if (iu >= P.nu) return;
+    const Ray r = make_ray(P, b_, iu, iv);
+    const Lay L = make_lay(P, r.axis);
+    const long long V = (long long)P.n[0] * P.n[1] * P.n[2];
+    const float* base = ((r.axis == 0) ? volT + (long long)b_ * V : vol + (long long)b_ * P.vol_stride);
+    float acc = 0.f;
+    for (int m = r.m0; m <= r.m1; ++m) {
+        int ib, ic; float fb, fc;
+        if (!sample_cell(r, m, ib, ic, fb, fc)) continue;
+        const float* pl = base + (long long)m * L.sa;
+        const bool b0 = (unsigned)ib < (unsigned)L.nb, b1 = (unsigned)(ib + 1) < (unsigned)L.nb;
+        const bool c0 = (unsigned)ic < (unsigned)L.nc, c1 = (unsigned)(ic + 1) < (unsigned)L.nc;
+        const float* r0 = pl + (long long)(c0 ? ic : 0) * L.sc + ib;
+        const float* r1 = pl + (long long)(c1 ? ic + 1 : 0) * L.sc + ib;
+        const float v00 = (b0 && c0) ? __ldg(r0) : 0.f, v10 = (b1 && c0) ? __ldg(r0 + 1) : 0.f;
+        const float v01 = (b0 && c1) ? __ldg(r1) : 0.f, v11 = (b1 && c1) ? __ldg(r1 + 1) : 0.f;
+        const float l0 = fmaf(fb, v10 - v00, v00), l1 = fmaf(fb, v11 - v01, v01);
+        acc += fmaf(fc, l1 - l0, l0);
+    }
+    drr[((long long)b_ * P.nv + iv) * P.nu + iu] = acc * r.w;
+}
+
+__device__ __forceinline__ void proj_red(float* addr, float v)
+{
+    asm volatile("red.global.add.f32 [%0], %1;" :: "l"(addr), "f"(v) : "memory");
+}
+
+// Transpose: every sample scatters g w {(1-fb)(1-fc), fb(1-fc), (1-fb)fc, fb fc} into its four corners;
+// x-dominant rays scatter into the y-fastest scratch, folded back by k_transpose_add.
+__global__ void __launch_bounds__(kProjThreads)
+k_project_backward(const float* __restrict__ gdrr, ProjParams P, float* __restrict__ gvol, float* __restrict__ gvolT)
+{
+    const int iu = blockIdx.x * kProjThreads + threadIdx.x, iv = blockIdx.y, b_ = blockIdx.z;
+    if (iu >= P.nu) return;
+    const Ray r = make_ray(P, b_, iu, iv);
+    const Lay L = make_lay(P, r.axis);
+    const long long V = (long long)P.n[0] * P.n[1] * P.n[2];
+    float* base = ((r.axis == 0) ? gvolT : gvol) + (long long)b_ * V;
+    const float g = gdrr[((long long)b_ * P.nv + iv) * P.nu + iu] * r.w;
+    if (g == 0.f) return;
+    for (int m = r.m0; m <= r.m1; ++m) {
+        int ib, ic; float fb, fc;
+        if (!sample_cell(r, m, ib, ic, fb, fc)) continue;
+        float* pl = base + (long long)m * L.sa;
+        const bool b0 = (unsigned)ib < (unsigned)L.nb, b1 = (unsigned)(ib + 1) < (unsigned)L.nb;
+        const bool c0 = (unsigned)ic < (unsigned)L.nc, c1 = (unsigned)(ic + 1) < (unsigned)L.nc;
+        float* r0 = pl + (long long)(c0 ? ic : 0) * L.sc + ib;
+        float* r1 = pl + (long long)(c1 ? ic + 1 : 0) * L.sc + ib;
+        const float g0 = g * (1.f - fc), g1 = g * fc;
+        if (b0 && c0) proj_red(r0, g0 * (1.f - fb));
+        if (b1 && c0) proj_red(r0 + 1, g0 * fb);
+        if (b0 && c1) proj_red(r1, g1 * (1.f - fb));
+        if (b1 && c1) proj_red(r1 + 1, g1 * fb);
+    }
+}
+
+// dst[b][z][x][y] = src[b][z][y][x]  (ADD: dst[b][z][y][x] += src[b][z][x][y] with the roles of nx, ny swapped)
+template <bool ADD>
+__global__ void __launch_bounds__(256)
+k_transpose_xy(const float* __restrict__ src, long long src_stride, int nx, int ny, int nz, float* __restrict__ dst)
+{
+    __shared__ float tile[32][33];
+    const int z = blockIdx.z % nz, b_ = blockIdx.z / nz;
+    const long long V = (long long)nx * ny * nz;
+    const float* s = src + (long long)b_ * src_stride + (long long)z * nx * ny;
+    float* d = dst + (long long)b_ * V + (long long)z * nx * ny;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int j = ty; j < 32; j += 8) {
+        const int x = x0 + tx, y = y0 + j;
+        tile[j][tx] = (x < nx && y < ny) ? s[(long long)y * nx + x] : 0.f;
+    }
+    __syncthreads();
+    for (int j = ty; j < 32; j += 8) {
+        const int y = y0 + tx, x = x0 + j;
+        if (x < nx && y < ny) {
+            float* o = d + (long long)x * ny + y;
+            if (ADD) *o += tile[tx][j]; else *o = tile[tx][j];
+        }
+    }
+}
+
+}  // namespace gsvox
+
+using namespace gsvox;
+
+static int fill_params(const gsvox_grid* g, const gsvox_cone_geometry* c, const float* angles_host, int32_t B,
+                       ProjParams* P)
+{
+    if (!g || !c || !angles_host || B < 1 || B > kProjMaxBatch) return GSVOX_EINVAL;
+    for (int k = 0; k < 3; ++k) {
+        if (!(g->spacing[k] > 0.f) || g->dims[k] < 1 || g->dims[k] > GSVOX_MAX_DIM) return GSVOX_EINVAL;
+        P->n[k] = g->dims[k]; P->o[k] = (double)g->origin[k]; P->h[k] = (double)g->spacing[k]; P->iso[k] = (double)c->iso[k];
+    }
+    if ((long long)g->dims[0] * g->dims[1] * g->dims[2] >= (1LL << 31)) return GSVOX_ELIMIT;
+    if (!(c->sad > 0.f) || !(c->sdd > 0.f) || c->nu < 1 || c->nv < 1 || c->nv > 65535 || !(c->du > 0.f) || !(c->dv > 0.f))
+        return GSVOX_EINVAL;
+    P->nu = c->nu; P->nv = c->nv; P->B = B;
+    P->sad = c->sad; P->sdd = c->sdd; P->du = c->du; P->dv = c->dv; P->off_u = c->off_u; P->off_v = c->off_v;
+    for (int b = 0; b < B; ++b) { P->ca[b] = cos((double)angles_host[b]); P->sa[b] = sin((double)angles_host[b]); }
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_project_scratch_bytes(const gsvox_grid* grid, int32_t B, size_t* bytes)
+{
+    if (!grid || !bytes || B < 1 || B > kProjMaxBatch) return GSVOX_EINVAL;
+    for (int k = 0; k < 3; ++k) if (grid->dims[k] < 1) return GSVOX_EINVAL;
+    *bytes = sizeof(float) * (size_t)grid->dims[0] * grid->dims[1] * grid->dims[2] * (size_t)B;
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_project_forward(const float* vol, int64_t vol_stride, const gsvox_grid* grid,
+                                     const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                                     void* scratch, float* drr, void* stream)
+{
+    ProjParams P;
+    int rc = fill_params(grid, geom, angles_host, B, &P);
+    if (rc != GSVOX_OK) return rc;
+    const long long V = (long long)P.n[0] * P.n[1] * P.n[2];
+    if (!vol || !scratch || !drr || (vol_stride != 0 && vol_stride != V)) return GSVOX_EINVAL;
+    P.vol_stride = vol_stride;
+    cudaStream_t st = (cudaStream_t)stream;
+    dim3 tg((P.n[0] + 31) / 32, (P.n[1] + 31) / 32, (unsigned)(P.n[2] * B));
+    k_transpose_xy<false><<<tg, 256, 0, st>>>(vol, vol_stride, P.n[0], P.n[1], P.n[2], (float*)scratch);
+    GSVOX_CUDA(cudaGetLastError());
+    dim3 pg((P.nu + kProjThreads - 1) / kProjThreads, (unsigned)P.nv, (unsigned)B);
+    k_project_forward<<<pg, kProjThreads, 0, st>>>(vol, (const float*)scratch, P, drr);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_project_backward(const float* grad_drr, const gsvox_grid* grid,
+                                      const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                                      void* scratch, float* grad_vol, void* stream)
+{
+    ProjParams P;
+    int rc = fill_params(grid, geom, angles_host, B, &P);
+    if (rc != GSVOX_OK) return rc;
+    if (!grad_drr || !scratch || !grad_vol) return GSVOX_EINVAL;
+    const long long V = (long long)P.n[0] * P.n[1] * P.n[2];
+    P.vol_stride = V;
+    cudaStream_t st = (cudaStream_t)stream;
+    GSVOX_CUDA(cudaMemsetAsync(grad_vol, 0, sizeof(float) * (size_t)V * B, st));
+    GSVOX_CUDA(cudaMemsetAsync(scratch, 0, sizeof(float) * (size_t)V * B, st));
+    dim3 pg((P.nu + kProjThreads - 1) / kProjThreads, (unsigned)P.nv, (unsigned)B);
+    k_project_backward<<<pg, kProjThreads, 0, st>>>(grad_drr, P, grad_vol, (float*)scratch);
+    GSVOX_CUDA(cudaGetLastError());
+    // fold the y-fastest scratch back: grad_vol[z][y][x] += scratch[z][x][y]  (a transpose with nx, ny swapped)
+    dim3 tg((P.n[1] + 31) / 32, (P.n[0] + 31) / 32, (unsigned)(P.n[2] * B));
+    k_transpose_xy<true><<<tg, 256, 0, st>>>((const float*)scratch, V, P.n[1], P.n[0], P.n[2], grad_vol);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
