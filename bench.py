@@ -269,6 +269,26 @@ def next_rows(torch, pkg, hbm_peak_gbs, quick=False):
         "forward": {"ms": mf, "bytes": bf, "GBps": bf / mf / 1e6, "frac_of_hbm_peak": bf / mf / 1e6 / hbm_peak_gbs},
         "backward": {"ms": mb, "bytes": bb, "GBps": bb / mb / 1e6, "frac_of_hbm_peak": bb / mb / 1e6 / hbm_peak_gbs,
                      "note": "8 fp32 atomics per voxel into grad I_ref (L2), merged pairwise by shuffle"}}
+    del iref, dvf, gw, out, gi, gd
+    # ---- rank 4: cone-beam projector, 8 dynamic CBCTs at 8 gantry angles (Table I geometry)
+    pc = gsvox_inputs.project_case(batch=8)
+    from paper_2503_22139_b200 import binding
+    vol, gdrr = dev(pc.vol), dev(pc.grad_drr())
+    ang = list(pc.angles)
+    scratch = binding._project_scratch(binding.make_grid(*pc.grid), 8, vol.device)
+    drr = torch.empty((8, pc.geom["nv"], pc.geom["nu"]), dtype=torch.float32, device="cuda")
+    gv = torch.empty_like(vol)
+    mf = _time_ms(torch, lambda: pkg.project_forward(vol, pc.grid, pc.geom, ang, out=drr, scratch=scratch), 20)
+    mb = _time_ms(torch, lambda: pkg.project_backward(gdrr, pc.grid, pc.geom, ang, out=gv, scratch=scratch), 20)
+    Vp = int(vol[0].numel())
+    npix = pc.geom["nu"] * pc.geom["nv"]
+    samples = 8 * npix * 200                     # one sample per voxel-centre plane of the dominant axis (x or y: 200)
+    bf = 4 * (8 * Vp + 8 * npix)
+    res["project_200x200x100_to_512x384_b8"] = {
+        "forward": {"ms": mf, "samples_per_s": samples / (mf * 1e-3), "bytes": bf, "GBps": bf / mf / 1e6,
+                    "frac_of_hbm_peak": bf / mf / 1e6 / hbm_peak_gbs,
+                    "note": "L1/L2-bound gather: 4 corner reads per sample, volumes (16 MB each) L2-resident"},
+        "backward": {"ms": mb, "samples_per_s": samples / (mb * 1e-3), "note": "4 fp32 atomics per sample"}}
     return res
 
 

@@ -104,19 +104,30 @@ k_project_forward(const float* __restrict__ vol, const float* __restrict__ volT,
     const Lay L = make_lay(P, r.axis);
     const long long V = (long long)P.n[0] * P.n[1] * P.n[2];
     const float* base = ((r.axis == 0) ? volT + (long long)b_ * V : vol + (long long)b_ * P.vol_stride);
+    // 32-bit offsets inside one volume (V < 2^31, checked on the host); cells wholly inside the plane
+    // (all but the rim) take the path without bounds tests
+    const int sa = (int)L.sa, sc = (int)L.sc, nb1 = L.nb - 1, nc1 = L.nc - 1;
     float acc = 0.f;
+    #pragma unroll 4
     for (int m = r.m0; m <= r.m1; ++m) {
         int ib, ic; float fb, fc;
-        if (!sample_cell(r, m, ib, ic, fb, fc)) continue;
-        const float* pl = base + (long long)m * L.sa;
-        const bool b0 = (unsigned)ib < (unsigned)L.nb, b1 = (unsigned)(ib + 1) < (unsigned)L.nb;
-        const bool c0 = (unsigned)ic < (unsigned)L.nc, c1 = (unsigned)(ic + 1) < (unsigned)L.nc;
-        const float* r0 = pl + (long long)(c0 ? ic : 0) * L.sc + ib;
-        const float* r1 = pl + (long long)(c1 ? ic + 1 : 0) * L.sc + ib;
-        const float v00 = (b0 && c0) ? __ldg(r0) : 0.f, v10 = (b1 && c0) ? __ldg(r0 + 1) : 0.f;
-        const float v01 = (b0 && c1) ? __ldg(r1) : 0.f, v11 = (b1 && c1) ? __ldg(r1 + 1) : 0.f;
-        const float l0 = fmaf(fb, v10 - v00, v00), l1 = fmaf(fb, v11 - v01, v01);
-        acc += fmaf(fc, l1 - l0, l0);
+        const bool good = sample_cell(r, m, ib, ic, fb, fc);
+        if ((unsigned)ib < (unsigned)nb1 && (unsigned)ic < (unsigned)nc1 && good) {
+            const float* q0 = base + (m * sa + ic * sc + ib);
+            const float v00 = __ldg(q0), v10 = __ldg(q0 + 1), v01 = __ldg(q0 + sc), v11 = __ldg(q0 + sc + 1);
+            const float l0 = fmaf(fb, v10 - v00, v00), l1 = fmaf(fb, v11 - v01, v01);
+            acc += fmaf(fc, l1 - l0, l0);
+        } else if (good) {
+            const float* pl = base + (long long)m * L.sa;
+            const bool b0 = (unsigned)ib < (unsigned)L.nb, b1 = (unsigned)(ib + 1) < (unsigned)L.nb;
+            const bool c0 = (unsigned)ic < (unsigned)L.nc, c1 = (unsigned)(ic + 1) < (unsigned)L.nc;
+            const float* r0 = pl + (long long)(c0 ? ic : 0) * L.sc + ib;
+            const float* r1 = pl + (long long)(c1 ? ic + 1 : 0) * L.sc + ib;
+            const float v00 = (b0 && c0) ? __ldg(r0) : 0.f, v10 = (b1 && c0) ? __ldg(r0 + 1) : 0.f;
+            const float v01 = (b0 && c1) ? __ldg(r1) : 0.f, v11 = (b1 && c1) ? __ldg(r1 + 1) : 0.f;
+            const float l0 = fmaf(fb, v10 - v00, v00), l1 = fmaf(fb, v11 - v01, v01);
+            acc += fmaf(fc, l1 - l0, l0);
+        }
     }
     drr[((long long)b_ * P.nv + iv) * P.nu + iu] = acc * r.w;
 }
