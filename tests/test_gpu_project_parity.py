@@ -64,6 +64,14 @@ def test_project_wide_detector_rays_miss_the_volume(pkg):
                                           sdd=300.0, seed=52))
 
 
+def test_project_steep_cone_z_dominant_rays(pkg):
+    """Outer detector rows run mostly along z: the third dominant-axis branch, forward and transpose."""
+    case = gsvox_inputs.project_case(batch=3, dims=(14, 12, 30), nu=9, nv=41, du=6.0, dv=12.0, sad=60.0, sdd=90.0,
+                                     seed=56, angles=[0.3, 1.7, 4.0])
+    assert (oracle.cone_rays(case.grid, case.geom, np.float32(0.3))["axis"] == 2).any()
+    parity(pkg, case)
+
+
 def test_project_shared_volume_equals_batched_copies(pkg):
     case = gsvox_inputs.project_case(batch=4, dims=(32, 28, 16), nu=64, nv=32, du=2.5, dv=2.5, sad=250.0, sdd=400.0, seed=53)
     v0 = dev(case.vol[0])

@@ -151,3 +151,16 @@ def test_shared_volume_and_rays_missing_the_grid():
     d2 = oracle.project_forward(np.stack([vol, vol]), grid, geom, [0.0, 1.0])
     assert np.array_equal(d, d2)
     assert d[0, 0, 0] == 0.0 and d[1, -1, -1] == 0.0 and d.max() > 0
+
+
+def test_steep_cone_rays_take_z_as_the_dominant_axis():
+    """A tall detector close to the source: the outer rows run mostly along z (axis 2), the branch a
+    clinical geometry never reaches.  Same independent sampler."""
+    rng = np.random.default_rng(6)
+    grid, geom = setup(dims=(14, 12, 30), nu=9, nv=41, du=6.0, dv=12.0, sad=60.0, sdd=90.0)
+    vol = rng.standard_normal((30, 12, 14)).astype(np.float32)
+    rays = oracle.cone_rays(grid, geom, np.float32(0.3))
+    assert (rays["axis"] == 2).any() and (rays["axis"] == 0).any()
+    got = oracle.project_forward(vol, grid, geom, [0.3])[0]
+    ref = independent_projection(vol, grid, geom, np.float64(np.float32(0.3)))
+    assert np.abs(got - ref).max() <= 3e-5 * np.abs(ref).max()
