@@ -438,3 +438,7 @@ def project_backward(grad_drr, grid, geom, angles):
             for lin, w in zip(idx, wt):
                 out[bi] += np.bincount(lin, weights=w * gs, minlength=out.shape[1])
     return out.reshape(angles.size, nz, ny, nx)
+
+
+# Gaussian-splat X-ray rasterizer (Eq. 6-9) — oracle/splat.py (torch fp64)
+from .splat import splat_backward, splat_forward, splat_forward_at, splat_terms   # noqa: E402,F401
