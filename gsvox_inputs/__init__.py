@@ -369,6 +369,57 @@ def project_case(batch=8, dims=(200, 200, 100), spacing=(2.0, 2.0, 2.0), nu=512,
                        origin=origin, spacing=tuple(spacing), seed=seed)
 
 
+@dataclass
+class SplatCase:
+    """Inputs of the Gaussian-splat X-ray rasterizer (Eq. 6-9, Table I)."""
+    name: str
+    pos: np.ndarray             # [n,3] fp32, world units (mm), isocentre at the origin
+    scale: np.ndarray           # [n,3]
+    quat: np.ndarray            # [n,4]
+    rho: np.ndarray             # [n]
+    angles: np.ndarray          # [B] fp32 radians
+    geom: dict
+    seed: object = 0
+
+    @property
+    def n(self):
+        return int(self.pos.shape[0])
+
+    @property
+    def batch(self):
+        return int(self.angles.shape[0])
+
+    def grad_drr(self):
+        rng = np.random.default_rng([80, self.batch] + list(np.atleast_1d(self.seed)))
+        return rng.standard_normal((self.batch, self.geom["nv"], self.geom["nu"]), dtype=np.float32)
+
+
+def splat_case(n=50_000, batch=8, extent=(400.0, 400.0, 200.0), voxel=2.0, nu=512, nv=384, du=0.776, dv=0.776,
+               sad=1000.0, sdd=1500.0, off_u=0.0, off_v=0.0, seed=8, angles=None, scales=(1.0, 4.0)):
+    """Stage-1 stand-in: the reference-frame CBCT Gaussians of config 2 in world
+    units — M = 50 000 (XCAT), centres uniform in an ellipsoid with semi-axes
+    0.45/0.35/0.48 of a 400 x 400 x 200 mm field of view (200 x 200 x 100 voxels of 2 mm), scales
+    log-uniform 1-4 voxels, random quaternions, 3-tissue attenuation mix — splatted onto the Table I
+    detector (512 x 384 pixels of 0.776 mm, SAD 1000 / SDD 1500) at `batch` gantry angles."""
+    rng = np.random.default_rng(seed)
+    semi = np.array([0.45, 0.35, 0.48]) * np.asarray(extent)
+    pts = np.empty((0, 3))
+    while pts.shape[0] < n:
+        c = rng.uniform(-1.0, 1.0, size=(2 * n + 16, 3))
+        pts = np.concatenate([pts, c[(c * c).sum(1) <= 1.0]])
+    pos = semi * pts[:n]
+    scale = _log_uniform(rng, scales[0] * voxel, scales[1] * voxel, (n, 3))
+    quat = _unit_quats(rng, n)
+    tissue = rng.choice(np.array([0.02, 0.2, 0.5]), size=n, p=[0.6, 0.3, 0.1])
+    rho = tissue + rng.normal(0.0, 0.01, size=n)
+    if angles is None:
+        angles = rng.uniform(0.0, 2 * np.pi, size=batch)
+    geom = dict(sad=float(sad), sdd=float(sdd), nu=int(nu), nv=int(nv), du=float(du), dv=float(dv),
+                off_u=float(off_u), off_v=float(off_v), iso=[0.0, 0.0, 0.0])
+    return SplatCase("splat_n%d_b%d" % (n, len(angles)), _f32(pos), _f32(scale), _f32(quat), _f32(rho),
+                     np.asarray(angles, np.float32), geom, seed=seed)
+
+
 FULL = {
     "config1": lambda: [config1()],
     "config2": lambda: [config2()],

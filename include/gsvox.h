@@ -256,6 +256,36 @@ int gsvox_project_forward(const float* vol, int64_t vol_stride, const gsvox_grid
 int gsvox_project_backward(const float* grad_drr, const gsvox_grid* grid, const gsvox_cone_geometry* geom,
                            const float* angles_host, int32_t B, void* scratch, float* grad_vol, void* stream);
 
+/* ---- Gaussian-splat X-ray rasterizer (Eq. 6-9) ---------------
+ * drr[b, iv, iu] = sum_i rho^_i exp(-1/2 (x^ - p^_i)^T Sigma^_i^-1 (x^ - p^_i))  for gantry angle b, with
+ * Sigma~ = J W Sigma W^T J^T (Eq. 8), Sigma^ = Sigma~[0:2,0:2], rho^ = rho sqrt(2 pi |Sigma~| / |Sigma^|)
+ * (Eq. 9).  Scanner = gsvox_cone_geometry (reading R1 = P1); camera frame at the source, rows of W =
+ * (u, v, central ray); ray space phi(t) = (t0/t2, t1/t2, |t|) (R2); cutoff = inclusive pixel box of the
+ * 3-sigma ellipse (R4); Gaussians at or behind the source plane, or degenerate, are skipped (R5).
+ * pos [n,3], scale [n,3], quat [n,4] (w,x,y,z), rho [n]: DEVICE pointers in WORLD units; angles_host
+ * [B] radians, HOST pointer, 1 <= B <= 64; drr [B,nv,nu] OVERWRITTEN.  workspace: caller-owned
+ * DEVICE memory, 256-byte aligned, gsvox_splat_workspace_bytes() long; key_capacity bounds the number
+ * of (16x16 tile, angle, Gaussian) keys: beyond it the call writes zeros and gsvox_splat_status
+ * reports overflow and the capacity needed.  No host synchronisation.                            */
+int gsvox_splat_workspace_bytes(int64_t n, const gsvox_cone_geometry* geom, int32_t B,
+                                int64_t key_capacity, size_t* bytes);
+int gsvox_splat_forward(const float* pos, const float* scale, const float* quat, const float* rho,
+                        int64_t n, const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                        void* workspace, size_t workspace_bytes, int64_t key_capacity,
+                        float* drr, void* stream);
+/* Backward for grad_drr = dL/ddrr [B,nv,nu], boxes frozen (R6).  MUST follow gsvox_splat_forward
+ * with the same inputs, geometry, angles and workspace (it reuses the 2D records and the tile
+ * lists).  grad_rho [n], grad_pos [n,3], grad_scale [n,3], grad_quat [n,4] OVERWRITTEN.          */
+int gsvox_splat_backward(const float* pos, const float* scale, const float* quat, const float* rho,
+                         int64_t n, const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                         void* workspace, size_t workspace_bytes, int64_t key_capacity,
+                         const float* grad_drr, float* grad_rho, float* grad_pos, float* grad_scale,
+                         float* grad_quat, void* stream);
+/* Outcome of the latest gsvox_splat_forward on this workspace (SYNCHRONISES): keys needed, pairs
+ * inside the cutoff over all angles, overflow flag, Gaussians skipped as degenerate.  HOST outputs. */
+int gsvox_splat_status(const void* workspace, int64_t* keys_needed, int64_t* pairs, int32_t* overflow,
+                       int32_t* skipped, void* stream);
+
 /* Live ALU rooflines of the device the calling thread has current (the hot path is
  * FP32-issue / MUFU bound, and MEASURED_PEAKS.json holds no FP32 figure).  Runs three register-only
  * microbenchmarks on `stream` and SYNCHRONISES: scalar FFMA chains (fp32_tflops, 2 flops per lane

@@ -1,8 +1,8 @@
 """gsvox: B200-native (sm_100a) differentiable 3D Gaussian voxelizer — the data-parallel hot
 path of PMF-STGR (arXiv 2503.22139, Eq. 4-5).  See DESIGN.md and include/gsvox.h."""
-from .binding import (EXPORTS, K_NAMES, LIB_PATH, GsvoxError, GsvoxGrid, GsvoxStatus, Plan, lib,
+from .binding import (EXPORTS, K_NAMES, LIB_PATH, GsvoxError, GsvoxGrid, GsvoxStatus, Plan, Splatter, lib,
                       make_grid, mbc_combine_backward, mbc_combine_forward, probe_peaks, project_backward, project_forward, warp_backward,
                       warp_forward)
 
-__all__ = ["EXPORTS", "K_NAMES", "LIB_PATH", "GsvoxError", "GsvoxGrid", "GsvoxStatus", "Plan", "lib",
+__all__ = ["EXPORTS", "K_NAMES", "LIB_PATH", "GsvoxError", "GsvoxGrid", "GsvoxStatus", "Plan", "Splatter", "lib",
            "make_grid", "mbc_combine_backward", "mbc_combine_forward", "probe_peaks", "project_backward", "project_forward", "warp_backward", "warp_forward"]

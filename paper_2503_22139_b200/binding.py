@@ -23,6 +23,7 @@ EXPORTS = [
     "gsvox_mbc_combine_forward", "gsvox_mbc_combine_backward", "gsvox_warp_forward", "gsvox_warp_backward",
     "gsvox_plan_set_slab", "gsvox_backward_accumulate", "gsvox_backward_finish", "gsvox_plan_accumulators",
     "gsvox_project_scratch_bytes", "gsvox_project_forward", "gsvox_project_backward",
+    "gsvox_splat_workspace_bytes", "gsvox_splat_forward", "gsvox_splat_backward", "gsvox_splat_status",
 ]
 
 
@@ -88,6 +89,10 @@ def lib():
     L.gsvox_project_scratch_bytes.argtypes = [gp, i32, szp]
     L.gsvox_project_forward.argtypes = [vp, i64, gp, cgp, vp, i32, vp, vp, vp]
     L.gsvox_project_backward.argtypes = [vp, gp, cgp, vp, i32, vp, vp, vp]
+    L.gsvox_splat_workspace_bytes.argtypes = [i64, cgp, i32, i64, szp]
+    L.gsvox_splat_forward.argtypes = [vp, vp, vp, vp, i64, cgp, vp, i32, vp, C.c_size_t, i64, vp, vp]
+    L.gsvox_splat_backward.argtypes = [vp, vp, vp, vp, i64, cgp, vp, i32, vp, C.c_size_t, i64, vp, vp, vp, vp, vp, vp]
+    L.gsvox_splat_status.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i32), C.POINTER(i32), vp]
     dp = C.POINTER(C.c_double)
     L.gsvox_probe_peaks.argtypes = [vp, dp, dp, dp, C.POINTER(i32), vp]
     L.gsvox_error_string.argtypes = [C.c_int]
@@ -230,6 +235,55 @@ def project_backward(grad_drr, grid, geom, angles, out=None, scratch=None):
     _check(lib().gsvox_project_backward(_dev(grad_drr, "grad_drr"), C.byref(g), C.byref(cg), ang, B,
                                         _dev(scratch, "scratch"), _dev(out, "grad_vol"), _stream()))
     return out
+
+
+class Splatter:
+    """Gaussian-splat X-ray rasterizer (gsvox_splat_*): owns the torch workspace for n Gaussians, B angles."""
+
+    def __init__(self, n_max, geom, batch, key_capacity=None, device="cuda"):
+        self.geom, self.cg = dict(geom), make_cone_geometry(geom)
+        self.n_max, self.batch = int(n_max), int(batch)
+        if key_capacity is None:
+            key_capacity = max(1 << 20, 48 * self.n_max * self.batch)
+        self.key_capacity = int(key_capacity)
+        self.device = torch.device(device)
+        nb = C.c_size_t(0)
+        _check(lib().gsvox_splat_workspace_bytes(self.n_max, C.byref(self.cg), self.batch, self.key_capacity, C.byref(nb)))
+        self.workspace_bytes = int(nb.value)
+        self._ws = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        self._base = (self._ws.data_ptr() + 255) & ~255
+
+    def _angles(self, angles):
+        if len(angles) != self.batch:
+            raise GsvoxError("expected %d angles" % self.batch)
+        return (C.c_float * len(angles))(*[float(a) for a in angles])
+
+    def forward(self, pos, scale, quat, rho, angles, out=None):
+        n = int(pos.shape[0])
+        if out is None:
+            out = torch.empty((self.batch, self.cg.nv, self.cg.nu), dtype=torch.float32, device=self.device)
+        _check(lib().gsvox_splat_forward(_dev(pos, "pos"), _dev(scale, "scale"), _dev(quat, "quat"), _dev(rho, "rho"), n,
+                                         C.byref(self.cg), self._angles(angles), self.batch, C.c_void_p(self._base),
+                                         self.workspace_bytes, self.key_capacity, _dev(out, "drr"), _stream()))
+        return out
+
+    def backward(self, pos, scale, quat, rho, angles, grad_drr, grads=None):
+        n = int(pos.shape[0])
+        if grads is None:
+            mk = lambda *sh: torch.empty(sh, dtype=torch.float32, device=self.device)
+            grads = (mk(n), mk(n, 3), mk(n, 3), mk(n, 4))
+        gr, gp, gs, gq = grads
+        _check(lib().gsvox_splat_backward(_dev(pos, "pos"), _dev(scale, "scale"), _dev(quat, "quat"), _dev(rho, "rho"), n,
+                                          C.byref(self.cg), self._angles(angles), self.batch, C.c_void_p(self._base),
+                                          self.workspace_bytes, self.key_capacity, _dev(grad_drr, "grad_drr"),
+                                          _dev(gr, "grad_rho"), _dev(gp, "grad_pos"), _dev(gs, "grad_scale"),
+                                          _dev(gq, "grad_quat"), _stream()))
+        return grads
+
+    def status(self):
+        k, p, o, sk = C.c_int64(0), C.c_int64(0), C.c_int32(0), C.c_int32(0)
+        _check(lib().gsvox_splat_status(C.c_void_p(self._base), C.byref(k), C.byref(p), C.byref(o), C.byref(sk), _stream()))
+        return {"keys_needed": int(k.value), "pairs": int(p.value), "overflow": bool(o.value), "skipped": int(sk.value)}
 
 
 class Plan:

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgsvox.so")
 SOURCES = ["gsvox_api.cu", "gsvox_host.cu", "gsvox_preprocess.cu", "gsvox_forward.cu", "gsvox_backward.cu",
-           "gsvox_epilogue.cu", "gsvox_probe.cu", "gsvox_dvf.cu", "gsvox_warp.cu", "gsvox_project.cu"]
+           "gsvox_epilogue.cu", "gsvox_probe.cu", "gsvox_dvf.cu", "gsvox_warp.cu", "gsvox_project.cu", "gsvox_splat.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--use_fast_math", "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "-cudart", "static"]
 

@@ -159,6 +159,9 @@ int cuda_fail(cudaError_t e, const char* what);          // records text, return
 int launch_preprocess(gsvox_plan* p, const float* pos, const float* scale, const float* quat,
                       int64_t n, cudaStream_t st);
 int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st);
+int launch_exclusive_scan(uint32_t* cnt, int nbins, uint32_t* partial, uint32_t* start,
+                          unsigned long long* keys_needed, unsigned int* overflow,
+                          unsigned long long key_capacity, cudaStream_t st);
 int launch_forward(gsvox_plan* p, const float* weight, int channels, float* out, cudaStream_t st);
 int launch_backward(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
                     float* gw, float* gp, float* gs, float* gq, cudaStream_t st);

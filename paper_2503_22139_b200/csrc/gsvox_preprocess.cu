@@ -270,7 +270,8 @@ k_scan_reduce(const uint32_t* __restrict__ cnt, int nbins, uint32_t* __restrict_
 }
 
 __global__ void __launch_bounds__(1024)
-k_scan_partials(uint32_t* __restrict__ partial, int nblocks, DevStatus* __restrict__ status,
+k_scan_partials(uint32_t* __restrict__ partial, int nblocks, unsigned long long* __restrict__ keys_needed,
+                unsigned int* __restrict__ overflow,
                 unsigned long long key_capacity)
 {
     // single block: serial-per-thread chunks + warp scans; nblocks is small (<= a few thousand)
@@ -292,8 +293,8 @@ k_scan_partials(uint32_t* __restrict__ partial, int nblocks, DevStatus* __restri
         if (b0 + k < nblocks) { uint32_t v = partial[b0 + k]; partial[b0 + k] = (uint32_t)run; run += v; }
     if (threadIdx.x == 1023) {
         unsigned long long total = sh[1023];
-        status->keys_needed = total;
-        status->overflow = (total > key_capacity || total > 0xfffffff0ull) ? 1u : 0u;
+        *keys_needed = total;
+        *overflow = (total > key_capacity || total > 0xfffffff0ull) ? 1u : 0u;
     }
 }
 
@@ -324,6 +325,21 @@ k_scan_apply(uint32_t* __restrict__ cnt, int nbins, const uint32_t* __restrict__
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 255) start[nbins] = run;
 }
 
+// cnt[nbins] -> start[nbins + 1] (exclusive scan, start[nbins] = total); cnt is overwritten by the same
+// offsets (write cursors for the scatter pass); *keys_needed = total, *overflow = total > capacity.
+// partial: scratch of ceil(nbins / kScanItemsPerBlock) + 1 words.  Shared by the voxelizer and the rasterizer.
+int launch_exclusive_scan(uint32_t* cnt, int nbins, uint32_t* partial, uint32_t* start,
+                          unsigned long long* keys_needed, unsigned int* overflow,
+                          unsigned long long key_capacity, cudaStream_t st)
+{
+    const int sblocks = (nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock;
+    k_scan_reduce<<<sblocks, 256, 0, st>>>(cnt, nbins, partial);
+    k_scan_partials<<<1, 1024, 0, st>>>(partial, sblocks, keys_needed, overflow, key_capacity);
+    k_scan_apply<<<sblocks, 256, 0, st>>>(cnt, nbins, partial, start);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
+
 int launch_preprocess(gsvox_plan* p, const float* pos, const float* scale, const float* quat,
                       int64_t n, cudaStream_t st)
 {
@@ -347,17 +363,11 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
         k_keys<0><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status);
         GSVOX_CUDA(cudaGetLastError());
     }
-    int sblocks = (p->nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock;
     { LaunchScope ls(p, GSVOX_K_SCAN, st);
-      k_scan_reduce<<<sblocks, 256, 0, st>>>(p->bin_count, p->nbins, p->scan_partial);
-      GSVOX_CUDA(cudaGetLastError()); }
-    { LaunchScope ls(p, GSVOX_K_SCAN, st);
-      k_scan_partials<<<1, 1024, 0, st>>>(p->scan_partial, sblocks, p->status,
-                                          (unsigned long long)p->key_capacity);
-      GSVOX_CUDA(cudaGetLastError()); }
-    { LaunchScope ls(p, GSVOX_K_SCAN, st);
-      k_scan_apply<<<sblocks, 256, 0, st>>>(p->bin_count, p->nbins, p->scan_partial, p->bin_start);
-      GSVOX_CUDA(cudaGetLastError()); }
+      int rc = launch_exclusive_scan(p->bin_count, p->nbins, p->scan_partial, p->bin_start, &p->status->keys_needed,
+                                     &p->status->overflow, (unsigned long long)p->key_capacity, st);
+      p->launches[GSVOX_K_SCAN] += 2;                       // the scan is three kernels
+      if (rc != GSVOX_OK) return rc; }
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_SCATTER, st);
         k_keys<1><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status);

@@ -1,0 +1,483 @@
+// gsvox_splat.cu — SURVEY.md 8(f) rank 3: Gaussian-splat X-ray rasterizer, forward and backward, batched
+// over the gantry angles of a training batch (Eq. 6-9; Stage 1 = 5000 of the 7000
+// iterations).
+//
+//   Eq. 8   Sigma~ = J W Sigma W^T J^T          (local affine approximation of the projective mapping)
+//   Eq. 9   I(r) = sum_i rho^_i exp(-1/2 (x^ - p^_i)^T Sigma^_i^-1 (x^ - p^_i)),
+//           Sigma^ = Sigma~[0:2,0:2],  rho^ = rho sqrt(2 pi |Sigma~| / |Sigma^|)
+// Readings R1-R6 (the paper leaves phi, J, W to "scanner parameters"): the
+// projector's scanner (P1); camera frame at the source with rows of W = (u, v, central ray);
+// ray space phi(t) = (t0/t2, t1/t2, |t|); pixel = SDD x^ on the detector grid; cutoff = inclusive
+// pixel box of the 3-sigma ellipse, decided in fp64; t2 <= 0 or degenerate -> skipped; backward
+// with frozen boxes.
+//
+// Same machinery as the voxelizer, one dimension down: s1 per-(angle, Gaussian) 2D record in fp64
+// (centre split into integer pixel + fp32 fraction, conic, amplitude, box) with the tile counts
+// fused in; s2 exclusive scan (shared with a2) + scatter: counting sort of (tile, Gaussian) keys,
+// 16x16-pixel tiles; s3 one CTA per (tile, angle), keys staged through shared memory, one thread
+// per pixel, ex2.approx; s4 backward: the tile's upstream gradient in shared memory, ONE THREAD PER
+// KEY walks box ∩ tile and reduces its six 2D gradients in registers, one vector atomic per key;
+// s5 per-Gaussian chain rule through Sigma^-1, |Sigma~|/|Sigma^|, J(t), W, R(q), S in fp64, summed
+// over the angles without atomics.
+#include <cmath>
+#include "gsvox_internal.cuh"
+
+namespace gsvox {
+
+constexpr int kSplatTile = 16;
+constexpr int kSplatMaxBatch = 64;
+constexpr int kSplatBatch = 64;                 // keys staged per __syncthreads
+constexpr double kSplatKappa = GSVOX_SIGMA_CUTOFF;
+
+struct __align__(16) Splat2D {
+    float cfu, cfv;        // fractional part of the centre in pixels, [-0.5, 0.5]
+    float A, B;            // conic in pixel units, already times -log2(e)/2:  E = A dx^2 + 2 B dx dy + C dy^2 (base 2)
+    float C, amp;
+    int16_t ciu, civ;      // integer part of the centre (may be off the detector)
+    int16_t u0, v0, u1, v1;   // inclusive pixel box; empty <=> u1 < u0
+    int32_t pad;
+};
+static_assert(sizeof(Splat2D) == 48, "Splat2D must be 48 bytes");
+
+struct SplatStatus { unsigned long long keys_needed, pairs; unsigned int overflow, skipped; };
+
+struct SplatParams {
+    int n, B, nu, nv, ntx, nty;
+    double sad, sdd, du, dv, off_u, off_v, iso[3];
+    double ca[kSplatMaxBatch], sa[kSplatMaxBatch];
+};
+
+struct SplatWs {            // views into the caller's workspace
+    SplatStatus* status; Splat2D* rec; uint32_t* bin_count; uint32_t* bin_start; uint32_t* partial;
+    uint32_t* keys; float* acc; int nbins; size_t total;
+};
+
+// Everything Eq. 8-9 needs for one (angle, Gaussian), fp64.
+struct SplatTerms {
+    bool valid;
+    double R[9], Sig[9], t[3], ell, T[9], St[9], det_t, det_h, amp_over_rho, P[3], dp, cu, cv;
+};
+
+__device__ __forceinline__ void mat3mul(const double* a, const double* b, double* c)
+{
+    #pragma unroll
+    for (int i = 0; i < 3; ++i)
+        #pragma unroll
+        for (int j = 0; j < 3; ++j) c[3 * i + j] = a[3 * i] * b[j] + a[3 * i + 1] * b[3 + j] + a[3 * i + 2] * b[6 + j];
+}
+
+__device__ __forceinline__ void splat_W(const SplatParams& P, int b, double* W, double* src)
+{
+    const double ca = P.ca[b], sa = P.sa[b];
+    W[0] = -sa; W[1] = ca;  W[2] = 0.0;       // u
+    W[3] = 0.0; W[4] = 0.0; W[5] = 1.0;       // v
+    W[6] = -ca; W[7] = -sa; W[8] = 0.0;       // central ray, source -> detector
+    src[0] = P.iso[0] + P.sad * ca; src[1] = P.iso[1] + P.sad * sa; src[2] = P.iso[2];
+}
+
+__device__ void splat_terms(const SplatParams& P, int b, const float* __restrict__ pos, const float* __restrict__ scale,
+                            const float* __restrict__ quat, int g, SplatTerms& o)
+{
+    const double p[3] = { pos[3 * g], pos[3 * g + 1], pos[3 * g + 2] };
+    const double s[3] = { scale[3 * g], scale[3 * g + 1], scale[3 * g + 2] };
+    const double q[4] = { quat[4 * g], quat[4 * g + 1], quat[4 * g + 2], quat[4 * g + 3] };
+    o.valid = false;
+    bool bad = false;
+    for (int k = 0; k < 3; ++k) bad |= !isfinite(p[k]) || !isfinite(s[k]) || !(s[k] > 0.0);
+    for (int k = 0; k < 4; ++k) bad |= !isfinite(q[k]);
+    const double n2 = q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3];
+    if (bad || !(n2 > 0.0)) return;
+    const double nn = sqrt(n2), r = q[0] / nn, x = q[1] / nn, y = q[2] / nn, z = q[3] / nn;
+    double* R = o.R;
+    R[0] = 1 - 2 * (y * y + z * z); R[1] = 2 * (x * y - r * z); R[2] = 2 * (x * z + r * y);
+    R[3] = 2 * (x * y + r * z); R[4] = 1 - 2 * (x * x + z * z); R[5] = 2 * (y * z - r * x);
+    R[6] = 2 * (x * z - r * y); R[7] = 2 * (y * z + r * x); R[8] = 1 - 2 * (x * x + y * y);
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j)
+            o.Sig[3 * i + j] = R[3 * i] * s[0] * s[0] * R[3 * j] + R[3 * i + 1] * s[1] * s[1] * R[3 * j + 1]
+                             + R[3 * i + 2] * s[2] * s[2] * R[3 * j + 2];
+    double W[9], src[3];
+    splat_W(P, b, W, src);
+    const double d[3] = { p[0] - src[0], p[1] - src[1], p[2] - src[2] };
+    for (int i = 0; i < 3; ++i) o.t[i] = W[3 * i] * d[0] + W[3 * i + 1] * d[1] + W[3 * i + 2] * d[2];
+    const double t0 = o.t[0], t1 = o.t[1], t2 = o.t[2];
+    if (!(t2 > 0.0)) return;                                   // R5: at or behind the source plane
+    o.ell = sqrt(t0 * t0 + t1 * t1 + t2 * t2);
+    const double J[9] = { 1 / t2, 0, -t0 / (t2 * t2),  0, 1 / t2, -t1 / (t2 * t2),  t0 / o.ell, t1 / o.ell, t2 / o.ell };
+    mat3mul(J, W, o.T);
+    double TS[9], Tt[9];
+    mat3mul(o.T, o.Sig, TS);
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) Tt[3 * i + j] = o.T[3 * j + i];
+    mat3mul(TS, Tt, o.St);
+    const double* S = o.St;
+    o.det_t = S[0] * (S[4] * S[8] - S[5] * S[7]) - S[1] * (S[3] * S[8] - S[5] * S[6]) + S[2] * (S[3] * S[7] - S[4] * S[6]);
+    o.det_h = S[0] * S[4] - S[1] * S[1];
+    const double ku = P.sdd / P.du, kv = P.sdd / P.dv;
+    o.P[0] = S[0] * ku * ku; o.P[1] = S[1] * ku * kv; o.P[2] = S[4] * kv * kv;
+    o.dp = o.P[0] * o.P[2] - o.P[1] * o.P[1];
+    o.cu = (P.sdd * t0 / t2 - P.off_u) / P.du + (P.nu - 1) / 2.0;
+    o.cv = (P.sdd * t1 / t2 - P.off_v) / P.dv + (P.nv - 1) / 2.0;
+    if (!(o.det_t > 0.0) || !(o.det_h > 0.0) || !(o.dp > 0.0) || !isfinite(o.cu) || !isfinite(o.cv)) return;
+    o.amp_over_rho = sqrt(2.0 * 3.14159265358979323846 * o.det_t / o.det_h);
+    o.valid = true;
+}
+
+// s1: record + tile counts.  One thread per (angle, Gaussian).
+__global__ void __launch_bounds__(128)
+k_splat_pre(SplatParams P, const float* __restrict__ pos, const float* __restrict__ scale, const float* __restrict__ quat,
+            const float* __restrict__ rho, Splat2D* __restrict__ rec, uint32_t* __restrict__ bin_count,
+            SplatStatus* __restrict__ status)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)P.n * P.B) return;
+    const int b = (int)(idx / P.n), g = (int)(idx - (long long)b * P.n);
+    Splat2D r;
+    r.cfu = r.cfv = r.A = r.B = r.C = r.amp = 0.f; r.ciu = r.civ = 0; r.u0 = r.v0 = 0; r.u1 = r.v1 = -1; r.pad = 0;
+    SplatTerms o;
+    splat_terms(P, b, pos, scale, quat, g, o);
+    const double rh = (double)rho[g];
+    if (o.valid && isfinite(rh)) {
+        const double ru = kSplatKappa * sqrt(o.P[0]), rv = kSplatKappa * sqrt(o.P[2]);
+        double u0 = ceil(o.cu - ru), u1 = floor(o.cu + ru), v0 = ceil(o.cv - rv), v1 = floor(o.cv + rv);
+        if (u0 < 0.0) u0 = 0.0; if (v0 < 0.0) v0 = 0.0;
+        if (u1 > P.nu - 1.0) u1 = P.nu - 1.0; if (v1 > P.nv - 1.0) v1 = P.nv - 1.0;
+        if (isfinite(ru) && isfinite(rv) && u1 >= u0 && v1 >= v0) {
+            const double k2 = -0.72134752044448170368;           // -log2(e)/2
+            r.A = (float)(k2 * o.P[2] / o.dp); r.B = (float)(-k2 * o.P[1] / o.dp); r.C = (float)(k2 * o.P[0] / o.dp);
+            r.amp = (float)(rh * o.amp_over_rho);
+            double ci = rint(o.cu), cj = rint(o.cv);
+            if (ci > 30000.0) ci = 30000.0; if (ci < -30000.0) ci = -30000.0;
+            if (cj > 30000.0) cj = 30000.0; if (cj < -30000.0) cj = -30000.0;
+            r.ciu = (int16_t)ci; r.civ = (int16_t)cj; r.cfu = (float)(o.cu - ci); r.cfv = (float)(o.cv - cj);
+            r.u0 = (int16_t)u0; r.v0 = (int16_t)v0; r.u1 = (int16_t)u1; r.v1 = (int16_t)v1;
+            const int tx0 = r.u0 / kSplatTile, tx1 = r.u1 / kSplatTile, ty0 = r.v0 / kSplatTile, ty1 = r.v1 / kSplatTile;
+            for (int ty = ty0; ty <= ty1; ++ty)
+                for (int tx = tx0; tx <= tx1; ++tx)
+                    atomicAdd(&bin_count[(b * P.nty + ty) * P.ntx + tx], 1u);
+            atomicAdd(&status->pairs, (unsigned long long)((u1 - u0 + 1.0) * (v1 - v0 + 1.0)));
+        }
+    } else if (b == 0) {
+        atomicAdd(&status->skipped, 1u);
+    }
+    rec[idx] = r;
+}
+
+// s2: scatter.  keys[slot] = angle * n + Gaussian.
+__global__ void __launch_bounds__(128)
+k_splat_scatter(SplatParams P, const Splat2D* __restrict__ rec, uint32_t* __restrict__ cursor, uint32_t* __restrict__ keys,
+                const SplatStatus* __restrict__ status)
+{
+    if (status->overflow) return;
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)P.n * P.B) return;
+    const int b = (int)(idx / P.n);
+    const Splat2D r = rec[idx];
+    if (r.u1 < r.u0) return;
+    const int tx0 = r.u0 / kSplatTile, tx1 = r.u1 / kSplatTile, ty0 = r.v0 / kSplatTile, ty1 = r.v1 / kSplatTile;
+    for (int ty = ty0; ty <= ty1; ++ty)
+        for (int tx = tx0; tx <= tx1; ++tx)
+            keys[atomicAdd(&cursor[(b * P.nty + ty) * P.ntx + tx], 1u)] = (uint32_t)idx;
+}
+
+__device__ __forceinline__ float ex2s(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// s3: one CTA (16 x 16 threads) per (tile, angle); thread = pixel; keys staged 64 at a time.
+__global__ void __launch_bounds__(256)
+k_splat_forward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* __restrict__ bin_start,
+                const uint32_t* __restrict__ keys, const SplatStatus* __restrict__ status, float* __restrict__ drr)
+{
+    __shared__ __align__(16) Splat2D s_rec[kSplatBatch];
+    const int tid = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
+    const int tx = tile % P.ntx, ty = tile / P.ntx;
+    const int px = tx * kSplatTile + (tid & 15), py = ty * kSplatTile + (tid >> 4);
+    uint32_t kbeg = 0, kend = 0;
+    if (!status->overflow) { kbeg = bin_start[b * P.ntx * P.nty + tile]; kend = bin_start[b * P.ntx * P.nty + tile + 1]; }
+    float acc = 0.f;
+    for (uint32_t base = kbeg; base < kend; base += kSplatBatch) {
+        const int nb = (int)min((uint32_t)kSplatBatch, kend - base);
+        __syncthreads();
+        if (tid < nb * 3) {                                    // three 16-byte pieces per record
+            const int j = tid / 3, part = tid - 3 * j;
+            reinterpret_cast<float4*>(s_rec + j)[part] = __ldg(reinterpret_cast<const float4*>(rec + keys[base + j]) + part);
+        }
+        __syncthreads();
+        #pragma unroll 4
+        for (int j = 0; j < nb; ++j) {
+            const Splat2D r = s_rec[j];
+            const bool inside = px >= r.u0 && px <= r.u1 && py >= r.v0 && py <= r.v1;
+            const float dx = (float)(px - r.ciu) - r.cfu, dy = (float)(py - r.civ) - r.cfv;
+            const float e = fmaf(r.A * dx, dx, fmaf(2.f * r.B * dx, dy, r.C * dy * dy));
+            acc += inside ? r.amp * ex2s(e) : 0.f;
+        }
+    }
+    if (px < P.nu && py < P.nv) drr[((size_t)b * P.nv + py) * P.nu + px] = acc;
+}
+
+// s4: one CTA (128 threads) per (tile, angle); the tile's upstream gradient in shared memory; ONE
+// THREAD PER KEY walks box ∩ tile and reduces the six raw moments of g E about the centre in
+// registers:  m = sum g E {1, dx, dy, dx^2, dx dy, dy^2};  one vector atomic set per key.
+__global__ void __launch_bounds__(128)
+k_splat_backward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* __restrict__ bin_start,
+                 const uint32_t* __restrict__ keys, const SplatStatus* __restrict__ status,
+                 const float* __restrict__ gdrr, float* __restrict__ acc)
+{
+    __shared__ float s_g[kSplatTile * kSplatTile];
+    if (status->overflow) return;
+    const int tid = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
+    const uint32_t kbeg = bin_start[b * P.ntx * P.nty + tile], kend = bin_start[b * P.ntx * P.nty + tile + 1];
+    if (kbeg == kend) return;
+    const int tx = tile % P.ntx, ty = tile / P.ntx;
+    const int ox = tx * kSplatTile, oy = ty * kSplatTile;
+    for (int e = tid; e < kSplatTile * kSplatTile; e += 128) {
+        const int px = ox + (e & 15), py = oy + (e >> 4);
+        s_g[e] = (px < P.nu && py < P.nv) ? __ldg(gdrr + ((size_t)b * P.nv + py) * P.nu + px) : 0.f;
+    }
+    __syncthreads();
+    for (uint32_t k = kbeg + tid; k < kend; k += 128) {
+        const uint32_t id = keys[k];
+        const float4* rp = reinterpret_cast<const float4*>(rec + id);
+        const float4 a = __ldg(rp), c = __ldg(rp + 1);
+        const int4 w = __ldg(reinterpret_cast<const int4*>(rp + 2));
+        const float cfu = a.x, cfv = a.y, A = a.z, Bc = a.w, C = c.x;                 // c.y = amp (applied in s5)
+        const int ciu = (int16_t)(__float_as_int(c.z) & 0xffff), civ = (int16_t)(__float_as_int(c.z) >> 16);
+        const int u0 = (int16_t)(__float_as_int(c.w) & 0xffff), v0 = (int16_t)(__float_as_int(c.w) >> 16);
+        const int u1 = (int16_t)(w.x & 0xffff), v1 = (int16_t)(w.x >> 16);
+        const int x0 = max(u0 - ox, 0), x1 = min(u1 - ox, kSplatTile - 1), y0 = max(v0 - oy, 0), y1 = min(v1 - oy, kSplatTile - 1);
+        float m0 = 0.f, mx = 0.f, my = 0.f, mxx = 0.f, mxy = 0.f, myy = 0.f;
+        for (int y = y0; y <= y1; ++y) {
+            const float dy = (float)(oy + y - civ) - cfv;
+            const float cy = C * dy * dy, by = 2.f * Bc * dy;
+            float r0 = 0.f, r1 = 0.f, r2 = 0.f;                   // row sums of g E {1, dx, dx^2}
+            for (int x = x0; x <= x1; ++x) {
+                const float dx = (float)(ox + x - ciu) - cfu;
+                const float gE = s_g[y * kSplatTile + x] * ex2s(fmaf(A * dx, dx, fmaf(by, dx, cy)));
+                r0 += gE; const float t = gE * dx; r1 += t; r2 = fmaf(t, dx, r2);
+            }
+            m0 += r0; mx += r1; mxx += r2;
+            my = fmaf(dy, r0, my); mxy = fmaf(dy, r1, mxy); myy = fmaf(dy * dy, r0, myy);
+        }
+        float* dst = acc + (size_t)id * 8;
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" :: "l"(dst), "f"(m0), "f"(mx), "f"(my), "f"(mxx) : "memory");
+        asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" :: "l"(dst + 4), "f"(mxy), "f"(myy) : "memory");
+    }
+}
+
+// s5: chain rule, one thread per Gaussian, fp64, summed over the angles in a loop (no atomics).
+// Upstream per (angle, Gaussian): the raw moments m = sum g E {1, dx, dy, dx^2, dx dy, dy^2} of s4.
+//   value = amp E,  E = exp(-1/2 q),  q = A dx^2 + 2 B dx dy + C dy^2,  dx = iu - cu,  [A B; B C] = P^-1
+//   dL/damp = m0;  dL/dA = -amp mxx / 2;  dL/dB = -amp mxy;  dL/dC = -amp myy / 2
+//   dL/dcu = amp (A mx + B my);  dL/dcv = amp (B mx + C my)
+// then back through P = K Sigma^ K, amp = rho sqrt(2 pi |Sigma~| / |Sigma^|), Sigma~ = T Sigma T^T,
+// T = J(t) W, t = W (p - source), Sigma = R S^2 R^T, R(q / |q|).
+__global__ void __launch_bounds__(128)
+k_splat_epilogue(SplatParams P, const float* __restrict__ pos, const float* __restrict__ scale, const float* __restrict__ quat,
+                 const float* __restrict__ rho, const Splat2D* __restrict__ rec, const float* __restrict__ acc,
+                 const SplatStatus* __restrict__ status,
+                 float* __restrict__ grho, float* __restrict__ gpos, float* __restrict__ gscale, float* __restrict__ gquat)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= P.n) return;
+    double d_rho = 0.0, d_p[3] = { 0, 0, 0 }, d_Sig[9] = { 0, 0, 0, 0, 0, 0, 0, 0, 0 };
+    const double rh = (double)rho[g];
+    SplatTerms o;
+    o.valid = false;
+    for (int b = 0; b < P.B && !status->overflow; ++b) {
+        const size_t idx = (size_t)b * P.n + g;
+        if (rec[idx].u1 < rec[idx].u0) continue;               // skipped or off the detector at this angle
+        splat_terms(P, b, pos, scale, quat, g, o);
+        if (!o.valid) continue;
+        const float* m = acc + idx * 8;
+        const double m0 = m[0], mx = m[1], my = m[2], mxx = m[3], mxy = m[4], myy = m[5];
+        const double amp = rh * o.amp_over_rho;
+        const double A = o.P[2] / o.dp, Bc = -o.P[1] / o.dp, C = o.P[0] / o.dp;
+        const double g_amp = m0, gA = -0.5 * amp * mxx, gB = -amp * mxy, gC = -0.5 * amp * myy;
+        const double g_cu = amp * (A * mx + Bc * my), g_cv = amp * (Bc * mx + C * my);
+        d_rho += g_amp * o.amp_over_rho;
+        // conic -> P:  GP = -Pinv Gc Pinv,  Gc = [[gA, gB/2], [gB/2, gC]]
+        const double c00 = gA, c01 = 0.5 * gB, c11 = gC;
+        const double x00 = A * c00 + Bc * c01, x01 = A * c01 + Bc * c11, x10 = Bc * c00 + C * c01, x11 = Bc * c01 + C * c11;
+        const double GP00 = -(x00 * A + x01 * Bc), GP01 = -(x00 * Bc + x01 * C), GP11 = -(x10 * Bc + x11 * C);
+        const double ku = P.sdd / P.du, kv = P.sdd / P.dv;
+        double GS[9] = { 0, 0, 0, 0, 0, 0, 0, 0, 0 };           // symmetric matrix gradient wrt Sigma~
+        GS[0] = GP00 * ku * ku; GS[4] = GP11 * kv * kv; GS[1] = GS[3] = GP01 * ku * kv;
+        // amplitude: amp = rho sqrt(2 pi det_t / det_h)
+        const double g_dett = g_amp * amp / (2.0 * o.det_t), g_deth = -g_amp * amp / (2.0 * o.det_h);
+        const double* S = o.St;
+        GS[0] += g_deth * S[4]; GS[4] += g_deth * S[0]; GS[1] -= g_deth * S[1]; GS[3] -= g_deth * S[1];
+        // d det_t = adj(Sigma~) : d Sigma~   (adjugate = cofactors, Sigma~ symmetric)
+        const double adj[9] = { S[4] * S[8] - S[5] * S[7], S[2] * S[7] - S[1] * S[8], S[1] * S[5] - S[2] * S[4],
+                                S[5] * S[6] - S[3] * S[8], S[0] * S[8] - S[2] * S[6], S[2] * S[3] - S[0] * S[5],
+                                S[3] * S[7] - S[4] * S[6], S[1] * S[6] - S[0] * S[7], S[0] * S[4] - S[1] * S[3] };
+        for (int k = 0; k < 9; ++k) GS[k] += g_dett * adj[k];
+        // Sigma~ = T Sigma T^T:  dL/dSigma += T^T GS T;  dL/dT = 2 GS T Sigma
+        double Tt[9], GT[9], tmp[9], tmp2[9];
+        for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) Tt[3 * i + j] = o.T[3 * j + i];
+        mat3mul(Tt, GS, tmp); mat3mul(tmp, o.T, tmp2);
+        for (int k = 0; k < 9; ++k) d_Sig[k] += tmp2[k];
+        mat3mul(GS, o.T, tmp); mat3mul(tmp, o.Sig, GT);
+        for (int k = 0; k < 9; ++k) GT[k] *= 2.0;
+        // T = J W:  dL/dJ = dL/dT W^T
+        double W[9], src[3], Wt[9], GJ[9];
+        splat_W(P, b, W, src);
+        for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) Wt[3 * i + j] = W[3 * j + i];
+        mat3mul(GT, Wt, GJ);
+        // J(t) and the centre (cu, cv) -> t
+        const double t0 = o.t[0], t1 = o.t[1], t2 = o.t[2], l = o.ell, l3 = l * l * l, it2 = 1.0 / (t2 * t2), it3 = it2 / t2;
+        double gt[3];
+        gt[0] = -GJ[2] * it2 + GJ[6] * (1.0 / l - t0 * t0 / l3) - GJ[7] * t0 * t1 / l3 - GJ[8] * t0 * t2 / l3 + g_cu * ku / t2;
+        gt[1] = -GJ[5] * it2 - GJ[6] * t0 * t1 / l3 + GJ[7] * (1.0 / l - t1 * t1 / l3) - GJ[8] * t1 * t2 / l3 + g_cv * kv / t2;
+        gt[2] = -(GJ[0] + GJ[4]) * it2 + 2.0 * (GJ[2] * t0 + GJ[5] * t1) * it3 - (GJ[6] * t0 + GJ[7] * t1) * t2 / l3
+              + GJ[8] * (1.0 / l - t2 * t2 / l3) - (g_cu * ku * t0 + g_cv * kv * t1) * it2;
+        for (int k = 0; k < 3; ++k) d_p[k] += W[k] * gt[0] + W[3 + k] * gt[1] + W[6 + k] * gt[2];   // W^T gt
+    }
+    grho[g] = (float)d_rho;
+    for (int k = 0; k < 3; ++k) gpos[3 * g + k] = (float)d_p[k];
+    // Sigma = R S^2 R^T  (R, s from the parameters; independent of the angle)
+    const double s[3] = { scale[3 * g], scale[3 * g + 1], scale[3 * g + 2] };
+    const double q[4] = { quat[4 * g], quat[4 * g + 1], quat[4 * g + 2], quat[4 * g + 3] };
+    const double n2 = q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3];
+    bool bad = !(n2 > 0.0) || !isfinite(n2);
+    for (int k = 0; k < 3; ++k) bad |= !(s[k] > 0.0) || !isfinite(s[k]);
+    if (bad) {
+        for (int k = 0; k < 3; ++k) gscale[3 * g + k] = 0.f;
+        for (int k = 0; k < 4; ++k) gquat[4 * g + k] = 0.f;
+        return;
+    }
+    const double qn = sqrt(n2), r = q[0] / qn, x = q[1] / qn, y = q[2] / qn, z = q[3] / qn;
+    const double R[9] = { 1 - 2 * (y * y + z * z), 2 * (x * y - r * z), 2 * (x * z + r * y),
+                          2 * (x * y + r * z), 1 - 2 * (x * x + z * z), 2 * (y * z - r * x),
+                          2 * (x * z - r * y), 2 * (y * z + r * x), 1 - 2 * (x * x + y * y) };
+    // dL/ds_k = 2 s_k (R^T G R)_kk;  D_R = 2 G R S^2   (G = d_Sig, symmetric)
+    double GR[9], DR[9];
+    mat3mul(d_Sig, R, GR);
+    for (int k = 0; k < 3; ++k) {
+        const double d = R[k] * GR[k] + R[3 + k] * GR[3 + k] + R[6 + k] * GR[6 + k];
+        gscale[3 * g + k] = (float)(2.0 * s[k] * d);
+    }
+    for (int i = 0; i < 3; ++i) for (int k = 0; k < 3; ++k) DR[3 * i + k] = 2.0 * GR[3 * i + k] * s[k] * s[k];
+    double gh[4];
+    gh[0] = 2 * (-z * DR[1] + y * DR[2] + z * DR[3] - x * DR[5] - y * DR[6] + x * DR[7]);
+    gh[1] = 2 * (y * DR[1] + z * DR[2] + y * DR[3] - 2 * x * DR[4] - r * DR[5] + z * DR[6] + r * DR[7] - 2 * x * DR[8]);
+    gh[2] = 2 * (-2 * y * DR[0] + x * DR[1] + r * DR[2] + x * DR[3] + z * DR[5] - r * DR[6] + z * DR[7] - 2 * y * DR[8]);
+    gh[3] = 2 * (-2 * z * DR[0] - r * DR[1] + x * DR[2] + r * DR[3] - 2 * z * DR[4] + y * DR[5] + x * DR[6] + y * DR[7]);
+    const double qh[4] = { r, x, y, z };
+    const double dot = qh[0] * gh[0] + qh[1] * gh[1] + qh[2] * gh[2] + qh[3] * gh[3];
+    for (int k = 0; k < 4; ++k) gquat[4 * g + k] = (float)((gh[k] - qh[k] * dot) / qn);
+}
+
+}  // namespace gsvox
+
+using namespace gsvox;
+
+static size_t sup256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+static int splat_setup(int64_t n, const gsvox_cone_geometry* c, const float* angles_host, int32_t B,
+                       int64_t key_capacity, void* workspace, size_t workspace_bytes, SplatParams* P, SplatWs* ws)
+{
+    if (!c || n < 0 || B < 1 || B > kSplatMaxBatch || key_capacity < 0) return GSVOX_EINVAL;
+    if (!(c->sad > 0.f) || !(c->sdd > 0.f) || c->nu < 1 || c->nv < 1 || !(c->du > 0.f) || !(c->dv > 0.f)) return GSVOX_EINVAL;
+    if (c->nu > GSVOX_MAX_DIM || c->nv > GSVOX_MAX_DIM || n * (int64_t)B > 0x7ffffff0LL || key_capacity > 0xfffffff0LL) return GSVOX_ELIMIT;
+    P->n = (int)n; P->B = B; P->nu = c->nu; P->nv = c->nv;
+    P->ntx = (c->nu + kSplatTile - 1) / kSplatTile; P->nty = (c->nv + kSplatTile - 1) / kSplatTile;
+    P->sad = c->sad; P->sdd = c->sdd; P->du = c->du; P->dv = c->dv; P->off_u = c->off_u; P->off_v = c->off_v;
+    for (int k = 0; k < 3; ++k) P->iso[k] = c->iso[k];
+    if (angles_host) for (int b = 0; b < B; ++b) { P->ca[b] = cos((double)angles_host[b]); P->sa[b] = sin((double)angles_host[b]); }
+    const long long nbins = (long long)P->ntx * P->nty * B;
+    if (nbins > 0x7ffffff0LL || P->ntx * (long long)P->nty > 0x7fffffffLL) return GSVOX_ELIMIT;
+    ws->nbins = (int)nbins;
+    size_t off = 0;
+    char* w = (char*)workspace;
+    ws->status = (SplatStatus*)(w + off);  off += sup256(sizeof(SplatStatus));      // status and bin_count contiguous: one memset
+    ws->bin_count = (uint32_t*)(w + off);  off += sup256(sizeof(uint32_t) * (size_t)(nbins + 1));
+    ws->bin_start = (uint32_t*)(w + off);  off += sup256(sizeof(uint32_t) * (size_t)(nbins + 1));
+    ws->partial = (uint32_t*)(w + off);    off += sup256(sizeof(uint32_t) * (size_t)((nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock + 1));
+    ws->rec = (Splat2D*)(w + off);         off += sup256(sizeof(Splat2D) * (size_t)n * B);
+    ws->keys = (uint32_t*)(w + off);       off += sup256(sizeof(uint32_t) * (size_t)key_capacity);
+    ws->acc = (float*)(w + off);           off += sup256(sizeof(float) * 8 * (size_t)n * B);
+    ws->total = off;
+    if (workspace && (((uintptr_t)workspace & 255) || workspace_bytes < off)) return GSVOX_EWORKSPACE;
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_splat_workspace_bytes(int64_t n, const gsvox_cone_geometry* geom, int32_t B,
+                                           int64_t key_capacity, size_t* bytes)
+{
+    if (!bytes) return GSVOX_EINVAL;
+    SplatParams P; SplatWs ws;
+    int rc = splat_setup(n, geom, nullptr, B, key_capacity, nullptr, 0, &P, &ws);
+    if (rc == GSVOX_OK) *bytes = ws.total;
+    return rc;
+}
+
+extern "C" int gsvox_splat_forward(const float* pos, const float* scale, const float* quat, const float* rho,
+                                   int64_t n, const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                                   void* workspace, size_t workspace_bytes, int64_t key_capacity,
+                                   float* drr, void* stream)
+{
+    if (!workspace || !angles_host || !drr) return GSVOX_EINVAL;
+    if (n > 0 && (!pos || !scale || !quat || !rho)) return GSVOX_EINVAL;
+    SplatParams P; SplatWs ws;
+    int rc = splat_setup(n, geom, angles_host, B, key_capacity, workspace, workspace_bytes, &P, &ws);
+    if (rc != GSVOX_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    GSVOX_CUDA(cudaMemsetAsync(ws.status, 0, (size_t)((char*)ws.bin_count - (char*)ws.status) + sizeof(uint32_t) * (size_t)(ws.nbins + 1), st));
+    const long long items = (long long)n * B;
+    if (items > 0) {
+        k_splat_pre<<<(unsigned)((items + 127) / 128), 128, 0, st>>>(P, pos, scale, quat, rho, ws.rec, ws.bin_count, ws.status);
+        GSVOX_CUDA(cudaGetLastError());
+    }
+    rc = launch_exclusive_scan(ws.bin_count, ws.nbins, ws.partial, ws.bin_start, &ws.status->keys_needed,
+                               &ws.status->overflow, (unsigned long long)key_capacity, st);
+    if (rc != GSVOX_OK) return rc;
+    if (items > 0) {
+        k_splat_scatter<<<(unsigned)((items + 127) / 128), 128, 0, st>>>(P, ws.rec, ws.bin_count, ws.keys, ws.status);
+        GSVOX_CUDA(cudaGetLastError());
+    }
+    dim3 grid((unsigned)(P.ntx * P.nty), (unsigned)B);
+    k_splat_forward<<<grid, 256, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, drr);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_splat_backward(const float* pos, const float* scale, const float* quat, const float* rho,
+                                    int64_t n, const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                                    void* workspace, size_t workspace_bytes, int64_t key_capacity,
+                                    const float* grad_drr, float* grad_rho, float* grad_pos, float* grad_scale,
+                                    float* grad_quat, void* stream)
+{
+    if (!workspace || !angles_host || !grad_drr) return GSVOX_EINVAL;
+    if (n > 0 && (!pos || !scale || !quat || !rho || !grad_rho || !grad_pos || !grad_scale || !grad_quat)) return GSVOX_EINVAL;
+    SplatParams P; SplatWs ws;
+    int rc = splat_setup(n, geom, angles_host, B, key_capacity, workspace, workspace_bytes, &P, &ws);
+    if (rc != GSVOX_OK) return rc;
+    if (n == 0) return GSVOX_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    GSVOX_CUDA(cudaMemsetAsync(ws.acc, 0, sizeof(float) * 8 * (size_t)n * B, st));
+    dim3 grid((unsigned)(P.ntx * P.nty), (unsigned)B);
+    k_splat_backward<<<grid, 128, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, grad_drr, ws.acc);
+    GSVOX_CUDA(cudaGetLastError());
+    k_splat_epilogue<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(P, pos, scale, quat, rho, ws.rec, ws.acc, ws.status,
+                                                                 grad_rho, grad_pos, grad_scale, grad_quat);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_splat_status(const void* workspace, int64_t* keys_needed, int64_t* pairs, int32_t* overflow,
+                                  int32_t* skipped, void* stream)
+{
+    if (!workspace) return GSVOX_EINVAL;
+    SplatStatus h;
+    cudaStream_t st = (cudaStream_t)stream;
+    GSVOX_CUDA(cudaMemcpyAsync(&h, workspace, sizeof h, cudaMemcpyDeviceToHost, st));
+    GSVOX_CUDA(cudaStreamSynchronize(st));
+    if (keys_needed) *keys_needed = (int64_t)h.keys_needed;
+    if (pairs) *pairs = (int64_t)h.pairs;
+    if (overflow) *overflow = (int32_t)h.overflow;
+    if (skipped) *skipped = (int32_t)h.skipped;
+    return GSVOX_OK;
+}

@@ -1,0 +1,150 @@
+"""GPU parity of the Gaussian-splat X-ray rasterizer (gsvox_splat_forward / gsvox_splat_backward;
+SURVEY.md 8(f) rank 3; Eq. 6-9) against oracle/splat.py (torch fp64, autograd backward).
+Forward max|err| <= 1e-5 max|drr| + 1e-6; gradients relative L2 <= 1e-4 per group (rho, pos, scale,
+quat); pair and key counts exact.  `-m gpu`, B200.
+"""
+import numpy as np
+import pytest
+
+import gsvox_inputs
+import oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+FWD_REL, FWD_ABS, GRAD_REL = 1e-5, 1e-6, 1e-4
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2503_22139_b200 as p
+    p.lib()
+    torch.cuda.set_device(0)
+    return p
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rel_l2(a, b):
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a.astype(np.float64) - b) / nb if nb > 0 else float(np.abs(a).max())
+
+
+def run_gpu(pkg, case, grad=None, key_capacity=None):
+    sp = pkg.Splatter(max(case.n, 1), case.geom, case.batch, key_capacity=key_capacity)
+    args = (dev(case.pos), dev(case.scale), dev(case.quat), dev(case.rho))
+    drr = sp.forward(*args, list(case.angles))
+    st = sp.status()
+    if st["overflow"] and key_capacity is None:
+        sp = pkg.Splatter(max(case.n, 1), case.geom, case.batch, key_capacity=st["keys_needed"])
+        drr = sp.forward(*args, list(case.angles))
+        st = sp.status()
+    grads = None
+    if grad is not None:
+        grads = [t.cpu().numpy() for t in sp.backward(*args, list(case.angles), dev(grad))]
+    torch.cuda.synchronize()
+    return drr.cpu().numpy(), grads, st
+
+
+def parity(pkg, case, backward=True):
+    g = case.grad_drr() if backward else None
+    drr, grads, st = run_gpu(pkg, case, grad=g)
+    assert not st["overflow"]
+    ref, pairs = oracle.splat_forward(case.pos, case.scale, case.quat, case.rho, case.geom, case.angles, return_pairs=True)
+    assert st["pairs"] == pairs, (st, pairs)
+    err = np.abs(drr - ref).max()
+    tol = FWD_REL * np.abs(ref).max() + FWD_ABS
+    assert err <= tol, "splat forward max|err| %.3e > tol %.3e" % (err, tol)
+    rels = {}
+    if backward:
+        refs = oracle.splat_backward(case.pos, case.scale, case.quat, case.rho, case.geom, case.angles, g)
+        for name, a, b in zip(("rho", "pos", "scale", "quat"), grads, refs):
+            rels[name] = rel_l2(a.reshape(b.shape), b)
+            assert rels[name] <= GRAD_REL, "splat grad %s rel L2 %.3e" % (name, rels[name])
+    return err / tol, rels
+
+
+def test_splat_small_all_octants_half_fan(pkg):
+    angles = [0.0, 0.6, 1.3, 2.2, 3.0, 3.9, 4.6, 5.7]
+    parity(pkg, gsvox_inputs.splat_case(n=300, batch=8, extent=(120.0, 120.0, 60.0), nu=90, nv=70, du=2.0, dv=2.5,
+                                        sad=300.0, sdd=450.0, off_u=11.0, off_v=-6.0, seed=61, angles=angles))
+
+
+def test_splat_narrow_and_wide_gaussians(pkg):
+    """Sub-pixel footprints next to footprints wider than the detector."""
+    parity(pkg, gsvox_inputs.splat_case(n=200, batch=3, extent=(100.0, 100.0, 60.0), nu=64, nv=48, du=2.0, dv=2.0,
+                                        sad=300.0, sdd=450.0, seed=62, scales=(0.15, 40.0)))
+
+
+def test_splat_degenerate_and_behind_the_source(pkg):
+    case = gsvox_inputs.splat_case(n=64, batch=2, extent=(100.0, 100.0, 60.0), nu=48, nv=40, du=3.0, dv=3.0,
+                                   sad=300.0, sdd=450.0, seed=63, angles=[0.0, 2.0])
+    case.pos[0] = (400.0, 0.0, 0.0)          # behind the source at angle 0 only
+    case.scale[1, 2] = 0.0; case.quat[2] = 0.0; case.pos[3, 1] = np.nan; case.scale[4, 0] = -1.0
+    case.pos[5] = (0.0, 0.0, 5000.0)         # far off the detector
+    drr, grads, st = run_gpu(pkg, case, grad=case.grad_drr())
+    keep = np.ones(case.n, bool); keep[1:5] = False
+    sub = lambda a: np.ascontiguousarray(a[keep])
+    ref = oracle.splat_forward(sub(case.pos), sub(case.scale), sub(case.quat), sub(case.rho), case.geom, case.angles)
+    assert np.isfinite(drr).all() and np.abs(drr - ref).max() <= FWD_REL * np.abs(ref).max() + FWD_ABS
+    refs = oracle.splat_backward(sub(case.pos), sub(case.scale), sub(case.quat), sub(case.rho), case.geom, case.angles,
+                                 case.grad_drr())
+    for a, b in zip(grads, refs):
+        a = a.reshape(case.n, -1)
+        assert np.all(a[1:5] == 0.0) and np.isfinite(a).all()
+        assert rel_l2(a[keep].reshape(b.shape), b) <= GRAD_REL
+    assert np.all(grads[1].reshape(case.n, 3)[5] == 0.0)
+
+
+def test_splat_key_overflow_is_reported_and_output_is_zero(pkg):
+    case = gsvox_inputs.splat_case(n=500, batch=2, extent=(120.0, 120.0, 60.0), nu=96, nv=64, du=2.0, dv=2.0,
+                                   sad=300.0, sdd=450.0, seed=64)
+    drr, _, st = run_gpu(pkg, case, key_capacity=64)
+    assert st["overflow"] and st["keys_needed"] > 64 and np.all(drr == 0.0)
+
+
+def test_splat_zero_gaussians(pkg):
+    case = gsvox_inputs.splat_case(n=4, batch=1, nu=32, nv=32, seed=65)
+    sp = pkg.Splatter(4, case.geom, 1)
+    z = lambda k: torch.zeros((0, k), device="cuda")
+    out = torch.full((1, 32, 32), 5.0, device="cuda")
+    sp.forward(z(3), z(3), z(4), torch.zeros(0, device="cuda"), list(case.angles), out=out)
+    assert float(out.abs().max()) == 0.0
+
+
+def test_splat_medium_config2_like(pkg):
+    parity(pkg, gsvox_inputs.splat_case(n=2000, batch=3, nu=256, nv=192, du=1.552, dv=1.552, seed=66))
+
+
+def test_splat_full_size_sampled_pixels(pkg):
+    """50 000 Gaussians on the Table I detector, 8 angles (the size bench times): the oracle evaluates
+    1000 sampled pixels per angle, and the gradients of the loss restricted to those pixels."""
+    case = gsvox_inputs.splat_case()
+    rng = np.random.default_rng(67)
+    pix = [(b, int(rng.integers(0, case.geom["nu"])), int(rng.integers(0, case.geom["nv"])))
+           for b in range(case.batch) for _ in range(1000)]
+    g = np.zeros((case.batch, case.geom["nv"], case.geom["nu"]), np.float32)
+    vals = rng.standard_normal(len(pix)).astype(np.float32)
+    for (b, iu, iv), v in zip(pix, vals):
+        g[b, iv, iu] = v
+    pix = sorted(set(pix))
+    drr, grads, st = run_gpu(pkg, case, grad=g)
+    assert not st["overflow"]
+    worst, peak = 0.0, 0.0
+    for b in range(case.batch):
+        sel = [(iu, iv) for (bb, iu, iv) in pix if bb == b]
+        ref = oracle.splat_forward_at(case.pos, case.scale, case.quat, case.rho, case.geom, case.angles[b], sel)
+        got = np.array([drr[b, iv, iu] for (iu, iv) in sel])
+        worst = max(worst, float(np.abs(got - ref).max())); peak = max(peak, float(np.abs(ref).max()))
+    assert worst <= FWD_REL * peak + FWD_ABS, (worst, peak)
+    refs = oracle.splat_backward(case.pos, case.scale, case.quat, case.rho, case.geom, case.angles, g, pixels=pix)
+    rels = {}
+    for name, a, b in zip(("rho", "pos", "scale", "quat"), grads, refs):
+        rels[name] = rel_l2(a.reshape(b.shape), b)
+        assert rels[name] <= GRAD_REL, (name, rels[name])
+    print("splat full size: forward err/tol %.3f, grads %s, pairs %.3e keys %.3e" %
+          (worst / (FWD_REL * peak + FWD_ABS), rels, st["pairs"], st["keys_needed"]))
