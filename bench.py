@@ -289,6 +289,37 @@ def next_rows(torch, pkg, hbm_peak_gbs, quick=False):
                     "frac_of_hbm_peak": bf / mf / 1e6 / hbm_peak_gbs,
                     "note": "L1/L2-bound gather: 4 corner reads per sample, volumes (16 MB each) L2-resident"},
         "backward": {"ms": mb, "samples_per_s": samples / (mb * 1e-3), "note": "4 fp32 atomics per sample"}}
+    del vol, gdrr, drr, gv, scratch
+    # ---- rank 3: Gaussian-splat X-ray rasterizer, 50 000 Gaussians at 8 gantry angles (Stage 1)
+    sc = gsvox_inputs.splat_case()
+    sp = pkg.Splatter(sc.n, sc.geom, sc.batch)
+    sargs = (dev(sc.pos), dev(sc.scale), dev(sc.quat), dev(sc.rho))
+    sang = list(sc.angles)
+    sdrr = sp.forward(*sargs, sang)
+    sst = sp.status()
+    if sst["overflow"]:
+        sp = pkg.Splatter(sc.n, sc.geom, sc.batch, key_capacity=int(1.05 * sst["keys_needed"]))
+        sdrr = sp.forward(*sargs, sang)
+        sst = sp.status()
+    sg = dev(sc.grad_drr())
+    sgr = [None]
+
+    def splat_fb():
+        sp.forward(*sargs, sang, out=sdrr)
+        sgr[0] = sp.backward(*sargs, sang, sg, grads=sgr[0])
+    mf = _time_ms(torch, lambda: sp.forward(*sargs, sang, out=sdrr), 20)
+    mfb = _time_ms(torch, splat_fb, 20)
+    # canonical flops per (Gaussian, pixel) pair: forward dx,dy (2) + quadratic form (3 mul + 2 fma = 7... counted 8)
+    # + ex2 (1) + amp*E + accumulate (2) = 13; backward recompute (11) + g E (1) + six moments (11) = 23
+    res["splat_50k_512x384_b8"] = {
+        "pairs_P_def": sst["pairs"], "keys": sst["keys_needed"],
+        "forward": {"ms": mf, "pairs_per_s": sst["pairs"] / (mf * 1e-3),
+                    "canonical_tflops": 13 * sst["pairs"] / (mf * 1e-3) / 1e12,
+                    "frac_of_fp32_peak": 13 * sst["pairs"] / (mf * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
+                    "note": "includes the per-(angle, Gaussian) preprocess and the tile binning"},
+        "forward_backward": {"ms": mfb, "pairs_per_s": sst["pairs"] / (mfb * 1e-3),
+                             "canonical_tflops": 36 * sst["pairs"] / (mfb * 1e-3) / 1e12,
+                             "frac_of_fp32_peak": 36 * sst["pairs"] / (mfb * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}}
     return res
 
 
