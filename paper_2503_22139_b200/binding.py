@@ -348,6 +348,32 @@ class Plan:
                                     _dev(gq, "grad_quat"), _stream()))
         return grads
 
+    # --- CUDA graph of one training step ----------------------------------------------
+    def capture_step(self, pos, scale, quat, weight, grad_out, out=None, grads=None):
+        """Capture gsvox_preprocess + gsvox_forward + gsvox_backward on the given (static) tensors into a
+        CUDA graph and return (graph, out, grads): graph.replay() re-runs the step on whatever the tensors
+        hold then.  The three calls never synchronise or allocate, so they are capturable as they are; for
+        launch-bound sizes (config 1: 11 launches for 20 us of work) the replay removes the launch gaps."""
+        ch = int(weight.shape[1])
+        nx, ny, nz = self.dims
+        n = int(pos.shape[0])
+        if out is None:
+            out = torch.empty((ch, nz, ny, nx), dtype=torch.float32, device=self.device)
+        if grads is None:
+            mk = lambda k: torch.empty((n, k), dtype=torch.float32, device=self.device)
+            grads = (mk(ch), mk(3), mk(3), mk(4))
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):                      # warm-up outside the capture (first-launch module loads)
+            self.preprocess(pos, scale, quat); self.forward(weight, out=out); self.backward(weight, grad_out, grads=grads)
+        torch.cuda.current_stream().wait_stream(side)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            self.preprocess(pos, scale, quat)
+            self.forward(weight, out=out)
+            self.backward(weight, grad_out, grads=grads)
+        return graph, out, grads
+
     # --- multi-GPU z-slabs (DESIGN.md section 8) --------------------------------------
     def set_slab(self, bz_begin, bz_end):
         _check(lib().gsvox_plan_set_slab(self._h, int(bz_begin), int(bz_end)))

@@ -311,3 +311,22 @@ def test_needle_keys_are_culled_only_when_negligible(pkg):
     st = plan.status()
     assert st["culled_keys"] > 2 * st["keys_needed"], st          # most of the boxes is empty space
     assert st["pairs_exec"] < 0.5 * st["pairs"]
+
+
+def test_cuda_graph_replay_matches_eager_and_follows_new_inputs(pkg):
+    """The three hot calls neither synchronise nor allocate, so one training step can be captured in a CUDA
+    graph; a replay after the parameters changed in place must give the new step's results."""
+    case = gsvox_inputs.config1()
+    plan = pkg.Plan(case.n, case.grid, max_channels=1)
+    pos, scale, quat, w, g = dev(case.pos), dev(case.scale), dev(case.quat), dev(case.weight), dev(case.grad_out())
+    graph, out, grads = plan.capture_step(pos, scale, quat, w, g)
+    graph.replay(); torch.cuda.synchronize()
+    ref = oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid)
+    check_forward(out.cpu().numpy(), ref)
+    pos2 = case.pos + np.float32(0.37)                       # new parameters, same buffers
+    pos.copy_(dev(pos2))
+    graph.replay(); torch.cuda.synchronize()
+    ref2 = oracle.forward(pos2, case.scale, case.quat, case.weight, case.grid)
+    check_forward(out.cpu().numpy(), ref2)
+    refs2 = oracle.backward(pos2, case.scale, case.quat, case.weight, case.grid, case.grad_out())
+    check_grads([t.cpu().numpy() for t in grads], refs2)
