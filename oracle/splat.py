@@ -15,8 +15,8 @@ rho^ = rho sqrt(2 pi |Sigma~| / |Sigma^|).  "phi, J and W are determined by scan
   R3 pixel (iu, iv) has ray-space coordinates x^ = (u/SDD, v/SDD), u = (iu - (nu-1)/2) du + off_u.
   R4 cutoff: the axis-aligned box of the 3-sigma ellipse on the detector, in pixels, inclusive,
      clipped to the detector, decided in fp64; nothing else is tested inside the box (as A3/A4).
-  R5 a Gaussian with t2 <= 0 (at or behind the source plane) or with degenerate parameters is
-     skipped.  R6 backward: supports frozen.
+  R5 a Gaussian with t2 <= 0 (at or behind the source plane), with degenerate parameters, or whose
+     centre projects more than 30000 pixels off the detector origin is skipped.  R6 backward: supports frozen.
 """
 import math
 
@@ -74,7 +74,8 @@ def splat_terms(pos, scale, quat, rho, geom, angle, kappa=KAPPA):
         v0 = torch.clamp(torch.ceil(cv - rv), min=0)
         v1 = torch.clamp(torch.floor(cv + rv), max=int(geom["nv"]) - 1)
         finite = torch.isfinite(cu) & torch.isfinite(cv) & torch.isfinite(ru) & torch.isfinite(rv) & (det_h > 0) & (det_t > 0)
-        valid = valid & finite & (u1 >= u0) & (v1 >= v0)
+        near = (cu.abs() <= 30000.0) & (cv.abs() <= 30000.0)          # R5: centres beyond +-30000 pixels are skipped
+        valid = valid & finite & near & (u1 >= u0) & (v1 >= v0)
         box = torch.stack([u0, v0, u1, v1], dim=1)
     return cu, cv, A, B, C, amp, box, valid
 
