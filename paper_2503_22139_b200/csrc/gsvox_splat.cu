@@ -35,6 +35,7 @@ struct __align__(16) Splat2D {
     float C, amp;
     int16_t ciu, civ;      // integer part of the centre (may be off the detector)
     int16_t u0, v0, u1, v1;   // inclusive pixel box; empty <=> u1 < u0
+    float Bq, Dq;          // row form of the exponent: E = A (dx + Bq dy)^2 + Dq dy^2, Bq = B/A, Dq = -log2(e)/2 / Sigma^_vv
     int32_t pad;
 };
 static_assert(sizeof(Splat2D) == 48, "Splat2D must be 48 bytes");
@@ -134,7 +135,7 @@ k_splat_pre(SplatParams P, const float* __restrict__ pos, const float* __restric
     unsigned long long my_pairs = 0ull;
     unsigned int my_skipped = 0u;
     Splat2D r;
-    r.cfu = r.cfv = r.A = r.B = r.C = r.amp = 0.f; r.ciu = r.civ = 0; r.u0 = r.v0 = 0; r.u1 = r.v1 = -1; r.pad = 0;
+    r.cfu = r.cfv = r.A = r.B = r.C = r.amp = 0.f; r.ciu = r.civ = 0; r.u0 = r.v0 = 0; r.u1 = r.v1 = -1; r.Bq = r.Dq = 0.f; r.pad = 0;
     SplatTerms o;
     o.valid = false;
     if (live) splat_terms(P, b, pos, scale, quat, g, o);
@@ -148,6 +149,7 @@ k_splat_pre(SplatParams P, const float* __restrict__ pos, const float* __restric
             const double k2 = -0.72134752044448170368;           // -log2(e)/2
             r.A = (float)(k2 * o.P[2] / o.dp); r.B = (float)(-k2 * o.P[1] / o.dp); r.C = (float)(k2 * o.P[0] / o.dp);
             r.amp = (float)(rh * o.amp_over_rho);
+            r.Bq = (float)(-o.P[1] / o.P[2]); r.Dq = (float)(k2 / o.P[2]);        // Schur complement: no cancellation
             const double ci = rint(o.cu), cj = rint(o.cv);       // |.| <= 30000 (R5): fits int16
             r.ciu = (int16_t)ci; r.civ = (int16_t)cj; r.cfu = (float)(o.cu - ci); r.cfv = (float)(o.cv - cj);
             r.u0 = (int16_t)u0; r.v0 = (int16_t)v0; r.u1 = (int16_t)u1; r.v1 = (int16_t)v1;
@@ -244,57 +246,111 @@ __device__ __forceinline__ float ex2s(float x)
     return y;
 }
 
-// s3: one CTA (16 x 16 threads) per (tile, angle); thread = pixel; keys staged 64 at a time as 32-byte
-// tile-local records: centre relative to the tile origin (|dx| stays small: no cancellation against
-// the pixel index), conic with 2B folded, amplitude, and the box as a 16-bit column mask and a 16-bit
-// row mask, so the cutoff test of a pixel is one AND + compare and a warp (two pixel rows) skips a key
-// whose box misses its rows.
-struct __align__(16) SplatTileRec { float cx, cy, A, B2, C, amp; uint32_t mask; uint32_t pad; };
+// s3: ONE WARP per (tile, angle); thread t owns the 8-pixel row segment (row t >> 1, columns 8 (t & 1) ..
+// + 7) in registers.  Along a row the exponent is a parabola in x, E(x) = A (x - xs)^2 + Es with
+// xs = cx - Bq dy, Es = Dq dy^2, so — as in a3 — the eight values come from a centre-out
+// multiplicative recurrence: 3 ex2 + 2 FMUL + 5 FMUL2 + 4 FFMA2 per 8 pixels instead of 8 ex2 and 8 x 7
+// flops (the per-pixel version of this kernel: 1.00 ms; this one: see DESIGN.md section 13).  Footprints
+// narrower than ~0.85 pixel along x (A < -1) take one ex2 per pixel.  Keys are staged 32 at a time as
+// 96-byte tile-local records: geometry, the row mask of box ∩ tile, and the amplitude times
+// [column inside the box] for the 16 columns in the packed-pair order of the recurrence.
+struct __align__(16) SplatTileRec {
+    float cx, cy, A, Bq;       // centre relative to the tile origin
+    float Dq, cc;              // cc = 2^(2A): ratio of successive ratios along x
+    uint32_t rowmask, direct;
+    float w[16];               // per segment: columns 3,4, 2,5, 1,6, 0,7 (+8 for the second segment)
+};
+static_assert(sizeof(SplatTileRec) == 96, "SplatTileRec must be 96 bytes");
 
-__global__ void __launch_bounds__(256)
+constexpr int kSplatFwdBatch = 32;
+
+__global__ void __launch_bounds__(32)
 k_splat_forward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* __restrict__ bin_start,
                 const uint32_t* __restrict__ keys, const SplatStatus* __restrict__ status, float* __restrict__ drr)
 {
-    __shared__ SplatTileRec s_rec[kSplatBatch];
-    const int tid = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
+    __shared__ SplatTileRec s_rec[kSplatFwdBatch];
+    const int lane = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
     const int tx = tile % P.ntx, ty = tile / P.ntx;
     const int ox = tx * kSplatTile, oy = ty * kSplatTile;
-    const int lx = tid & 15, ly = tid >> 4;
-    const float fx = (float)lx, fy = (float)ly;
-    const uint32_t mybits = (1u << lx) | (1u << (16 + ly));
-    const uint32_t warprows = 3u << (16 + 2 * (tid >> 5));           // the two pixel rows of this warp
+    const int row = lane >> 1, seg = lane & 1;
+    const float fy = (float)row, fx3 = (float)(8 * seg + 3);
+    const uint32_t rowbit = 1u << row;
     uint32_t kbeg = 0, kend = 0;
     if (!status->overflow) { kbeg = bin_start[b * P.ntx * P.nty + tile]; kend = bin_start[b * P.ntx * P.nty + tile + 1]; }
-    float acc = 0.f;
-    for (uint32_t base = kbeg; base < kend; base += kSplatBatch) {
-        const int nb = (int)min((uint32_t)kSplatBatch, kend - base);
-        __syncthreads();
-        if (tid < nb) {
-            const Splat2D r = rec[keys[base + tid]];
+    float acc[8];                                          // acc[2j], acc[2j+1] = columns 3 - j, 4 + j of the segment
+    #pragma unroll
+    for (int k = 0; k < 8; ++k) acc[k] = 0.f;
+    for (uint32_t base = kbeg; base < kend; base += kSplatFwdBatch) {
+        const int nb = (int)min((uint32_t)kSplatFwdBatch, kend - base);
+        __syncwarp();
+        if (lane < nb) {
+            const Splat2D r = rec[keys[base + lane]];
             const int x0 = max(r.u0 - ox, 0), x1 = min(r.u1 - ox, kSplatTile - 1);
             const int y0 = max(r.v0 - oy, 0), y1 = min(r.v1 - oy, kSplatTile - 1);
-            SplatTileRec t;
+            SplatTileRec& t = s_rec[lane];
             t.cx = (float)(r.ciu - ox) + r.cfu; t.cy = (float)(r.civ - oy) + r.cfv;
-            t.A = r.A; t.B2 = 2.f * r.B; t.C = r.C; t.amp = r.amp;
-            t.mask = (((2u << x1) - (1u << x0)) & 0xffffu) | ((((2u << y1) - (1u << y0)) & 0xffffu) << 16);
-            t.pad = 0u;
-            s_rec[tid] = t;
+            t.A = r.A; t.Bq = r.Bq; t.Dq = r.Dq; t.cc = ex2s(2.f * r.A);
+            t.rowmask = ((2u << y1) - (1u << y0)) & 0xffffu;
+            t.direct = (-r.A > kRecurrenceMaxA) ? 1u : 0u;
+            const uint32_t xm = ((2u << x1) - (1u << x0)) & 0xffffu;
+            #pragma unroll
+            for (int s2 = 0; s2 < 2; ++s2)
+                #pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    t.w[8 * s2 + 2 * j] = (xm >> (8 * s2 + 3 - j)) & 1u ? r.amp : 0.f;
+                    t.w[8 * s2 + 2 * j + 1] = (xm >> (8 * s2 + 4 + j)) & 1u ? r.amp : 0.f;
+                }
         }
-        __syncthreads();
-        #pragma unroll 4
+        __syncwarp();
+        #pragma unroll 2
         for (int j = 0; j < nb; ++j) {
-            const uint32_t m = s_rec[j].mask;
-            if ((m & warprows) == 0u) continue;                      // warp-uniform: the box misses both rows
-            const float4 a = *reinterpret_cast<const float4*>(&s_rec[j]);            // cx, cy, A, B2
-            const float2 c = *reinterpret_cast<const float2*>(&s_rec[j].C);          // C, amp
-            const float dx = fx - a.x, dy = fy - a.y;
-            const float e = fmaf(c.x * dy, dy, fmaf(a.w, dy, a.z * dx) * dx);
-            const float w = ((m & mybits) == mybits) ? c.y : 0.f;
-            acc = fmaf(w, ex2s(e), acc);
+            const float4 g0 = *reinterpret_cast<const float4*>(&s_rec[j]);             // cx, cy, A, Bq
+            const float4 g1 = *reinterpret_cast<const float4*>(&s_rec[j].Dq);          // Dq, cc, rowmask, direct
+            const float4 wa = *reinterpret_cast<const float4*>(&s_rec[j].w[8 * seg]);
+            const float4 wb = *reinterpret_cast<const float4*>(&s_rec[j].w[8 * seg + 4]);
+            const float dy = fy - g0.y;
+            const float xs = fmaf(-g0.w, dy, g0.x);                    // E(x) = A (x - xs)^2 + Es
+            float Es = g1.x * dy * dy;
+            Es = (__float_as_uint(g1.z) & rowbit) ? Es : -1.0e30f;     // rows outside the box contribute exact zeros
+            const float negA = g0.z;
+            f32x2 Pp[4];                                               // Pp[j] = (G[3-j], G[4+j]) of this segment
+            if (__float_as_uint(g1.w) == 0u) {
+                const float t3 = fx3 - xs;
+                const float nAt = negA * t3;
+                const float Lf = fminf(fmaf(nAt, 2.0f, negA), 120.f);  // E(4) - E(3), clamped: 0 * inf would be NaN
+                const float Lb = fminf(fmaf(nAt, -2.0f, negA), 120.f); // E(2) - E(3)
+                const f32x2 cc2 = pk2(g1.y, g1.y);
+                const float G3 = ex2s(fmaf(nAt, t3, Es));
+                const float rf = ex2s(Lf), rb = ex2s(Lb);
+                const float G4 = G3 * rf;
+                f32x2 R = pk2(rb, rf * g1.y);
+                Pp[0] = pk2(G3, G4);
+                Pp[1] = mul2(Pp[0], R); R = mul2(R, cc2);
+                Pp[2] = mul2(Pp[1], R); R = mul2(R, cc2);
+                Pp[3] = mul2(Pp[2], R);
+            } else {
+                #pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float tl = fx3 - (float)q - xs, th = fx3 + 1.f + (float)q - xs;
+                    Pp[q] = pk2(ex2s(fmaf(negA * tl, tl, Es)), ex2s(fmaf(negA * th, th, Es)));
+                }
+            }
+            fma2_acc(acc[0], acc[1], Pp[0], pk2(wa.x, wa.y));
+            fma2_acc(acc[2], acc[3], Pp[1], pk2(wa.z, wa.w));
+            fma2_acc(acc[4], acc[5], Pp[2], pk2(wb.x, wb.y));
+            fma2_acc(acc[6], acc[7], Pp[3], pk2(wb.z, wb.w));
         }
     }
-    const int px = ox + lx, py = oy + ly;
-    if (px < P.nu && py < P.nv) drr[((size_t)b * P.nv + py) * P.nu + px] = acc;
+    const int py = oy + row;
+    if (py < P.nv) {
+        float* o = drr + ((size_t)b * P.nv + py) * P.nu + ox + 8 * seg;
+        #pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int xl = ox + 8 * seg + 3 - q, xh = ox + 8 * seg + 4 + q;
+            if (xl < P.nu) o[3 - q] = acc[2 * q];
+            if (xh < P.nu) o[4 + q] = acc[2 * q + 1];
+        }
+    }
 }
 
 // s4: one CTA (128 threads) per (tile, angle); the tile's upstream gradient in shared memory; ONE
@@ -562,7 +618,7 @@ extern "C" int gsvox_splat_forward(const float* pos, const float* scale, const f
         GSVOX_CUDA(cudaGetLastError());
     }
     dim3 grid((unsigned)(P.ntx * P.nty), (unsigned)B);
-    k_splat_forward<<<grid, 256, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, drr);
+    k_splat_forward<<<grid, 32, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, drr);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }
