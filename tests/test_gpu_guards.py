@@ -1,0 +1,109 @@
+"""No kernel may write outside the buffers it is handed: every output (and the workspace) of each C-ABI
+call is carved out of one arena with sentinel-filled guard zones on both sides, on ragged shapes
+that exercise every tail path; the guards must be intact afterwards.  (compute-sanitizer is not
+available on this pool; this is the bounds check it would have given.)  `-m gpu`, B200.
+"""
+import numpy as np
+import pytest
+
+import gsvox_inputs
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+GUARD = 4096            # floats on each side
+SENT = -123456.0
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2503_22139_b200 as p
+    p.lib()
+    torch.cuda.set_device(0)
+    return p
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+class Arena:
+    """Carves float32 tensors out of one allocation, 64-float aligned, with guard zones between them."""
+    def __init__(self, shapes):
+        sizes = [int(np.prod(s)) for s in shapes]
+        total = GUARD + sum(((n + 63) // 64) * 64 + GUARD for n in sizes)
+        self.buf = torch.full((total,), SENT, dtype=torch.float32, device="cuda")
+        self.views, self.spans = [], []
+        off = GUARD
+        for s, n in zip(shapes, sizes):
+            self.views.append(self.buf[off:off + n].view(*s))
+            self.spans.append((off, off + n))
+            off += ((n + 63) // 64) * 64 + GUARD
+
+    def check(self):
+        torch.cuda.synchronize()
+        mask = torch.ones(self.buf.numel(), dtype=torch.bool, device="cuda")
+        for a, b in self.spans:
+            mask[a:b] = False
+        bad = (self.buf[mask] != SENT).nonzero()
+        assert bad.numel() == 0, "guard zone overwritten at %d positions" % bad.numel()
+        for v in self.views:
+            assert torch.isfinite(v).all() and not (v == SENT).all()
+
+
+def test_voxelizer_outputs_stay_inside_their_buffers(pkg):
+    case = gsvox_inputs.subvolume_case()                       # 37 x 29 x 21, C = 3, anisotropic spacing
+    nx, ny, nz = case.dims
+    C = case.channels
+    ar = Arena([(C, nz, ny, nx), (case.n, C), (case.n, 3), (case.n, 3), (case.n, 4)])
+    out, gw, gp, gs, gq = ar.views
+    plan = pkg.Plan(case.n, case.grid, max_channels=C)
+    plan.preprocess(dev(case.pos), dev(case.scale), dev(case.quat))
+    plan.forward(dev(case.weight), out=out)
+    plan.backward(dev(case.weight), dev(case.grad_out()), grads=(gw, gp, gs, gq))
+    ar.check()
+
+
+def test_combine_warp_project_outputs_stay_inside_their_buffers(pkg):
+    rng = np.random.default_rng(0)
+    shape = (7, 9, 11)                                         # V = 693: not a multiple of 4
+    B, L = 5, 3
+    e = dev(rng.standard_normal((L, 3) + shape).astype(np.float32)); coef = dev(rng.standard_normal((B, L, 3)).astype(np.float32))
+    g = dev(rng.standard_normal((B, 3) + shape).astype(np.float32))
+    ar = Arena([(B, 3) + shape, (L, 3) + shape, (B, L, 3)])
+    d, ge, gc = ar.views
+    pkg.mbc_combine_forward(e, coef, out=d)
+    pkg.mbc_combine_backward(e, coef, g, grads=(ge, gc))
+    ar.check()
+
+    wc = gsvox_inputs.warp_case(batch=3, dims=(37, 29, 21), spacing=(2.0, 1.5, 0.75), amp_vox=6.0, seed=41)
+    nx, ny, nz = wc.dims
+    ar = Arena([(3, nz, ny, nx), (nz, ny, nx), (3, 3, nz, ny, nx)])
+    out, gi, gd = ar.views
+    pkg.warp_forward(dev(wc.iref), dev(wc.dvf), wc.grid, out=out)
+    pkg.warp_backward(dev(wc.iref), dev(wc.dvf), wc.grid, dev(wc.grad_out()), grads=(gi, gd))
+    ar.check()
+
+    pc = gsvox_inputs.project_case(batch=3, dims=(37, 45, 21), spacing=(2.0, 1.5, 2.5), nu=70, nv=40, du=3.0, dv=3.0,
+                                   sad=300.0, sdd=450.0, seed=51, angles=[0.2, 1.0, 2.9])
+    V = 37 * 45 * 21
+    ar = Arena([(3, 40, 70), (3, 21, 45, 37), (3 * V,), (3 * V,)])
+    drr, gv, s1, s2 = ar.views
+    pkg.project_forward(dev(pc.vol), pc.grid, pc.geom, list(pc.angles), out=drr, scratch=s1)
+    pkg.project_backward(dev(pc.grad_drr()), pc.grid, pc.geom, list(pc.angles), out=gv, scratch=s2)
+    ar.check()
+
+
+def test_splat_outputs_stay_inside_their_buffers(pkg):
+    sc = gsvox_inputs.splat_case(n=300, batch=3, extent=(120.0, 120.0, 60.0), nu=90, nv=70, du=2.0, dv=2.5,
+                                 sad=300.0, sdd=450.0, off_u=11.0, off_v=-6.0, seed=61, angles=[0.0, 1.3, 3.9])
+    ar = Arena([(3, 70, 90), (sc.n,), (sc.n, 3), (sc.n, 3), (sc.n, 4)])
+    drr, gr, gp, gs, gq = ar.views
+    sp = pkg.Splatter(sc.n, sc.geom, sc.batch)
+    a = (dev(sc.pos), dev(sc.scale), dev(sc.quat), dev(sc.rho))
+    sp.forward(*a, list(sc.angles), out=drr)
+    sp.backward(*a, list(sc.angles), dev(sc.grad_drr()), grads=(gr, gp, gs, gq))
+    assert not sp.status()["overflow"]
+    ar.check()
