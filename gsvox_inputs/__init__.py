@@ -420,6 +420,74 @@ def splat_case(n=50_000, batch=8, extent=(400.0, 400.0, 200.0), voxel=2.0, nu=51
                      np.asarray(angles, np.float32), geom, seed=seed)
 
 
+@dataclass
+class Stage3Case:
+    """Inputs of one Stage-2/3 step: reference Gaussians, three MBC levels, per-projection
+    coefficients, gantry angles, all in world units (mm) on one voxel grid centred at the isocentre."""
+    name: str
+    dims: tuple
+    spacing: tuple
+    origin: tuple
+    ref: tuple                  # (pos, scale, quat, rho[n,1])
+    levels: list                # [(pos, scale, quat, feat[n,3]), ...]
+    coef: np.ndarray            # [B, L, 3]
+    angles: np.ndarray          # [B]
+    geom: dict
+    seed: object = 0
+
+    @property
+    def grid(self):
+        return (np.asarray(self.origin, np.float32), np.asarray(self.spacing, np.float32),
+                np.asarray(self.dims, np.int32))
+
+    @property
+    def batch(self):
+        return int(self.angles.shape[0])
+
+    def grad_drr(self):
+        rng = np.random.default_rng([81, self.batch] + list(np.atleast_1d(self.seed)))
+        return rng.standard_normal((self.batch, self.geom["nv"], self.geom["nu"]), dtype=np.float32)
+
+
+def stage3_case(batch=8, dims=(200, 200, 100), voxel=2.0, n_ref=100_000, n_levels=(8_000, 10_648, 13_824),
+                nu=512, nv=384, du=0.776, dv=0.776, sad=1000.0, sdd=1500.0, seed=9, dvf_mm=4.0):
+    """The paper's patient-study sizes (M = 100 000 reference Gaussians, MBC levels 20^3 / 22^3 /
+    24^3 Gaussians; 200 x 200 x 100 voxels of 2 mm; Table I detector).  Reference Gaussians as config 2 (scales
+    logU(1,4) voxels, 3-tissue rho); MBC Gaussians as config 3's levels scaled to this grid (scales logU(16,32) /
+    (6,12) / (2,5) voxels x 200/128), features N(0,1) mm; coefficients N(0, dvf_mm / sqrt(levels * mean overlap)),
+    sized so that displacements are a few mm."""
+    rng = np.random.default_rng(seed)
+    ext = np.asarray(dims, np.float64) * voxel
+    origin = tuple(-(n - 1) / 2.0 * voxel for n in dims)
+
+    def in_ellipsoid(n):
+        pts = np.empty((0, 3))
+        while pts.shape[0] < n:
+            c = rng.uniform(-1.0, 1.0, size=(2 * n + 16, 3))
+            pts = np.concatenate([pts, c[(c * c).sum(1) <= 1.0]])
+        return np.array([0.45, 0.35, 0.48]) * ext * pts[:n]
+    pos = in_ellipsoid(n_ref)
+    scale = _log_uniform(rng, 1.0 * voxel, 4.0 * voxel, (n_ref, 3))
+    tissue = rng.choice(np.array([0.02, 0.2, 0.5]), size=n_ref, p=[0.6, 0.3, 0.1])
+    rho = (tissue + rng.normal(0.0, 0.01, size=n_ref)).reshape(n_ref, 1)
+    ref = (_f32(pos), _f32(scale), _f32(_unit_quats(rng, n_ref)), _f32(rho))
+    k = voxel * dims[0] / 128.0
+    levels = []
+    for n, (a, b) in zip(n_levels, ((16.0, 32.0), (6.0, 12.0), (2.0, 5.0))):
+        p = rng.uniform(-0.5, 0.5, size=(n, 3)) * ext
+        levels.append((_f32(p), _f32(_log_uniform(rng, a * k, b * k, (n, 3))), _f32(_unit_quats(rng, n)),
+                       _f32(rng.standard_normal((n, 3)))))
+    # typical |e_{i,k}(x)| ~ sqrt(number of Gaussians overlapping a voxel): keep |d| at a few mm
+    overlap = [n * (2.5 * k * (a + b) / 2) ** 3 / float(np.prod(ext)) for n, (a, b) in
+               zip(n_levels, ((16.0, 32.0), (6.0, 12.0), (2.0, 5.0)))]
+    coef = rng.standard_normal((batch, len(n_levels), 3)) * dvf_mm / np.sqrt(3.0 * np.maximum(1.0, np.asarray(overlap)))[None, :, None]
+    angles = rng.uniform(0.0, 2 * np.pi, size=batch)
+    geom = dict(sad=float(sad), sdd=float(sdd), nu=int(nu), nv=int(nv), du=float(du), dv=float(dv),
+                off_u=0.0, off_v=0.0, iso=[0.0, 0.0, 0.0])
+    return Stage3Case("stage3_b%d" % batch, tuple(dims), (voxel,) * 3, origin, ref, levels, _f32(coef),
+                      np.asarray(angles, np.float32), geom, seed=seed)
+
+
 FULL = {
     "config1": lambda: [config1()],
     "config2": lambda: [config2()],

@@ -6,3 +6,6 @@ from .binding import (EXPORTS, K_NAMES, LIB_PATH, GsvoxError, GsvoxGrid, GsvoxSt
 
 __all__ = ["EXPORTS", "K_NAMES", "LIB_PATH", "GsvoxError", "GsvoxGrid", "GsvoxStatus", "Plan", "Splatter", "lib",
            "make_grid", "mbc_combine_backward", "mbc_combine_forward", "probe_peaks", "project_backward", "project_forward", "warp_backward", "warp_forward"]
+from .pipeline import Stage3Step  # noqa: E402
+
+__all__.append("Stage3Step")
