@@ -320,6 +320,29 @@ def next_rows(torch, pkg, hbm_peak_gbs, quick=False):
         "forward_backward": {"ms": mfb, "pairs_per_s": sst["pairs"] / (mfb * 1e-3),
                              "canonical_tflops": 36 * sst["pairs"] / (mfb * 1e-3) / 1e12,
                              "frac_of_fp32_peak": 36 * sst["pairs"] / (mfb * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}}
+    del sargs, sdrr, sg
+    # ---- the rows chained: one Stage-3 step at the paper's patient-study sizes (Table I)
+    s3 = gsvox_inputs.stage3_case(batch=8)
+    step = pkg.Stage3Step(s3.grid, s3.geom, len(s3.ref[0]), [len(l[0]) for l in s3.levels], s3.batch)
+    ref = tuple(dev(a) for a in s3.ref)
+    levels = [tuple(dev(a) for a in lv) for lv in s3.levels]
+    coef, gdr, angs = dev(s3.coef), dev(s3.grad_drr()), list(s3.angles)
+    step.fit(ref, levels)                                                      # size the key buffers once
+
+    def s3_fwd():
+        step.forward(ref, levels, coef, angs)
+
+    def s3_fb():
+        step.forward(ref, levels, coef, angs)
+        step.backward(gdr)
+    mf = _time_ms(torch, s3_fwd, 10)
+    mfb = _time_ms(torch, s3_fb, 10)
+    res["stage3_step_200x200x100_b8"] = {
+        "workload": "100k reference + 8000/10648/13824 MBC Gaussians -> I_ref, 9 MBC volumes, 8 DVFs, 8 warped volumes, "
+                    "8 DRRs of 512x384, and back to every Gaussian parameter and coefficient",
+        "forward_ms": mf, "forward_backward_ms": mfb,
+        "context": "the paper's whole iteration (this chain + CNN encoder + losses + Adam) averages ~340 ms on an RTX 4090 "
+                   "(40 min / 7000 iterations, PAPER.md:152, 203)"}
     return res
 
 

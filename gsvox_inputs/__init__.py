@@ -453,9 +453,11 @@ def stage3_case(batch=8, dims=(200, 200, 100), voxel=2.0, n_ref=100_000, n_level
                 nu=512, nv=384, du=0.776, dv=0.776, sad=1000.0, sdd=1500.0, seed=9, dvf_mm=4.0):
     """The paper's patient-study sizes (M = 100 000 reference Gaussians, MBC levels 20^3 / 22^3 /
     24^3 Gaussians; 200 x 200 x 100 voxels of 2 mm; Table I detector).  Reference Gaussians as config 2 (scales
-    logU(1,4) voxels, 3-tissue rho); MBC Gaussians as config 3's levels scaled to this grid (scales logU(16,32) /
-    (6,12) / (2,5) voxels x 200/128), features N(0,1) mm; coefficients N(0, dvf_mm / sqrt(levels * mean overlap)),
-    sized so that displacements are a few mm."""
+    logU(1,4) voxels, 3-tissue rho).  MBC Gaussians: the paper gives the counts but not the sizes; with 20-24
+    Gaussians per axis the lattice pitch is ~10 x 10 x 5 voxels, so the three coarse-to-fine levels take scales
+    logU(6,12) / (4,8) / (2,5) voxels (a reading; config 3's 16-32 voxels belong to its 1 000-Gaussian level),
+    features N(0,1) mm; coefficients N(0, dvf_mm / sqrt(levels * mean overlap)), sized so that displacements are a
+    few mm."""
     rng = np.random.default_rng(seed)
     ext = np.asarray(dims, np.float64) * voxel
     origin = tuple(-(n - 1) / 2.0 * voxel for n in dims)
@@ -471,15 +473,15 @@ def stage3_case(batch=8, dims=(200, 200, 100), voxel=2.0, n_ref=100_000, n_level
     tissue = rng.choice(np.array([0.02, 0.2, 0.5]), size=n_ref, p=[0.6, 0.3, 0.1])
     rho = (tissue + rng.normal(0.0, 0.01, size=n_ref)).reshape(n_ref, 1)
     ref = (_f32(pos), _f32(scale), _f32(_unit_quats(rng, n_ref)), _f32(rho))
-    k = voxel * dims[0] / 128.0
+    k = voxel
+    level_scales = ((6.0, 12.0), (4.0, 8.0), (2.0, 5.0))
     levels = []
-    for n, (a, b) in zip(n_levels, ((16.0, 32.0), (6.0, 12.0), (2.0, 5.0))):
+    for n, (a, b) in zip(n_levels, level_scales):
         p = rng.uniform(-0.5, 0.5, size=(n, 3)) * ext
         levels.append((_f32(p), _f32(_log_uniform(rng, a * k, b * k, (n, 3))), _f32(_unit_quats(rng, n)),
                        _f32(rng.standard_normal((n, 3)))))
     # typical |e_{i,k}(x)| ~ sqrt(number of Gaussians overlapping a voxel): keep |d| at a few mm
-    overlap = [n * (2.5 * k * (a + b) / 2) ** 3 / float(np.prod(ext)) for n, (a, b) in
-               zip(n_levels, ((16.0, 32.0), (6.0, 12.0), (2.0, 5.0)))]
+    overlap = [n * (2.5 * k * (a + b) / 2) ** 3 / float(np.prod(ext)) for n, (a, b) in zip(n_levels, level_scales)]
     coef = rng.standard_normal((batch, len(n_levels), 3)) * dvf_mm / np.sqrt(3.0 * np.maximum(1.0, np.asarray(overlap)))[None, :, None]
     angles = rng.uniform(0.0, 2 * np.pi, size=batch)
     geom = dict(sad=float(sad), sdd=float(sdd), nu=int(nu), nv=int(nv), du=float(du), dv=float(dv),

@@ -38,6 +38,21 @@ class Stage3Step:
         self.scratch = B_._project_scratch(B_.make_grid(*grid), batch, dev)
         self._saved = None
 
+    def fit(self, ref, levels, slack=1.05):
+        """Size the (brick, Gaussian) key buffers for these Gaussians: preprocess once, read the device status
+        (synchronises) and re-create any plan whose key capacity is too small.  Call once before the loop."""
+        def fitted(plan, params, ch):
+            plan.preprocess(*params[:3])
+            st = plan.status()
+            if st["overflow"]:
+                plan = B_.Plan(plan.n_max, self.grid, max_channels=ch, key_capacity=int(slack * st["keys_needed"]) + 1024)
+                plan.preprocess(*params[:3])
+                assert not plan.status()["overflow"]
+            return plan
+        self.plan_ref = fitted(self.plan_ref, ref, 1)
+        self.plans = [fitted(p, lv, 3) for p, lv in zip(self.plans, levels)]
+        return self
+
     def forward(self, ref, levels, coef, angles):
         """ref = (pos, scale, quat, rho[n,1]); levels = [(pos, scale, quat, feat[n,3]), ...]; coef [B,L,3];
         angles: B radians (host).  -> drr [B, nv, nu] (a buffer owned by this object)."""
