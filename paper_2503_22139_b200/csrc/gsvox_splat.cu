@@ -26,7 +26,6 @@ namespace gsvox {
 
 constexpr int kSplatTile = 16;
 constexpr int kSplatMaxBatch = 64;
-constexpr int kSplatBatch = 64;                 // keys staged per __syncthreads
 constexpr double kSplatKappa = GSVOX_SIGMA_CUTOFF;
 
 struct __align__(16) Splat2D {
