@@ -148,3 +148,22 @@ def test_splat_full_size_sampled_pixels(pkg):
         assert rels[name] <= GRAD_REL, (name, rels[name])
     print("splat full size: forward err/tol %.3f, grads %s, pairs %.3e keys %.3e" %
           (worst / (FWD_REL * peak + FWD_ABS), rels, st["pairs"], st["keys_needed"]))
+
+
+def test_splat_single_isolated_gaussians_worst_case_tolerance(pkg):
+    """One Gaussian per image, footprints around the recurrence / direct switch (sigma ~ 0.85 pixel along
+    x) and up: no averaging over neighbours hides the error of the multiplicative recurrence."""
+    geom = dict(sad=300.0, sdd=450.0, nu=64, nv=48, du=1.0, dv=1.0, off_u=0.0, off_v=0.0, iso=[0.0, 0.0, 0.0])
+    worst = 0.0
+    for k, sig_mm in enumerate([0.45, 0.55, 0.6, 0.7, 0.9, 1.3, 2.0, 3.7]):            # x 1.5 magnification = pixels
+        rng = np.random.default_rng(100 + k)
+        case = gsvox_inputs.SplatCase("one", np.asarray([[rng.uniform(-5, 5), rng.uniform(-5, 5), rng.uniform(-4, 4)]], np.float32),
+                                      np.asarray([[sig_mm, sig_mm * rng.uniform(0.7, 1.5), sig_mm * rng.uniform(0.7, 1.5)]], np.float32),
+                                      rng.standard_normal((1, 4)).astype(np.float32), np.asarray([0.9], np.float32),
+                                      np.asarray([rng.uniform(0, 6.28)], np.float32), geom, seed=100 + k)
+        drr, _, st = run_gpu(pkg, case)
+        ref = oracle.splat_forward(case.pos, case.scale, case.quat, case.rho, geom, case.angles)
+        tol = FWD_REL * np.abs(ref).max() + FWD_ABS
+        worst = max(worst, float(np.abs(drr - ref).max() / tol))
+    assert worst <= 1.0, worst
+    print("splat isolated Gaussians: worst err/tol %.3f" % worst)
