@@ -77,3 +77,18 @@ def sharded_backward(plan, weight, grad_out, ranks, grads=None, all_reduce=None)
     if ranks.on:
         (all_reduce or dist.all_reduce)(plan.accumulators(ch))
     return plan.backward_finish(ch, grads=grads)
+
+
+def batch_bounds(batch, rank, world):
+    """The 8(f) operators (combine, warp, projector, rasterizer) are independent per projection of a batch:
+    rank r takes projections [lo, hi) of the B, no data-path collective in forward; in backward only the
+    gradients of the SHARED parameters (Gaussians, I_ref) are summed over ranks (all_reduce_grads)."""
+    return slab_bounds(batch, rank, world)
+
+
+def all_reduce_grads(tensors, ranks, all_reduce=None):
+    """Sum per-rank partial gradients of shared parameters in place (one call per tensor; NCCL on GPUs)."""
+    if ranks.on:
+        for t in tensors:
+            (all_reduce or dist.all_reduce)(t)
+    return tensors

@@ -120,3 +120,37 @@ def test_two_rank_gloo_sharded_backward_all_reduces_between_the_halves():
     for o in outs:
         assert o["calls"] == ["acc", "view1", "fin"]
         assert o["sum"] == 3.0                               # 1 + 2: summed over both ranks before a5
+
+
+BATCH_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import torch
+from paper_2503_22139_b200.dist import Ranks, batch_bounds, all_reduce_grads
+r = Ranks(backend="gloo")
+lo, hi = batch_bounds(8, r.rank, r.world)
+g = [torch.full((5, 3), float(hi - lo)), torch.full((5,), float(r.rank + 1))]       # partial gradients of shared parameters
+all_reduce_grads(g, r)
+r.close()
+print(json.dumps({"rank": r.rank, "b": [lo, hi], "g0": float(g[0][0, 0]), "g1": float(g[1][0])}))
+"""
+
+
+def test_two_rank_gloo_projection_batch_sharding_and_gradient_sum():
+    import json
+    port = free_port()
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", LOCAL_RANK=str(rank),
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, "-c", BATCH_WORKER % ROOT], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = []
+    for p in procs:
+        o, e = p.communicate(timeout=120)
+        assert p.returncode == 0, e[-2000:]
+        outs.append(json.loads(o.strip().splitlines()[-1]))
+    outs.sort(key=lambda o: o["rank"])
+    assert outs[0]["b"] == [0, 4] and outs[1]["b"] == [4, 8]
+    for o in outs:
+        assert o["g0"] == 8.0 and o["g1"] == 3.0             # sums over both ranks
