@@ -320,7 +320,11 @@ class Plan:
             lib().gsvox_plan_destroy(self._h)
             self._h = C.c_void_p(None)
 
-    __del__ = close
+    def __del__(self):
+        try:                 # at interpreter shutdown the module globals close() uses may already be gone
+            self.close()
+        except Exception:
+            pass
 
     # --- the three hot-path calls -----------------------------------------------------
     def preprocess(self, pos, scale, quat):
