@@ -261,14 +261,20 @@ struct __align__(16) SplatTileRec {
 };
 static_assert(sizeof(SplatTileRec) == 96, "SplatTileRec must be 96 bytes");
 
+#ifndef SPLAT_FWD_WARPS
+#define SPLAT_FWD_WARPS 4   // measured: 1 warp 0.52 ms, 2: 0.45, 4: 0.40, 8: 0.40 (50 k Gaussians x 8 angles)
+#endif
 constexpr int kSplatFwdBatch = 32;
+constexpr int kSplatFwdWarps = SPLAT_FWD_WARPS;   // warps of a CTA take the tile's key batches round-robin; partial tiles summed in smem
 
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32 * kSplatFwdWarps)
 k_splat_forward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* __restrict__ bin_start,
                 const uint32_t* __restrict__ keys, const SplatStatus* __restrict__ status, float* __restrict__ drr)
 {
-    __shared__ SplatTileRec s_rec[kSplatFwdBatch];
-    const int lane = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
+    __shared__ SplatTileRec s_recs[kSplatFwdWarps][kSplatFwdBatch];
+    __shared__ float s_part[kSplatFwdWarps > 1 ? kSplatFwdWarps - 1 : 1][8][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tile = blockIdx.x, b = blockIdx.y;
+    SplatTileRec* s_rec = s_recs[warp];
     const int tx = tile % P.ntx, ty = tile / P.ntx;
     const int ox = tx * kSplatTile, oy = ty * kSplatTile;
     const int row = lane >> 1, seg = lane & 1;
@@ -279,7 +285,7 @@ k_splat_forward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* 
     float acc[8];                                          // acc[2j], acc[2j+1] = columns 3 - j, 4 + j of the segment
     #pragma unroll
     for (int k = 0; k < 8; ++k) acc[k] = 0.f;
-    for (uint32_t base = kbeg; base < kend; base += kSplatFwdBatch) {
+    for (uint32_t base = kbeg + warp * kSplatFwdBatch; base < kend; base += kSplatFwdBatch * kSplatFwdWarps) {
         const int nb = (int)min((uint32_t)kSplatFwdBatch, kend - base);
         __syncwarp();
         if (lane < nb) {
@@ -339,6 +345,18 @@ k_splat_forward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* 
             fma2_acc(acc[4], acc[5], Pp[2], pk2(wb.x, wb.y));
             fma2_acc(acc[6], acc[7], Pp[3], pk2(wb.z, wb.w));
         }
+    }
+    if (kSplatFwdWarps > 1) {
+        if (warp > 0) {
+            #pragma unroll
+            for (int k = 0; k < 8; ++k) s_part[warp - 1][k][lane] = acc[k];
+        }
+        __syncthreads();
+        if (warp > 0) return;
+        #pragma unroll
+        for (int w = 0; w < kSplatFwdWarps - 1; ++w)
+            #pragma unroll
+            for (int k = 0; k < 8; ++k) acc[k] += s_part[w][k][lane];
     }
     const int py = oy + row;
     if (py < P.nv) {
@@ -617,7 +635,7 @@ extern "C" int gsvox_splat_forward(const float* pos, const float* scale, const f
         GSVOX_CUDA(cudaGetLastError());
     }
     dim3 grid((unsigned)(P.ntx * P.nty), (unsigned)B);
-    k_splat_forward<<<grid, 32, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, drr);
+    k_splat_forward<<<grid, 32 * kSplatFwdWarps, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, drr);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }
