@@ -142,8 +142,9 @@ __device__ __forceinline__ void proj_red(float* addr, float v)
 // Neighbouring detector pixels are ~0.26 voxel apart in the volume (0.776 mm pixels, magnification
 // 1.5, 2 mm voxels), so runs of 3-4 consecutive lanes hit the SAME cell on a plane: their four corner
 // contributions are summed by a segmented shuffle reduction (runs = maximal stretches of lanes with
-// equal (ib, ic), split every 8 lanes so that three doubling steps suffice) and only the head of a run
-// issues the atomics.
+// equal (ib, ic), split every CUT lanes so that log2(CUT) doubling steps suffice) and only the head of a
+// run issues the atomics.  The kernel is bound by instruction issue, not by the atomics: merging PAIRS
+// (CUT = 2, 4 shuffles) beats longer runs until ~4.5 lanes share a cell (host picks CUT, see below).
 __device__ __forceinline__ void scatter4(float* __restrict__ base, const Lay& L, int m, int ib, int ic,
                                          float a00, float a10, float a01, float a11)
 {
@@ -158,6 +159,7 @@ __device__ __forceinline__ void scatter4(float* __restrict__ base, const Lay& L,
     if (b1 && c1) proj_red(r1 + 1, a11);
 }
 
+template <int CUT>
 __global__ void __launch_bounds__(kProjThreads)
 k_project_backward(const float* __restrict__ gdrr, ProjParams P, float* __restrict__ gvol, float* __restrict__ gvolT)
 {
@@ -181,31 +183,39 @@ k_project_backward(const float* __restrict__ gdrr, ProjParams P, float* __restri
         }
         return;
     }
+    const int sa = (int)L.sa, sc = (int)L.sc, nb1 = L.nb - 1, nc1 = L.nc - 1;      // 32-bit offsets inside one volume, as in the forward
     int mlo = (live && r.m0 <= r.m1) ? r.m0 : 0x7fffffff, mhi = (live && r.m0 <= r.m1) ? r.m1 : -1;
     for (int o = 16; o > 0; o >>= 1) {
         mlo = min(mlo, __shfl_xor_sync(full, mlo, o));
         mhi = max(mhi, __shfl_xor_sync(full, mhi, o));
     }
+    const bool on = live && g != 0.f;
+    const int m0 = on ? r.m0 : 0x7fffffff, m1 = on ? r.m1 : -1;
     for (int m = mlo; m <= mhi; ++m) {
         int ib, ic; float fb, fc;
         const bool good = sample_cell(r, m, ib, ic, fb, fc);
-        const bool act = live && good && m >= r.m0 && m <= r.m1 && g != 0.f;
+        const bool act = good && m >= m0 && m <= m1;
         const int key = act ? (ic + 1) * 40000 + (ib + 1) : -1 - lane;          // dims <= 32760: no collision, no overflow
         const float g0 = act ? g * (1.f - fc) : 0.f, g1 = act ? g * fc : 0.f;
         float a00 = g0 * (1.f - fb), a10 = g0 * fb, a01 = g1 * (1.f - fb), a11 = g1 * fb;
         const int kprev = __shfl_up_sync(full, key, 1);
         const unsigned bmask = __ballot_sync(full, lane == 0 || key != kprev);   // run starts
         const int start = 31 - __clz(bmask & (0xffffffffu >> (31 - lane)));
-        const bool head = ((lane - start) & 7) == 0;                             // runs are cut every 8 lanes
+        const bool head = ((lane - start) & (CUT - 1)) == 0;                     // runs are cut every CUT lanes
         const unsigned hmask = __ballot_sync(full, head);
-        const unsigned ahead = (lane < 31) ? (hmask >> (lane + 1)) : 0xffffffffu; // heads strictly after this lane
+        const unsigned ahead = ~((~hmask >> lane) >> 1);                         // heads strictly after this lane; ones beyond lane 31
         #pragma unroll
-        for (int o = 1; o <= 4; o <<= 1) {
+        for (int o = 1; o < CUT; o <<= 1) {
             const float v00 = __shfl_down_sync(full, a00, o), v10 = __shfl_down_sync(full, a10, o);
             const float v01 = __shfl_down_sync(full, a01, o), v11 = __shfl_down_sync(full, a11, o);
-            if (lane + o < 32 && (ahead & ((1u << o) - 1u)) == 0u) { a00 += v00; a10 += v10; a01 += v01; a11 += v11; }
+            if ((ahead & ((1u << o) - 1u)) == 0u) { a00 += v00; a10 += v10; a01 += v01; a11 += v11; }
         }
-        if (head && act) scatter4(base, L, m, ib, ic, a00, a10, a01, a11);
+        if (head && act) {
+            if ((unsigned)ib < (unsigned)nb1 && (unsigned)ic < (unsigned)nc1) {   // cell wholly inside the plane: no bounds tests
+                float* q0 = base + (m * sa + ic * sc + ib);
+                proj_red(q0, a00); proj_red(q0 + 1, a10); proj_red(q0 + sc, a01); proj_red(q0 + sc + 1, a11);
+            } else scatter4(base, L, m, ib, ic, a00, a10, a01, a11);
+        }
     }
 }
 
@@ -298,7 +308,12 @@ extern "C" int gsvox_project_backward(const float* grad_drr, const gsvox_grid* g
     GSVOX_CUDA(cudaMemsetAsync(grad_vol, 0, sizeof(float) * (size_t)V * B, st));
     GSVOX_CUDA(cudaMemsetAsync(scratch, 0, sizeof(float) * (size_t)V * B, st));
     dim3 pg((P.nu + kProjThreads - 1) / kProjThreads, (unsigned)P.nv, (unsigned)B);
-    k_project_backward<<<pg, kProjThreads, 0, st>>>(grad_drr, P, grad_vol, (float*)scratch);
+    // lanes (adjacent detector pixels) per in-plane cell at the isocentre; measured on a B200 at 8 x 512x384 rays:
+    // ratio 0.97 / 1.45 / 1.93 / 3.02 / 3.87 -> merging pairs wins (2.69, 2.87, 3.17, 1.43, 1.08 ms; no merging 2.78,
+    // 3.48, 3.84, 1.97, 1.68), ratio 4.83 / 6.04 / 7.73 -> runs of 4 win (0.83, 0.64, 0.52 ms); runs of 8 never win
+    const double lanes_per_cell = fmin(P.h[0], P.h[1]) / (P.du * P.sad / P.sdd);
+    if (lanes_per_cell >= 4.5) k_project_backward<4><<<pg, kProjThreads, 0, st>>>(grad_drr, P, grad_vol, (float*)scratch);
+    else                       k_project_backward<2><<<pg, kProjThreads, 0, st>>>(grad_drr, P, grad_vol, (float*)scratch);
     GSVOX_CUDA(cudaGetLastError());
     // fold the y-fastest scratch back: grad_vol[z][y][x] += scratch[z][x][y]  (a transpose with nx, ny swapped)
     dim3 tg((P.n[1] + 31) / 32, (P.n[0] + 31) / 32, (unsigned)(P.n[2] * B));
