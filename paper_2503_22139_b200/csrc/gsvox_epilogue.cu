@@ -11,7 +11,7 @@ namespace gsvox {
 // a5: chain rule, one thread per Gaussian, fp64 (negligible cost; keeps the rounding of the
 // kernel's fp32 sums the only fp32 error in the gradients).
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 3)
 k_epilogue(const GsAux* __restrict__ aux, const GsRec* __restrict__ rec, const float* __restrict__ acc, int astride, int n, int C,
            GridDev gd, const DevStatus* __restrict__ status,
            float* __restrict__ gw, float* __restrict__ gp, float* __restrict__ gs, float* __restrict__ gq)

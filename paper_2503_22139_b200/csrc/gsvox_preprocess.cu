@@ -16,7 +16,7 @@ constexpr double kCullBoxRatio = 8.0;     // config 4's 6:1 Gaussians stay below
 
 __device__ __forceinline__ bool finite_d(double v) { return isfinite(v); }
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 3)
 k_preprocess(const float* __restrict__ pos, const float* __restrict__ scale,
              const float* __restrict__ quat, int n, GridDev gd,
              GsRec* __restrict__ rec, GsAux* __restrict__ aux, DevStatus* __restrict__ status)

@@ -459,7 +459,7 @@ k_splat_backward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t*
 //   dL/dcu = amp (A mx + B my);  dL/dcv = amp (B mx + C my)
 // then back through P = K Sigma^ K, amp = rho sqrt(2 pi |Sigma~| / |Sigma^|), Sigma~ = T Sigma T^T,
 // T = J(t) W, t = W (p - source), Sigma = R S^2 R^T, R(q / |q|).
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 4)
 k_splat_epilogue(SplatParams P, const float* __restrict__ pos, const float* __restrict__ scale, const float* __restrict__ quat,
                  const float* __restrict__ rho, const Splat2D* __restrict__ rec, const float* __restrict__ acc,
                  const SplatStatus* __restrict__ status,
