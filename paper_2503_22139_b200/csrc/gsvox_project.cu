@@ -220,28 +220,66 @@ k_project_backward(const float* __restrict__ gdrr, ProjParams P, float* __restri
     }
 }
 
-// dst[b][z][x][y] = src[b][z][y][x]  (ADD: dst[b][z][y][x] += src[b][z][x][y] with the roles of nx, ny swapped)
-template <bool ADD>
+// dst[b][z][x][y] = src[b][z][y][x]  (ADD: dst[b][z][y][x] += src[b][z][x][y] with the roles of nx, ny swapped).
+// One CTA per 64 x 64 tile of one (b, z) slice, 1-D grid (slice-major).  VEC: nx, ny multiples of 4 and 16-byte
+// aligned bases -> float4 global loads and stores (16 KB in flight per CTA); otherwise scalar with bounds tests.
+constexpr int kTrTile = 64;
+template <bool ADD, bool VEC>
 __global__ void __launch_bounds__(256)
-k_transpose_xy(const float* __restrict__ src, long long src_stride, int nx, int ny, int nz, float* __restrict__ dst)
+k_transpose_xy(const float* __restrict__ src, long long src_stride, int nx, int ny, int nz, int tiles_x, int tiles_y,
+               float* __restrict__ dst)
 {
-    __shared__ float tile[32][33];
-    const int z = blockIdx.z % nz, b_ = blockIdx.z / nz;
+    __shared__ float tile[kTrTile][kTrTile + 1];
+    const int tid = threadIdx.x;
+    const unsigned tiles = (unsigned)(tiles_x * tiles_y);
+    const unsigned slice = blockIdx.x / tiles, tl = blockIdx.x % tiles;
+    const int z = (int)(slice % (unsigned)nz), b_ = (int)(slice / (unsigned)nz);
+    const int x0 = (int)(tl % (unsigned)tiles_x) * kTrTile, y0 = (int)(tl / (unsigned)tiles_x) * kTrTile;
     const long long V = (long long)nx * ny * nz;
     const float* s = src + (long long)b_ * src_stride + (long long)z * nx * ny;
     float* d = dst + (long long)b_ * V + (long long)z * nx * ny;
-    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    for (int j = ty; j < 32; j += 8) {
-        const int x = x0 + tx, y = y0 + j;
-        tile[j][tx] = (x < nx && y < ny) ? s[(long long)y * nx + x] : 0.f;
-    }
-    __syncthreads();
-    for (int j = ty; j < 32; j += 8) {
-        const int y = y0 + tx, x = x0 + j;
-        if (x < nx && y < ny) {
-            float* o = d + (long long)x * ny + y;
-            if (ADD) *o += tile[tx][j]; else *o = tile[tx][j];
+    if (VEC) {
+        const int c4 = (tid & 15) * 4, r0 = tid >> 4;
+        float4 v[4];
+        #pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int y = y0 + r0 + 16 * i, x = x0 + c4;
+            v[i] = (x < nx && y < ny) ? __ldg(reinterpret_cast<const float4*>(s + y * nx + x)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        #pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            float* t = &tile[r0 + 16 * i][c4];
+            t[0] = v[i].x; t[1] = v[i].y; t[2] = v[i].z; t[3] = v[i].w;
+        }
+        __syncthreads();
+        float4 o[4];
+        #pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int x = x0 + r0 + 16 * i, y = y0 + c4;
+            if (ADD) o[i] = (x < nx && y < ny) ? *reinterpret_cast<const float4*>(d + x * ny + y) : make_float4(0.f, 0.f, 0.f, 0.f);
+            else o[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        #pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int xr = r0 + 16 * i, x = x0 + xr, y = y0 + c4;
+            if (x < nx && y < ny) {
+                o[i].x += tile[c4][xr]; o[i].y += tile[c4 + 1][xr]; o[i].z += tile[c4 + 2][xr]; o[i].w += tile[c4 + 3][xr];
+                *reinterpret_cast<float4*>(d + x * ny + y) = o[i];
+            }
+        }
+    } else {
+        const int tx = tid & 63, ty = tid >> 6;
+        for (int j = ty; j < kTrTile; j += 4) {
+            const int x = x0 + tx, y = y0 + j;
+            tile[j][tx] = (x < nx && y < ny) ? s[y * nx + x] : 0.f;
+        }
+        __syncthreads();
+        for (int j = ty; j < kTrTile; j += 4) {
+            const int y = y0 + tx, x = x0 + j;
+            if (x < nx && y < ny) {
+                float* o = d + x * ny + y;
+                if (ADD) *o += tile[tx][j]; else *o = tile[tx][j];
+            }
         }
     }
 }
@@ -249,6 +287,20 @@ k_transpose_xy(const float* __restrict__ src, long long src_stride, int nx, int 
 }  // namespace gsvox
 
 using namespace gsvox;
+
+template <bool ADD>
+static int launch_transpose(const float* src, long long src_stride, int nx, int ny, int nz, int B, float* dst, cudaStream_t st)
+{
+    const int tiles_x = (nx + kTrTile - 1) / kTrTile, tiles_y = (ny + kTrTile - 1) / kTrTile;
+    const long long blocks = (long long)tiles_x * tiles_y * nz * B;
+    if (blocks > 0x7fffffffLL) return GSVOX_ELIMIT;
+    const bool vec = (nx % 4 == 0) && (ny % 4 == 0) && (src_stride % 4 == 0) &&
+                     (((uintptr_t)src | (uintptr_t)dst) & 15u) == 0;
+    if (vec) k_transpose_xy<ADD, true><<<(unsigned)blocks, 256, 0, st>>>(src, src_stride, nx, ny, nz, tiles_x, tiles_y, dst);
+    else     k_transpose_xy<ADD, false><<<(unsigned)blocks, 256, 0, st>>>(src, src_stride, nx, ny, nz, tiles_x, tiles_y, dst);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
 
 static int fill_params(const gsvox_grid* g, const gsvox_cone_geometry* c, const float* angles_host, int32_t B,
                        ProjParams* P)
@@ -286,9 +338,8 @@ extern "C" int gsvox_project_forward(const float* vol, int64_t vol_stride, const
     if (!vol || !scratch || !drr || (vol_stride != 0 && vol_stride != V)) return GSVOX_EINVAL;
     P.vol_stride = vol_stride;
     cudaStream_t st = (cudaStream_t)stream;
-    dim3 tg((P.n[0] + 31) / 32, (P.n[1] + 31) / 32, (unsigned)(P.n[2] * B));
-    k_transpose_xy<false><<<tg, 256, 0, st>>>(vol, vol_stride, P.n[0], P.n[1], P.n[2], (float*)scratch);
-    GSVOX_CUDA(cudaGetLastError());
+    rc = launch_transpose<false>(vol, vol_stride, P.n[0], P.n[1], P.n[2], B, (float*)scratch, st);
+    if (rc != GSVOX_OK) return rc;
     dim3 pg((P.nu + kProjThreads - 1) / kProjThreads, (unsigned)P.nv, (unsigned)B);
     k_project_forward<<<pg, kProjThreads, 0, st>>>(vol, (const float*)scratch, P, drr);
     GSVOX_CUDA(cudaGetLastError());
@@ -317,8 +368,5 @@ extern "C" int gsvox_project_backward(const float* grad_drr, const gsvox_grid* g
     else                       k_project_backward<2><<<pg, kProjThreads, 0, st>>>(grad_drr, P, grad_vol, (float*)scratch);
     GSVOX_CUDA(cudaGetLastError());
     // fold the y-fastest scratch back: grad_vol[z][y][x] += scratch[z][x][y]  (a transpose with nx, ny swapped)
-    dim3 tg((P.n[1] + 31) / 32, (P.n[0] + 31) / 32, (unsigned)(P.n[2] * B));
-    k_transpose_xy<true><<<tg, 256, 0, st>>>((const float*)scratch, V, P.n[1], P.n[0], P.n[2], grad_vol);
-    GSVOX_CUDA(cudaGetLastError());
-    return GSVOX_OK;
+    return launch_transpose<true>((const float*)scratch, V, P.n[1], P.n[0], P.n[2], B, grad_vol, st);
 }
