@@ -150,6 +150,36 @@ k_warp_backward(const float* __restrict__ iref, const float* __restrict__ dvf, c
     const bool taken = __shfl_up_sync(full, (int)take_next, 1) && (lane > 0);       // my left add is done by lane-1
     if (!ok) g = 0.f;                                               // non-finite displacement: zero gradients
     float gx = 0.f, gy = 0.f, gz = 0.f;
+    // all 32 cells wholly inside the grid (every warp but those at the rim): 32-bit offsets from one base, no bounds tests
+    const bool interior = ok && (unsigned)cx < (unsigned)(wg.nx - 1) && (unsigned)cy < (unsigned)(wg.ny - 1) &&
+                          (unsigned)cz < (unsigned)(wg.nz - 1);
+    if (__all_sync(full, interior)) {
+        const unsigned base = ((unsigned)cz * wg.ny + cy) * wg.nx + cx;
+        const float* ip = iref + base;
+        float* gp = giref + base;
+        const int sy_ = wg.nx, sz_ = wg.nx * wg.ny;
+        #pragma unroll
+        for (int az = 0; az < 2; ++az) {
+            const float wz = az ? fz : 1.f - fz, sz = az ? 1.f : -1.f;
+            #pragma unroll
+            for (int ay = 0; ay < 2; ++ay) {
+                const float wy = ay ? fy : 1.f - fy, sy = ay ? 1.f : -1.f;
+                const int off = az * sz_ + ay * sy_;
+                const float v0 = __ldg(ip + off), v1 = __ldg(ip + off + 1);
+                const float gwyz = g * wy * wz;
+                const float a0 = gwyz * (1.f - fx);
+                float a1 = gwyz * fx;
+                const float na0 = __shfl_down_sync(full, a0, 1);
+                if (take_next) a1 += na0;
+                if (!taken) red_add(gp + off, a0);
+                red_add(gp + off + 1, a1);
+                const float lin = fmaf(fx, v1 - v0, v0);
+                gx = fmaf(wy * wz, v1 - v0, gx);
+                gy = fmaf(sy * wz, lin, gy);
+                gz = fmaf(wy * sz, lin, gz);
+            }
+        }
+    } else
     #pragma unroll
     for (int az = 0; az < 2; ++az) {
         const int zz = cz + az;
