@@ -108,3 +108,14 @@ def test_project_full_size_paper_geometry(pkg):
     keeps the numpy oracle to under a minute."""
     ratio, rel = parity(pkg, gsvox_inputs.project_case(batch=2))
     print("project full size: forward err/tol %.3f, backward rel L2 %.3e" % (ratio, rel))
+
+
+@pytest.mark.parametrize("dims", [(12, 8, 1100), (9, 10, 1100)])
+def test_project_many_slices(pkg, dims):
+    """nz x B = 70 400 (b, z) slices: the transposes index slices on a 1-D grid (a gridDim.z of slices would stop
+    at 65 535).  (12, 8, .) takes the float4 transpose, (9, 10, .) the scalar one."""
+    B = 64
+    angles = np.linspace(0.0, 2 * np.pi, B, endpoint=False) + 0.05
+    case = gsvox_inputs.project_case(batch=B, dims=dims, spacing=(3.0, 3.0, 0.25), nu=10, nv=12, du=8.0, dv=30.0,
+                                     sad=150.0, sdd=220.0, seed=57, angles=angles)
+    parity(pkg, case)
