@@ -76,39 +76,42 @@ __device__ __forceinline__ float warp_sample(const float* __restrict__ iref, con
     return acc;
 }
 
-// VPT consecutive x per thread (4: 128-bit loads of d and a 128-bit store; needs nx % 4 == 0).
-// 32-bit index arithmetic: V < 2^31 is checked on the host.
-template <int VPT>
+// A warp takes 32 * kWarpNJ consecutive voxels; lane l handles voxels l, l + 32, ... of them, so every load, store and
+// corner gather of a warp touches neighbouring addresses (4 consecutive x per thread with 128-bit loads strides the
+// gathers by 16 bytes, 16 sectors per gather instead of 5: 0.37 ms against 0.30 ms at 256x256x128, B = 8).  32-bit index
+// arithmetic: V < 2^31 is checked on the host.
+constexpr int kWarpNJ = 4;
 __global__ void __launch_bounds__(kWarpThreads)
 k_warp_forward(const float* __restrict__ iref, const float* __restrict__ dvf, WarpGrid wg, int B,
                float* __restrict__ out)
 {
     const unsigned V = (unsigned)wg.nx * wg.ny * wg.nz;
-    const unsigned v = (blockIdx.x * kWarpThreads + threadIdx.x) * VPT;
+    const unsigned gwarp = (blockIdx.x * kWarpThreads + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const unsigned v0 = gwarp * (32u * kWarpNJ) + lane;
     const int b = blockIdx.y;
-    if (v >= V) return;
-    const unsigned row = v / (unsigned)wg.nx;
-    const int x = (int)(v - row * wg.nx), z = (int)(row / (unsigned)wg.ny), y = (int)(row - (unsigned)z * wg.ny);
+    if (v0 >= V) return;
+    const unsigned row = v0 / (unsigned)wg.nx;
+    int x = (int)(v0 - row * wg.nx), z = (int)(row / (unsigned)wg.ny), y = (int)(row - (unsigned)z * wg.ny);
     const float* d = dvf + (size_t)b * 3 * V;
-    float dx[VPT], dy[VPT], dz[VPT], res[VPT];
-    if (VPT == 4) {
-        const float4 a = __ldcs(reinterpret_cast<const float4*>(d + v));
-        const float4 c = __ldcs(reinterpret_cast<const float4*>(d + V + v));
-        const float4 e = __ldcs(reinterpret_cast<const float4*>(d + 2 * (size_t)V + v));
-        dx[0] = a.x; dx[VPT - 1] = a.w; dy[0] = c.x; dy[VPT - 1] = c.w; dz[0] = e.x; dz[VPT - 1] = e.w;
-        if (VPT > 2) { dx[1] = a.y; dx[2] = a.z; dy[1] = c.y; dy[2] = c.z; dz[1] = e.y; dz[2] = e.z; }
-    } else {
-        dx[0] = __ldcs(d + v); dy[0] = __ldcs(d + V + v); dz[0] = __ldcs(d + 2 * (size_t)V + v);
+    float* o = out + (size_t)b * V;
+    float dx[kWarpNJ], dy[kWarpNJ], dz[kWarpNJ];
+    #pragma unroll
+    for (int j = 0; j < kWarpNJ; ++j) {
+        const unsigned v = v0 + 32u * j;
+        const bool live = v < V;
+        dx[j] = live ? __ldcs(d + v) : 0.f; dy[j] = live ? __ldcs(d + V + v) : 0.f; dz[j] = live ? __ldcs(d + 2 * (size_t)V + v) : 0.f;
     }
     #pragma unroll
-    for (int j = 0; j < VPT; ++j) {
-        int cx, cy, cz; float fx, fy, fz;
-        const bool ok = warp_cell(dx[j], dy[j], dz[j], wg, x + j, y, z, cx, cy, cz, fx, fy, fz);
-        res[j] = ok ? warp_sample(iref, wg, cx, cy, cz, fx, fy, fz) : 0.f;
+    for (int j = 0; j < kWarpNJ; ++j) {
+        const unsigned v = v0 + 32u * j;
+        if (v < V) {
+            int cx, cy, cz; float fx, fy, fz;
+            const bool ok = warp_cell(dx[j], dy[j], dz[j], wg, x, y, z, cx, cy, cz, fx, fy, fz);
+            __stcs(o + v, ok ? warp_sample(iref, wg, cx, cy, cz, fx, fy, fz) : 0.f);
+        }
+        x += 32;
+        while (x >= wg.nx) { x -= wg.nx; if (++y >= wg.ny) { y = 0; ++z; } }
     }
-    float* o = out + (size_t)b * V + v;
-    if (VPT == 4) __stcs(reinterpret_cast<float4*>(o), make_float4(res[0], res[1 % VPT], res[2 % VPT], res[3 % VPT]));
-    else __stcs(o, res[0]);
 }
 
 __device__ __forceinline__ void red_add(float* addr, float v)
@@ -237,11 +240,9 @@ extern "C" int gsvox_warp_forward(const float* iref, const float* dvf, const gsv
     if (rc != GSVOX_OK) return rc;
     if (!iref || !dvf || !out) return GSVOX_EINVAL;
     const long long V = (long long)wg.nx * wg.ny * wg.nz;
-    const bool vec = (wg.nx % 4 == 0) && ((((uintptr_t)dvf | (uintptr_t)out) & 15) == 0);
-    const long long items = vec ? V / 4 : V;
-    dim3 gridDim((unsigned)((items + kWarpThreads - 1) / kWarpThreads), (unsigned)B);
-    if (vec) k_warp_forward<4><<<gridDim, kWarpThreads, 0, (cudaStream_t)stream>>>(iref, dvf, wg, B, out);
-    else     k_warp_forward<1><<<gridDim, kWarpThreads, 0, (cudaStream_t)stream>>>(iref, dvf, wg, B, out);
+    const long long per_cta = (long long)kWarpThreads * kWarpNJ;
+    dim3 gridDim((unsigned)((V + per_cta - 1) / per_cta), (unsigned)B);
+    k_warp_forward<<<gridDim, kWarpThreads, 0, (cudaStream_t)stream>>>(iref, dvf, wg, B, out);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }
