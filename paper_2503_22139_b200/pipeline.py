@@ -37,6 +37,19 @@ class Stage3Step:
         self.g_coef = f(batch, self.L, 3)
         self.scratch = B_._project_scratch(B_.make_grid(*grid), batch, dev)
         self._saved = None
+        # the four voxelizers are independent: each runs on its own stream so that the small binning kernels of one
+        # overlap the brick kernels of another (the C ABI takes the stream; nothing else changes)
+        self._side = [torch.cuda.Stream(device=dev) for _ in range(self.L)]
+
+    def _fork(self):
+        main = torch.cuda.current_stream()
+        for st in self._side:
+            st.wait_stream(main)
+        return main
+
+    def _join(self, main):
+        for st in self._side:
+            main.wait_stream(st)
 
     def fit(self, ref, levels, slack=1.05):
         """Size the (brick, Gaussian) key buffers for these Gaussians: preprocess once, read the device status
@@ -56,11 +69,14 @@ class Stage3Step:
     def forward(self, ref, levels, coef, angles):
         """ref = (pos, scale, quat, rho[n,1]); levels = [(pos, scale, quat, feat[n,3]), ...]; coef [B,L,3];
         angles: B radians (host).  -> drr [B, nv, nu] (a buffer owned by this object)."""
+        main = self._fork()
+        for i, lv in enumerate(levels):
+            with torch.cuda.stream(self._side[i]):
+                self.plans[i].preprocess(*lv[:3])
+                self.plans[i].forward(lv[3], out=self.e[i])
         self.plan_ref.preprocess(*ref[:3])
         self.plan_ref.forward(ref[3], out=self.iref)
-        for i, lv in enumerate(levels):
-            self.plans[i].preprocess(*lv[:3])
-            self.plans[i].forward(lv[3], out=self.e[i])
+        self._join(main)
         B_.mbc_combine_forward(self.e, coef, out=self.dvf)
         B_.warp_forward(self.iref[0], self.dvf, self.grid, out=self.warped)
         B_.project_forward(self.warped, self.grid, self.geom, angles, out=self.drr, scratch=self.scratch)
@@ -74,6 +90,13 @@ class Stage3Step:
         B_.project_backward(grad_drr, self.grid, self.geom, angles, out=self.g_warped, scratch=self.scratch)
         B_.warp_backward(self.iref[0], self.dvf, self.grid, self.g_warped, grads=(self.g_iref[0], self.g_dvf))
         B_.mbc_combine_backward(self.e, coef, self.g_dvf, grads=(self.g_e, self.g_coef))
-        g_levels = [self.plans[i].backward(lv[3], self.g_e[i]) for i, lv in enumerate(levels)]
+        main = self._fork()
+        g_levels = []
+        for i, lv in enumerate(levels):
+            with torch.cuda.stream(self._side[i]):
+                g_levels.append(self.plans[i].backward(lv[3], self.g_e[i]))
+                for t in g_levels[-1]:
+                    t.record_stream(main)          # allocated on the side stream, consumed on the caller's
         g_ref = self.plan_ref.backward(ref[3], self.g_iref)
+        self._join(main)
         return {"ref": g_ref, "levels": g_levels, "coef": self.g_coef}
