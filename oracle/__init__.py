@@ -215,19 +215,12 @@ def dvf_backward(levels, coef, grid, grad_dvf, kappa=KAPPA):
       dL/de_{i,k}     = sum_b coef[b,i,k] grad_dvf[b,k]      then the voxelizer's analytic backward.
     The C oracle takes fp32 upstream gradients; dL/de is handed over as an exact hi+lo fp32 split
     (the backward is linear in the upstream gradient)."""
-    coef = np.asarray(_f32(coef), dtype=np.float64)
     g = np.asarray(_f32(grad_dvf), dtype=np.float64)
     e = mbc_volumes(levels, grid, kappa)
-    B, L = coef.shape[0], coef.shape[1]
-    grad_coef = np.zeros((B, L, 3))
+    grad_e, grad_coef = mbc_combine_backward(e, coef, g)
     per_level = []
     for i, (p, s, q, f) in enumerate(levels):
-        ge = np.zeros((3,) + e.shape[2:])
-        for b in range(B):
-            for k in range(3):
-                grad_coef[b, i, k] = float(np.sum(g[b, k] * e[i, k]))
-                ge[k] += coef[b, i, k] * g[b, k]
-        hi, lo = _split_f32(ge)
+        hi, lo = _split_f32(grad_e[i])
         a = backward(p, s, q, f, grid, hi, kappa)
         c = backward(p, s, q, f, grid, lo, kappa)
         per_level.append(tuple(x + y for x, y in zip(a, c)))
@@ -239,25 +232,23 @@ def dvf_backward(levels, coef, grid, grad_dvf, kappa=KAPPA):
 # The paper does not say how I_ref is evaluated between voxel centres or outside the volume.
 # Readings (W1-W4): trilinear interpolation of the voxel-centre samples; a corner
 # outside the grid contributes 0 (zero padding, corner by corner); d is in world units like
-# origin/spacing, so the sample position in index units is u_k = i_k + d_k / h_k; the cell index
-# floor(u_k) is decided on t_k = fp32(fp32(d_k) * fp32(1 / h_k)) — one fp32 reciprocal of the spacing, one
-# fp32 multiply (the kernel's precision and operation order: both sides take the integer decision in
-# the same precision), everything after that is fp64; a non-finite displacement, or one of 2^22 voxels
-# or more, yields 0 and zero gradients.  Backward is the exact derivative of the
-# piecewise-trilinear interpolant (kinks at integer u have measure zero).
+# origin/spacing, so the sample position in index units is u_k = i_k + d_k / h_k (the origin cancels);
+# the cell is floor(d_k / h_k) and the interpolation fraction d_k / h_k - floor(d_k / h_k), both in
+# fp64 on the fp32 inputs promoted exactly — the plain reading of Eq. 2, no fp32 step anywhere; a
+# non-finite displacement, or one of 2^22 voxels or more, yields 0 and zero gradients.  Backward is
+# the exact derivative of the piecewise-trilinear interpolant (kinks at integer u have measure zero).
 # --------------------------------------------------------------------------------------------
 def _warp_cells(dvf, spacing, dims):
     """-> integer base corner i0 [B,3,nz,ny,nx] (int64), fraction f [B,3,nz,ny,nx] fp64, finite mask."""
     nx, ny, nz = (int(v) for v in dims)
-    d32 = _f32(dvf).reshape(-1, 3, nz, ny, nx)
-    h32 = _f32(spacing).reshape(3)
-    inv_h32 = (np.float32(1.0) / h32).astype(np.float32)      # 1/h rounded once to fp32 ...
+    d = np.asarray(_f32(dvf), dtype=np.float64).reshape(-1, 3, nz, ny, nx)
+    h = np.asarray(_f32(spacing), dtype=np.float64).reshape(3)
     with np.errstate(invalid="ignore", over="ignore"):
-        t = (d32 * inv_h32[None, :, None, None, None]).astype(np.float32)   # ... then ONE fp32 multiply, as on the device
+        t = d / h[None, :, None, None, None]                   # displacement in voxels, fp64
     finite = np.all(np.isfinite(t), axis=1) & np.all(np.abs(t) < 4194304.0, axis=1)   # |t| < 2^22 voxels
-    t = np.where(finite[:, None], t, np.float32(0))
+    t = np.where(finite[:, None], t, 0.0)
     tf = np.floor(t)
-    frac = (t - tf).astype(np.float64)                         # exact in fp32
+    frac = t - tf
     idx = np.stack(np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij"))   # z,y,x
     base = np.empty(t.shape, dtype=np.int64)
     base[:, 0] = idx[2][None] + tf[:, 0].astype(np.int64)      # x
@@ -330,14 +321,14 @@ def warp_backward(iref, dvf, grid, grad_out):
 #     largest (first of x,y,z on ties), one sample per voxel-centre plane m of that axis, bilinear
 #     interpolation in the plane, corners outside the grid read 0, each sample weighted by the path
 #     length between planes h_a |D| / |D_a|.
-#  P3 per-ray constants (u0, su, v0, sv, weight) are computed in fp64 and rounded to fp32; the
-#     in-plane sample position is the fp32 value u0 + fp32(m * su) (two roundings, no FMA), and the
-#     cell is decided on it — the kernel's precision and order; everything after is fp64.
+#  P3 everything in fp64: per-ray constants (p0, ps, q0, qs, weight), the in-plane sample position
+#     p0 + m ps of plane m, its cell floor(.) and the bilinear fractions.  (The interpolant is continuous
+#     in the position, so an implementation that rounds the position differs by |grad I| x its rounding.)
 #  P4 backward is the exact transpose (the projector is linear in the volume); no geometry gradients.
 # --------------------------------------------------------------------------------------------
 def cone_rays(grid, geom, angle):
     """geom = dict(sad, sdd, nu, nv, du, dv, off_u, off_v, iso[3]).  -> per-pixel [nv, nu] arrays:
-    dominant axis a, and fp32 (p0, ps, q0, qs, weight) for the two in-plane axes (b, c) = the axes
+    dominant axis a, and fp64 (p0, ps, q0, qs, weight) for the two in-plane axes (b, c) = the axes
     other than a in ascending order, all in voxel index units."""
     o, h, dims = _grid(grid)
     o = o.astype(np.float64); h = h.astype(np.float64)
@@ -369,7 +360,7 @@ def cone_rays(grid, geom, angle):
             wa = h[ax] * norm / np.abs(Da)
         p0[sel], ps[sel], q0[sel], qs[sel], w[sel] = p0a[sel], psa[sel], q0a[sel], qsa[sel], wa[sel]
     for k, v in (("p0", p0), ("ps", ps), ("q0", q0), ("qs", qs), ("w", w)):
-        out[k] = v.astype(np.float32)
+        out[k] = v
     return out
 
 
@@ -387,14 +378,13 @@ def _project_terms(grid, geom, angle):
             continue
         b, c = others[ax]
         p0, ps, q0, qs = (rays[k][sel] for k in ("p0", "ps", "q0", "qs"))
-        w = rays["w"][sel].astype(np.float64)
+        w = rays["w"][sel]
         for m in range(n[ax]):
-            fm = np.float32(m)
-            p = (p0 + (fm * ps).astype(np.float32)).astype(np.float32)      # two fp32 roundings, no FMA (P3)
-            q = (q0 + (fm * qs).astype(np.float32)).astype(np.float32)
+            p = p0 + m * ps                                                 # fp64 (P3)
+            q = q0 + m * qs
             good = (np.abs(p) < 4194304.0) & (np.abs(q) < 4194304.0)
             pf, qf = np.floor(np.where(good, p, 0)), np.floor(np.where(good, q, 0))
-            fp_, fq = (np.where(good, p, 0) - pf).astype(np.float64), (np.where(good, q, 0) - qf).astype(np.float64)
+            fp_, fq = np.where(good, p, 0) - pf, np.where(good, q, 0) - qf
             ib, ic = pf.astype(np.int64), qf.astype(np.int64)
             idx, wt = [], []
             for db in (0, 1):

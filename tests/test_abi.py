@@ -81,6 +81,7 @@ def test_product_does_not_import_the_oracle():
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith((".py", ".c", ".h")):
             text = open(os.path.join(ROOT, "oracle", f)).read()
-            assert "paper_2503_22139_b200" not in text.replace("(paper_2503_22139_b200", "").replace(
-                "paper_2503_22139_b200)", "").replace("paper_2503_22139_b200/", "") or True
+            # the oracle may NAME the product package in prose (its header says who may import what); it may not
+            # load it: no import, no ctypes/dlopen of the product library
+            assert "libgsvox.so" not in text and "binding" not in text, f
             assert not re.search(r"^\s*(import|from)\s+paper_2503_22139_b200\b", text, flags=re.M), f

@@ -193,3 +193,54 @@ def test_backward_against_central_differences_frozen_support():
                 val = fd(fun0, base, idx, eps)
                 got = per0[i][order[names[which]]][idx]
                 assert val == pytest.approx(got, rel=5e-5, abs=5e-6), (i, names[which], idx)
+
+
+def test_mbc_combine_backward_pinned_by_differences_adjoint_and_library_contraction():
+    """oracle.mbc_combine_backward (the reference of gsvox_mbc_combine_backward, the batch path) against
+    things other than itself: (i) mbc_combine is bilinear, so central differences of L = <g, combine(e, coef)>
+    are exact up to rounding; (ii) the adjoint identities <g, combine(e, c)> = <dL/de, e> = <dL/dcoef, c>;
+    (iii) numpy's tensor contraction of the same index pattern d[b,k] = sum_i c[b,i,k] e[i,k] (PAPER.md:58-61,
+    Eq. 3; :141 for the index meaning); (iv) zero pattern: coefficient (b,i,k) sees only e[i,k] and g[b,k]."""
+    rng = np.random.default_rng(77)
+    B, L, shp = 3, 4, (3, 4, 5)
+    e = rng.standard_normal((L, 3) + shp)
+    coef = rng.standard_normal((B, L, 3)).astype(np.float32)
+    g = rng.standard_normal((B, 3) + shp)
+    ge, gc = oracle.mbc_combine_backward(e, coef, g)
+    assert ge.shape == e.shape and gc.shape == (B, L, 3)
+    loss = lambda ee, cc: float(np.sum(g * oracle.mbc_combine(ee, cc)))
+    base = loss(e, coef)
+    # (ii)
+    assert float(np.sum(ge * e)) == pytest.approx(base, rel=1e-12)
+    assert float(np.sum(gc * coef.astype(np.float64))) == pytest.approx(base, rel=1e-12)
+    # (i) bilinear => a central difference with any step is exact
+    for idx in [(0, 0, 0), (2, 3, 1), (1, 2, 2)]:
+        cp, cm = coef.copy(), coef.copy()
+        cp[idx] += 0.5; cm[idx] -= 0.5
+        assert loss(e, cp) - loss(e, cm) == pytest.approx(gc[idx], rel=1e-11, abs=1e-12)
+    for idx in [(0, 0, 0, 0, 0), (3, 2, 2, 3, 4), (1, 1, 0, 2, 1)]:
+        ep, em = e.copy(), e.copy()
+        ep[idx] += 0.5; em[idx] -= 0.5
+        assert loss(ep, coef) - loss(em, coef) == pytest.approx(ge[idx], rel=1e-11, abs=1e-12)
+    # (iii)
+    c64 = coef.astype(np.float64)
+    assert np.allclose(oracle.mbc_combine(e, coef), np.einsum("bik,ikzyx->bkzyx", c64, e), rtol=1e-13, atol=1e-13)
+    assert np.allclose(ge, np.einsum("bik,bkzyx->ikzyx", c64, g), rtol=1e-13, atol=1e-13)
+    assert np.allclose(gc, np.einsum("bkzyx,ikzyx->bik", g, e), rtol=1e-13, atol=1e-13)
+    # (iv)
+    g1 = np.zeros_like(g); g1[1, 2] = g[1, 2]
+    ge1, gc1 = oracle.mbc_combine_backward(e, coef, g1)
+    mask = np.zeros((B, L, 3), bool); mask[1, :, 2] = True
+    assert np.all(gc1[~mask] == 0.0) and np.all(gc1[mask] != 0.0)
+    assert np.all(ge1[:, :2] == 0.0) and np.all(ge1[:, 2] != 0.0)
+
+
+def test_dvf_backward_goes_through_mbc_combine_backward():
+    """dvf_backward's coefficient gradient IS mbc_combine_backward's on the voxelized MBC volumes (so the pins of
+    dvf_backward above — closed form, Euler identities, central differences — also hold it in place)."""
+    case = small_case()
+    lv, _ = case.levels()
+    g = case.grad_dvf()
+    gc, _ = oracle.dvf_backward(lv, case.coef, case.grid, g)
+    _, gc2 = oracle.mbc_combine_backward(oracle.mbc_volumes(lv, case.grid), case.coef, g)
+    assert np.array_equal(gc, gc2)

@@ -7,6 +7,7 @@ import pytest
 
 import gsvox_inputs
 import oracle
+from parity_util import per_row_worst
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -64,6 +65,7 @@ def test_voxelizer_random_cases(pkg, seed):
     for name, a, b in zip("wpsq", grads, refs):
         if np.linalg.norm(b) > 1e-12:
             assert rel_l2(a, b) <= 1e-4, (seed, name, rel_l2(a, b))
+            assert per_row_worst(a, b)[0] <= 1.0, (seed, name, per_row_worst(a, b))
         else:
             assert np.abs(a).max() <= 1e-6, (seed, name)
 

@@ -9,6 +9,7 @@ import pytest
 
 import gsvox_inputs
 import oracle
+from parity_util import check_grad_groups, fmt
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -56,14 +57,16 @@ def check_forward(out, ref):
     return err, tol
 
 
-def check_grads(grads, refs):
-    rels = {}
-    for name, a, b in zip(("w", "p", "s", "q"), grads, refs):
-        nb = np.linalg.norm(b)
-        rel = np.linalg.norm(a.astype(np.float64) - b) / nb if nb > 0 else np.abs(a).max()
-        rels[name] = rel
-        assert rel <= GRAD_REL, "grad %s rel L2 %.3e > %.1e" % (name, rel, GRAD_REL)
-    return rels
+def check_grads(grads, refs, case=None, label=""):
+    """north_star's group criterion (relative L2 <= 1e-4 per group) and the per-Gaussian bound of parity_util."""
+    describe = None
+    if case is not None and case.n > 0:
+        def describe(i):
+            box = oracle.geometry(case.pos[i:i + 1], case.scale[i:i + 1], case.quat[i:i + 1], case.grid)["box"][0]
+            return "pos %s scale %s box %s" % (case.pos[i].tolist(), case.scale[i].tolist(), box.tolist())
+    res = check_grad_groups(("w", "p", "s", "q"), grads, refs, tol=GRAD_REL, describe=describe, label=label)
+    print("%s gradients: %s" % (label or (case.name if case is not None else ""), fmt(res)))
+    return {k: v[0] for k, v in res.items()}
 
 
 def check_geometry_and_bins(plan, case):
@@ -128,7 +131,7 @@ def full_parity(pkg, case, **kw):
     ref = oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid)
     check_forward(out, ref)
     refs = oracle.backward(case.pos, case.scale, case.quat, case.weight, case.grid, g)
-    check_grads(grads, refs)
+    check_grads(grads, refs, case)
     return plan
 
 
@@ -210,7 +213,7 @@ def test_degenerate_empty_and_outside(pkg):
     ref = oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid)
     check_forward(out, ref)
     refs = oracle.backward(case.pos, case.scale, case.quat, case.weight, case.grid, g)
-    check_grads(grads, refs)
+    check_grads(grads, refs, case)
     for a in grads:
         assert np.isfinite(a).all() and not a[1:8].any()
 

@@ -8,6 +8,7 @@ import pytest
 
 import gsvox_inputs
 import oracle
+from parity_util import check_grad_groups, fmt
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -62,9 +63,9 @@ def parity(pkg, case, backward=True):
     rels = {}
     if backward:
         refs = oracle.splat_backward(case.pos, case.scale, case.quat, case.rho, case.geom, case.angles, g)
-        for name, a, b in zip(("rho", "pos", "scale", "quat"), grads, refs):
-            rels[name] = rel_l2(a.reshape(b.shape), b)
-            assert rels[name] <= GRAD_REL, "splat grad %s rel L2 %.3e" % (name, rels[name])
+        res = check_grad_groups(("rho", "pos", "scale", "quat"), grads, refs, tol=GRAD_REL, label="splat " + case.name)
+        print("splat %s gradients: %s" % (case.name, fmt(res)))
+        rels = {k: v[0] for k, v in res.items()}
     return err / tol, rels
 
 
@@ -142,10 +143,9 @@ def test_splat_full_size_sampled_pixels(pkg):
         worst = max(worst, float(np.abs(got - ref).max())); peak = max(peak, float(np.abs(ref).max()))
     assert worst <= FWD_REL * peak + FWD_ABS, (worst, peak)
     refs = oracle.splat_backward(case.pos, case.scale, case.quat, case.rho, case.geom, case.angles, g, pixels=pix)
-    rels = {}
-    for name, a, b in zip(("rho", "pos", "scale", "quat"), grads, refs):
-        rels[name] = rel_l2(a.reshape(b.shape), b)
-        assert rels[name] <= GRAD_REL, (name, rels[name])
+    res = check_grad_groups(("rho", "pos", "scale", "quat"), grads, refs, tol=GRAD_REL, label="splat full size")
+    print("splat full size gradients: %s" % fmt(res))
+    rels = {k: v[0] for k, v in res.items()}
     print("splat full size: forward err/tol %.3f, grads %s, pairs %.3e keys %.3e" %
           (worst / (FWD_REL * peak + FWD_ABS), rels, st["pairs"], st["keys_needed"]))
 

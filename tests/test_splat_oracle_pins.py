@@ -171,3 +171,84 @@ def test_autograd_gradients_against_central_differences_and_invariants():
             return loss(*args)
         d1 = (at(eps) - at(-eps)) / (2 * eps); d2 = (at(2 * eps) - at(-2 * eps)) / (4 * eps)
         assert (4 * d1 - d2) / 3 == pytest.approx(grad[idx], rel=2e-5, abs=1e-7)
+
+
+def test_sampled_backward_equals_the_full_backward_on_a_masked_upstream_gradient():
+    """splat_backward(pixels=...) (what the full-size GPU parity uses) = the full backward — pinned above by
+    central differences — with the upstream gradient zeroed outside the listed pixels.  kappa = 3: live boxes,
+    Gaussians clipped by the detector edge and Gaussians whose box holds none of the sampled pixels included."""
+    rng = np.random.default_rng(8)
+    n = 12
+    pos = f32(rng.uniform(-60, 60, (n, 3))); scale = f32(rng.uniform(2, 9, (n, 3)))
+    quat = f32(rng.standard_normal((n, 4))); rho = f32(rng.standard_normal(n))
+    angles = [0.3, 1.9, 4.4]
+    g = rng.standard_normal((3, GEOM["nv"], GEOM["nu"])).astype(np.float32)
+    pix = [(int(rng.integers(0, 3)), int(rng.integers(0, GEOM["nu"])), int(rng.integers(0, GEOM["nv"]))) for _ in range(400)]
+    pix = sorted(set(pix))
+    gm = np.zeros_like(g)
+    for b, iu, iv in pix:
+        gm[b, iv, iu] = g[b, iv, iu]
+    full = oracle.splat_backward(pos, scale, quat, rho, GEOM, angles, gm)
+    samp = oracle.splat_backward(pos, scale, quat, rho, GEOM, angles, g, pixels=pix)
+    assert np.abs(full[0]).max() > 0
+    for a, b in zip(full, samp):
+        assert np.allclose(a, b, rtol=1e-12, atol=1e-14 * max(1.0, np.abs(a).max()))
+    # and the forward sampler agrees with the image
+    img = oracle.splat_forward(pos, scale, quat, rho, GEOM, angles)
+    for bsel in range(3):
+        sel = [(iu, iv) for (b, iu, iv) in pix if b == bsel]
+        vals = oracle.splat_forward_at(pos, scale, quat, rho, GEOM, np.float32(angles[bsel]), sel)
+        assert np.allclose(vals, [img[bsel, iv, iu] for iu, iv in sel], rtol=1e-13, atol=1e-15)
+
+
+def test_autograd_gradients_against_central_differences_with_live_3_sigma_boxes():
+    """kappa = 3 (the product's cutoff): the boxes are strictly inside the detector and live (pixels outside
+    contribute nothing), the support is frozen (R6) — asserted: no box changes under any perturbation applied —
+    and Richardson central differences of the oracle's own forward match its autograd backward."""
+    rng = np.random.default_rng(16)
+    n = 2
+    q64 = lambda a: f32(np.round(np.asarray(a) * 64) / 64)
+    angles = [0.3, 1.9]
+
+    def boxes(p, s, q, r):
+        out = []
+        for a in angles:
+            t = oracle.splat_terms(*[oracle.splat._t(x) for x in (p, s, q)], oracle.splat._t(r).reshape(-1), GEOM, a)
+            assert bool(t[7].all())
+            out.append(t[6].numpy().copy())
+        return np.stack(out)
+
+    eps = 2.0 ** -10
+    for attempt in range(200):                                # deterministic search for a set whose boxes stay put
+        pos = q64(rng.uniform(-8, 8, (n, 3))); scale = q64(rng.uniform(1.5, 3.0, (n, 3)))
+        quat = q64(rng.standard_normal((n, 4))); rho = q64(rng.uniform(0.3, 1, n))
+        box0 = boxes(pos, scale, quat, rho)
+        ok = (box0[..., 0] > 0).all() and (box0[..., 1] > 0).all() and (box0[..., 2] < GEOM["nu"] - 1).all() \
+            and (box0[..., 3] < GEOM["nv"] - 1).all()
+        for arr in (pos, scale, quat):
+            for idx in np.ndindex(*arr.shape):
+                for e in (eps, -eps, 2 * eps, -2 * eps):
+                    a2 = arr.copy(); a2[idx] += e
+                    args = [a2 if x is arr else x for x in (pos, scale, quat, rho)]
+                    ok = ok and np.array_equal(boxes(*args), box0)
+        if ok:
+            break
+    assert ok, "no frozen-box configuration found"
+    area = (box0[..., 2] - box0[..., 0] + 1) * (box0[..., 3] - box0[..., 1] + 1)
+    assert area.max() < 0.5 * GEOM["nu"] * GEOM["nv"]        # the cutoff is live: each box is a small part of the detector
+    g = rng.standard_normal((2, GEOM["nv"], GEOM["nu"])).astype(np.float32)
+    gr, gp, gs, gq = oracle.splat_backward(pos, scale, quat, rho, GEOM, angles, g)
+
+    def loss(p, s, q, r):
+        return float((oracle.splat_forward(p, s, q, r, GEOM, angles) * g).sum())
+    for arr, grad in [(pos, gp), (scale, gs), (quat, gq), (rho, gr)]:
+        fd = np.zeros_like(grad)
+        for idx in np.ndindex(*arr.shape):
+            def at(e):
+                a2 = arr.copy(); a2[idx] += e
+                args = [a2 if x is arr else x for x in (pos, scale, quat, rho)]
+                return loss(*args)
+            d1 = (at(eps) - at(-eps)) / (2 * eps); d2 = (at(2 * eps) - at(-2 * eps)) / (4 * eps)
+            fd[idx] = (4 * d1 - d2) / 3
+        err = np.linalg.norm(fd - grad) / np.linalg.norm(grad)
+        assert err < 2e-5, err
