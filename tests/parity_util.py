@@ -4,9 +4,11 @@ Two gradient criteria:
   * the pass criterion of record, north_star's: relative L2 error <= 1e-4 per parameter group over ALL Gaussians;
   * a per-Gaussian bound on top, because a group norm over 5e5 Gaussians cannot see a few hundred completely
     wrong rows (one broken key class, one brick-edge case):
-        |g_gpu,i - g_ref,i|_2  <=  PER_REL |g_ref,i|_2 + PER_ABS median_j |g_ref,j|_2      for every Gaussian i,
+        |g_gpu,i - g_ref,i|_2  <=  PER_REL |g_ref,i|_2 + PER_ABS rms_j |g_ref,j|_2      for every Gaussian i,
     PER_REL = 1e-3, PER_ABS = 1e-4 (the absolute term carries Gaussians whose gradient is a near-cancelling sum:
-    fp32 accumulation error scales with the terms, not with their sum).  The worst offender is reported.
+    fp32 accumulation error scales with the terms, not with their sum; the scale is the root mean square of the
+    row norms, not their median: 70 % of config 4's Gaussians are isotropic, their dL/dq is exactly 0 in the
+    oracle and so is the median).  The worst offender is reported.
 """
 import numpy as np
 
@@ -21,7 +23,7 @@ def rel_l2(a, b):
 
 
 def per_row_worst(a, b):
-    """-> (worst ratio err_i / (PER_REL |b_i| + PER_ABS median|b|), its row index, err_i, |b_i|)."""
+    """-> (worst ratio err_i / (PER_REL |b_i| + PER_ABS rms|b|), its row index, err_i, |b_i|)."""
     b = np.asarray(b, dtype=np.float64)
     a = np.asarray(a, dtype=np.float64).reshape(b.shape)
     if b.size == 0:
@@ -30,9 +32,8 @@ def per_row_worst(a, b):
     a2 = a.reshape(b.shape[0], -1)
     nb = np.linalg.norm(b2, axis=1)
     err = np.linalg.norm(a2 - b2, axis=1)
-    live = nb > 0
-    med = float(np.median(nb[live])) if live.any() else 0.0
-    allow = PER_REL * nb + PER_ABS * med
+    rms = float(np.sqrt(np.mean(nb * nb)))
+    allow = PER_REL * nb + PER_ABS * rms
     ratio = np.where(allow > 0, err / np.where(allow > 0, allow, 1.0), np.where(err > 0, np.inf, 0.0))
     i = int(np.argmax(ratio))
     return float(ratio[i]), i, float(err[i]), float(nb[i])
