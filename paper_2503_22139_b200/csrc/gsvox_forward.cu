@@ -18,6 +18,7 @@
 // take the direct path, one EX2 per voxel: the recurrence would lose accuracy and could
 // underflow there (error budget).  Direct keys are class 0 of the brick's
 // key range, so which path a staged key takes is known from bin_start, not from its data.
+#include <cstdlib>
 #include "gsvox_internal.cuh"
 
 namespace gsvox {
@@ -236,6 +237,249 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
     }
 }
 
+
+// ==========================================================================================
+// C = 1 fast path: one WARP per brick, two rows per thread.
+//
+// What binds k_forward above is not arithmetic but operand delivery: every key costs each of the brick's two
+// warps ~21 words through LDS, and a warp-wide LDS.128 occupies the SM's one shared-memory return path for
+// 2-4 cycles whether or not all lanes read the same address (ncu: l1tex 85-94 % busy, mio_throttle the
+// top stall; a first pair-of-keys kernel that halved the instruction count ran SLOWER for that reason).
+// Here a key's 20 words are loaded once per brick: the warp covers all 64 rows, thread (y, z) owning the
+// rows (y, z) and (y, z + 4).  The row setup runs once for both rows in packed f32x2 instructions whose
+// key operands are scalar registers broadcast to both halves (SASS: the .F32 operand form), so the staged
+// record needs no interleaving; the three exponents per row then feed the centre-out recurrence of
+// k_forward.  Per key: 5 LDS.128, ~13 setup + 2 x 16 row instructions, 6 EX2; the FP32 pipe is the limit
+// (packed instructions take two pipe cycles).  A half (4 z-layers) no row of which lies in the box skips
+// its recurrence.  The batch's 64-byte records (and weights) arrive by cp.async, issued one batch ahead;
+// single-warp CTAs need no __syncthreads, 32 of them are resident per SM.
+// "Slow" keys (c stored negative) take a scalar route: direct-exponential keys (A > 1, class 0) and keys
+// whose first ratio 2^Lf, 2^Lb could overflow on some row of the brick (A (1 + 2 max|t3|) >= 120: the fast
+// path has no clamp — such rows hold nothing but zeros, yet inf * 0 must not be formed).
+// ==========================================================================================
+constexpr int kB1Batch = 32;
+constexpr int kB1Words = 20;                        // staged record; also the stride of the raw copy (16 + weight, padded): conflict-free 128-bit per-lane access
+
+__device__ __forceinline__ void cp_async16(uint32_t saddr, const void* g)
+{ asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" :: "r"(saddr), "l"(g) : "memory"); }
+__device__ __forceinline__ void cp_async4(uint32_t saddr, const void* g)
+{ asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(saddr), "l"(g) : "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// staged record (floats):  0 cx3  1 ncy  2 ncz  3 negA | 4 l01  5 l02  6 l12  7 nD1 | 8 nD2  9 +-c  10 mask(z 0..3)  11 mask(z 4..7)
+//                          12..19  w * [k inside the box in x] (fast keys: * c^{0,0,1,1,3,3,6,6}) in the order k = 3,4, 2,5 | 1,6, 0,7
+//                          c < 0 marks a slow key
+// cx3 = 3 - cx, ncy = -cy, ncz = -cz, l01 = +l01, l02 = +l02:  t3 = 3 - xs = cx3 + l01 dy + l02 dz.
+
+// One row from its two exponents: E3 (value at k = 3) and Lf = E(4) - E(3).  The row is the parabola
+// E(k) = E3 + (k - 3) Lf - A (k - 3)(k - 4), so  G(k) = G3 rho^(k-3) c^((k-3)(k-4)/2),  rho = 2^Lf, c = 2^-2A:
+// a plain geometric sequence times a factor that depends on the key and k only — staged into the weights
+// (w'_k = w [k in box] c^{0,0,1,1,3,3,6,6} in the centre-out order).  One FMUL + three FMUL2 for eight values.
+// G3 rho^(k-3) never overflows for A <= 1: its exponent is Es - A (t3 +- ...)^2 + 12 A <= 12.
+__device__ __forceinline__ void recur_accumulate(float E3, float Lf, const float4 wa, const float4 wb, float (&acc)[8])
+{
+    const float G3 = ex2f(E3), rf = ex2f(Lf), rb = ex2f(-Lf);
+    const float G4 = G3 * rf;
+    const f32x2 R = pk2(rb, rf);
+    const f32x2 P0 = pk2(G3, G4);
+    const f32x2 P1 = mul2(P0, R);
+    const f32x2 P2 = mul2(P1, R);
+    const f32x2 P3 = mul2(P2, R);
+    fma2_acc(acc[0], acc[1], P0, pk2(wa.x, wa.y));
+    fma2_acc(acc[2], acc[3], P1, pk2(wa.z, wa.w));
+    fma2_acc(acc[4], acc[5], P2, pk2(wb.x, wb.y));
+    fma2_acc(acc[6], acc[7], P3, pk2(wb.z, wb.w));
+}
+
+// One row of a slow key, scalar.
+__device__ __forceinline__ void eval_row_slow(const float* __restrict__ r, bool inrow, float fy, float fz, float (&acc)[8])
+{
+    const float dy = fy + r[1], dz = fz + r[2];
+    const float negA = r[3];
+    const float u1 = fmaf(r[6], dz, dy);
+    const float t3 = fmaf(r[5], dz, fmaf(r[4], dy, r[0]));
+    float Es = fmaf(r[8] * dz, dz, (r[7] * u1) * u1);
+    Es = inrow ? Es : -1.0e30f;
+    float G[8];                                                     // order 3,4,2,5,1,6,0,7
+    if (-negA > kRecurrenceMaxA) {
+        #pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float tl = t3 - (float)j, th = t3 + (float)(1 + j);          // (3 - j) - xs, (4 + j) - xs
+            G[2 * j] = ex2f(fmaf(negA * tl, tl, Es)); G[2 * j + 1] = ex2f(fmaf(negA * th, th, Es));
+        }
+    } else {
+        const float cc = fabsf(r[9]);
+        const float nAt = negA * t3;
+        float rf = ex2f(fminf(fmaf(nAt, 2.0f, negA), 120.f)), rb = ex2f(fminf(fmaf(nAt, -2.0f, negA), 120.f));
+        G[0] = ex2f(fmaf(nAt, t3, Es));
+        G[1] = G[0] * rf; rf *= cc; G[3] = G[1] * rf; rf *= cc; G[5] = G[3] * rf; rf *= cc; G[7] = G[5] * rf;
+        G[2] = G[0] * rb; rb *= cc; G[4] = G[2] * rb; rb *= cc; G[6] = G[4] * rb;
+    }
+    #pragma unroll
+    for (int k = 0; k < 8; ++k) acc[k] = fmaf(G[k], r[12 + k], acc[k]);
+}
+
+__device__ __forceinline__ void eval_key_b1(const float* __restrict__ r, uint32_t lanebit, float fy, float fz,
+                                            float (&acc0)[8], float (&acc1)[8])
+{
+    const float4 q0 = *reinterpret_cast<const float4*>(r);
+    const float4 q1 = *reinterpret_cast<const float4*>(r + 4);
+    const float4 q2 = *reinterpret_cast<const float4*>(r + 8);
+    const uint32_t m0 = __float_as_uint(q2.z), m1 = __float_as_uint(q2.w);
+    if (q2.y < 0.f) {                                               // slow key (warp-uniform)
+        if (m0) eval_row_slow(r, (m0 & lanebit) != 0u, fy, fz, acc0);
+        if (m1) eval_row_slow(r, (m1 & lanebit) != 0u, fy, fz + 4.0f, acc1);
+        return;
+    }
+    const float4 wa = *reinterpret_cast<const float4*>(r + 12);
+    const float4 wb = *reinterpret_cast<const float4*>(r + 16);
+    // setup of both rows at once: (row z, row z + 4) in the two halves of a packed register
+    const float dy = fy + q0.y;
+    const f32x2 dz = add2(pk2(fz, fz + 4.0f), pk2(q0.z, q0.z));
+    const f32x2 u1 = fma2(pk2(q1.z, q1.z), dz, pk2(dy, dy));
+    const float tA = fmaf(q1.x, dy, q0.x);
+    const f32x2 t3 = fma2(pk2(q1.y, q1.y), dz, pk2(tA, tA));
+    const f32x2 Es = fma2(mul2(pk2(q2.x, q2.x), dz), dz, mul2(mul2(pk2(q1.w, q1.w), u1), u1));
+    const f32x2 negA = pk2(q0.w, q0.w);
+    const f32x2 nAt = mul2(negA, t3);
+    const f32x2 E3 = fma2(nAt, t3, Es);
+    const f32x2 Lf = fma2(nAt, pk2(2.0f, 2.0f), negA);
+    float E3a, E3b, Lfa, Lfb;
+    upk2(E3, E3a, E3b); upk2(Lf, Lfa, Lfb);
+    if (m0) {
+        E3a = (m0 & lanebit) ? E3a : -1.0e30f;                      // rows outside the box contribute exact zeros
+        recur_accumulate(E3a, Lfa, wa, wb, acc0);
+    }
+    if (m1) {
+        E3b = (m1 & lanebit) ? E3b : -1.0e30f;
+        recur_accumulate(E3b, Lfb, wa, wb, acc1);
+    }
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(32)
+k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
+             const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
+             const float* __restrict__ weight, int wstride, int c0,
+             float* __restrict__ out, GridDev gd)
+{
+    __shared__ __align__(16) float s_raw[kB1Batch * kB1Words];
+    __shared__ __align__(16) float s_rec[kB1Batch * kB1Words];
+
+    const int lane = threadIdx.x;
+    const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];
+    const int bx = b % gd.nb[0], by = (b / gd.nb[0]) % gd.nb[1], bz = b / (gd.nb[0] * gd.nb[1]);
+    const int b0x = bx * kBrick, b0y = by * kBrick, b0z = bz * kBrick;
+    const int ry = lane & 7, rz = lane >> 3;                        // rows (ry, rz) and (ry, rz + 4)
+    const float fy = (float)ry, fz = (float)rz;
+    const uint32_t lanebit = 1u << lane;
+
+    float acc0[8], acc1[8];                         // acc[2j], acc[2j+1] = voxels 3 - j, 4 + j
+    #pragma unroll
+    for (int j = 0; j < 8; ++j) { acc0[j] = 0.f; acc1[j] = 0.f; }
+
+    uint32_t kbeg = 0, kend = 0;
+    if (!status->overflow) { kbeg = bin_start[b * kNumClasses]; kend = bin_start[(b + 1) * kNumClasses]; }
+
+    const uint32_t raw_addr = (uint32_t)__cvta_generic_to_shared(s_raw + lane * kB1Words);
+    auto fetch = [&](uint32_t gid) {                // this lane's record + weight -> s_raw, asynchronously
+        const char* rp = reinterpret_cast<const char*>(rec + gid);
+        cp_async16(raw_addr, rp); cp_async16(raw_addr + 16, rp + 16);
+        cp_async16(raw_addr + 32, rp + 32); cp_async16(raw_addr + 48, rp + 48);
+        cp_async4(raw_addr + 64, weight + (size_t)gid * wstride + c0);
+    };
+    uint32_t gid_next = 0;
+    if (kbeg + lane < kend) fetch(keys[kbeg + lane]);
+    cp_async_commit();
+    if (kbeg + kB1Batch + lane < kend) gid_next = keys[kbeg + kB1Batch + lane];
+
+    for (uint32_t base = kbeg; base < kend; base += kB1Batch) {
+        cp_async_wait_all();
+        __syncwarp();                               // the previous batch's records have been read by every lane
+        if (base + lane < kend) {
+            const float4* rp = reinterpret_cast<const float4*>(s_raw + lane * kB1Words);
+            const float4 a = rp[0], bq = rp[1], c = rp[2], d = rp[3];
+            const float w = s_raw[lane * kB1Words + 16];
+            const int w1i = __float_as_int(d.y), w2i = __float_as_int(d.z), w3i = __float_as_int(d.w);
+            const int lox = (int16_t)(w1i & 0xffff), loy = (int16_t)(w1i >> 16), loz = (int16_t)(w2i & 0xffff);
+            const int hix = (int16_t)(w2i >> 16), hiy = (int16_t)(w3i & 0xffff), hiz = (int16_t)(w3i >> 16);
+            const int x0 = max(lox - b0x, 0), x1 = min(hix - b0x, 7);
+            const int y0 = max(loy - b0y, 0), y1 = min(hiy - b0y, 7);
+            const int z0 = max(loz - b0z, 0), z1 = min(hiz - b0z, 7);
+            const uint32_t ym = ((2u << y1) - (1u << y0)) & 0xffu;
+            const uint32_t zm = ((2u << z1) - (1u << z0)) & 0xffu;
+            const uint32_t xm = ((2u << x1) - (1u << x0)) & 0xffu;
+            const uint32_t rep = ym * 0x01010101u;
+            const uint32_t sel0 = ((zm & 1u) ? 0xffu : 0u) | ((zm & 2u) ? 0xff00u : 0u) |
+                                  ((zm & 4u) ? 0xff0000u : 0u) | ((zm & 8u) ? 0xff000000u : 0u);
+            const uint32_t zh = zm >> 4;
+            const uint32_t sel1 = ((zh & 1u) ? 0xffu : 0u) | ((zh & 2u) ? 0xff00u : 0u) |
+                                  ((zh & 4u) ? 0xff0000u : 0u) | ((zh & 8u) ? 0xff000000u : 0u);
+            const float cx = (float)(__float_as_int(bq.x) - b0x) + a.x;
+            const float cy = (float)(__float_as_int(bq.y) - b0y) + a.y;
+            const float cz = (float)(__float_as_int(bq.z) - b0z) + a.z;
+            const float cx3 = 3.0f - cx, negA = bq.w, l01 = -c.x, l02 = -c.y;
+            // largest |t3| over the 64 rows: dy in [-cy, 7 - cy], dz in [-cz, 7 - cz]
+            const float t3max = fabsf(cx3) + fabsf(l01) * fmaxf(fabsf(cy), fabsf(7.0f - cy)) +
+                                fabsf(l02) * fmaxf(fabsf(cz), fabsf(7.0f - cz));
+            const bool slow = (-negA > kRecurrenceMaxA) || !(-negA * fmaf(2.0f, t3max, 1.0f) < 120.f);
+            const float cc = fabsf(a.w);
+            float4* o = reinterpret_cast<float4*>(s_rec + lane * kB1Words);
+            o[0] = make_float4(cx3, -cy, -cz, negA);
+            o[1] = make_float4(l01, l02, c.z, c.w);
+            o[2] = make_float4(d.x, slow ? -fmaxf(cc, 1.0e-30f) : cc,       // c = 2^-2A underflows to 0 for A > 63: -0 would not read as slow
+                               __uint_as_float(rep & sel0), __uint_as_float(rep & sel1));
+            // fast keys: the key-and-k part of the row profile, c^((k-3)(k-4)/2), goes into the weights (recur_accumulate)
+            const float w1 = slow ? w : w * cc, c3 = cc * cc * cc, w3 = slow ? w : w * c3, w6 = slow ? w : w * (c3 * c3);
+            o[3] = make_float4((xm & 8u) ? w : 0.f, (xm & 16u) ? w : 0.f, (xm & 4u) ? w1 : 0.f, (xm & 32u) ? w1 : 0.f);
+            o[4] = make_float4((xm & 2u) ? w3 : 0.f, (xm & 64u) ? w3 : 0.f, (xm & 1u) ? w6 : 0.f, (xm & 128u) ? w6 : 0.f);
+        }
+        __syncwarp();
+        // next batch's records on their way while this one is evaluated
+        if (base + kB1Batch + lane < kend) fetch(gid_next);
+        cp_async_commit();
+        if (base + 2 * kB1Batch + lane < kend) gid_next = keys[base + 2 * kB1Batch + lane];
+        const int nb = (int)min((uint32_t)kB1Batch, kend - base);
+        #pragma unroll 1
+        for (int j = 0; j < nb; ++j) eval_key_b1(s_rec + j * kB1Words, lanebit, fy, fz, acc0, acc1);
+    }
+
+    // write the two rows once (zeros for empty bricks); x fastest
+    const size_t plane = (size_t)gd.dims[0] * gd.dims[1] * gd.dims[2];
+    #pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int gy = b0y + ry, gz = b0z + rz + 4 * h;
+        if (gy < gd.dims[1] && gz < gd.dims[2]) {
+            const size_t rowoff = ((size_t)gz * gd.dims[1] + gy) * gd.dims[0] + b0x;
+            float v[8];
+            #pragma unroll
+            for (int j = 0; j < 4; ++j) { v[3 - j] = h ? acc1[2 * j] : acc0[2 * j]; v[4 + j] = h ? acc1[2 * j + 1] : acc0[2 * j + 1]; }
+            float* o = out + (size_t)c0 * plane + rowoff;
+            if (VEC) {
+                if (b0x + 3 < gd.dims[0]) __stcs(reinterpret_cast<float4*>(o), make_float4(v[0], v[1], v[2], v[3]));
+                if (b0x + 7 < gd.dims[0]) __stcs(reinterpret_cast<float4*>(o) + 1, make_float4(v[4], v[5], v[6], v[7]));
+            } else {
+                #pragma unroll
+                for (int k2 = 0; k2 < 8; ++k2)
+                    if (b0x + k2 < gd.dims[0]) o[k2] = v[k2];
+            }
+        }
+    }
+}
+
+static int launch_fwd_b1(gsvox_plan* p, const float* weight, int C, int c0, float* out, cudaStream_t st)
+{
+    LaunchScope ls(p, GSVOX_K_FORWARD, st);
+    const bool vec = (p->gd.dims[0] % 4 == 0) && (((uintptr_t)out & 15) == 0);
+    const int nblocks = (p->gd.slab1 - p->gd.slab0) * p->gd.nb[0] * p->gd.nb[1];
+    if (nblocks <= 0) return GSVOX_OK;
+    if (vec) k_forward_b1<true><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd);
+    else     k_forward_b1<false><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
+}
+
 template <int CH>
 static int launch_fwd_ch(gsvox_plan* p, const float* weight, int C, int c0, float* out, cudaStream_t st)
 {
@@ -261,7 +505,8 @@ int launch_forward(gsvox_plan* p, const float* weight, int channels, float* out,
         int left = channels - c0;
         if (left >= 9)      { rc = launch_fwd_ch<9>(p, weight, channels, c0, out, st); c0 += 9; }
         else if (left >= 3) { rc = launch_fwd_ch<3>(p, weight, channels, c0, out, st); c0 += 3; }
-        else                { rc = launch_fwd_ch<1>(p, weight, channels, c0, out, st); c0 += 1; }
+        else                { rc = (getenv("GSVOX_FWD_OLD") ? launch_fwd_ch<1>(p, weight, channels, c0, out, st)
+                                                            : launch_fwd_b1(p, weight, channels, c0, out, st)); c0 += 1; }
     }
     return rc;
 }

@@ -3,10 +3,9 @@
 // batched over the B projections of a training batch, forward and backward.
 //
 // Readings W1-W4: trilinear interpolation of the voxel-centre samples; a corner outside
-// the grid contributes 0; d is in world units, the sample sits at index u_k = i_k + d_k / h_k; the
-// cell index is decided on t_k = d_k * (1 / h_k) in fp32 (reciprocal rounded once, one multiply, floor;
-// the fraction t - floor t is exact), so positions far from the origin lose nothing to the magnitude of i_k; a non-finite
-// displacement yields 0 and zero gradients.
+// the grid contributes 0; d is in world units, the sample sits at index u_k = i_k + d_k / h_k, its
+// cell is floor(d_k / h_k) EXACTLY (see warp_cell), so positions far from the origin lose nothing to the
+// magnitude of i_k; a non-finite displacement yields 0 and zero gradients.
 //
 // HBM/L2-bound gather.  One thread per output voxel, x fastest: the three d loads, the g load and
 // the store are coalesced; the eight corner reads hit L1/L2 (I_ref is 33 MB at 256x256x128, inside
@@ -20,20 +19,39 @@ namespace gsvox {
 
 constexpr int kWarpThreads = 256;
 
-struct WarpGrid { int nx, ny, nz; float inv_hx, inv_hy, inv_hz; float hx, hy, hz; };
+struct WarpGrid { int nx, ny, nz; float inv_hx, inv_hy, inv_hz; float hx, hy, hz; int inexact; };   // inexact: bit k set <=> 1/h_k is not a power of two
+
+// One axis of the cell decision.  t = d * fp32(1/h) carries two fp32 roundings, |t - d/h| <= 2^-23 |t|, so
+// floor(t) can differ from floor(d/h) only within that distance of a cell face.  The interpolant is continuous
+// there, but its slope (grad d) is not, so such samples are settled exactly: the sign of the fused
+// d - k h is the sign of the exact value (one rounding, never to the other side of 0), which tells whether
+// k <= d/h < k + 1.  Rare branch (|t| >= 8 or a fraction within 2e-6 of 0 or 1); skipped altogether when 1/h
+// is exact in fp32 (power-of-two spacing: t is then exact).
+__device__ __forceinline__ void settle_cell(float d, float h, float t, float& fl, float& f)
+{
+    const float r0 = fmaf(-fl, h, d), r1 = fmaf(-(fl + 1.f), h, d);
+    if (r0 < 0.f) fl -= 1.f; else if (r1 >= 0.f) fl += 1.f;
+    f = fminf(fmaxf(t - fl, 0.f), 1.f);
+}
 
 // Cell of one sample: base corner (may be outside the grid) and fractions; false if non-finite or
-// |t| >= 2^22 voxels.  t = d * (1/h): one fp32 multiply by the reciprocal the host rounded once (reading
-// W3; the oracle does the same two roundings).  floor -> int without a second conversion instruction:
-// for |fl| < 2^22, fl + 1.5 * 2^23 holds the integer in its low mantissa bits.
+// |t| >= 2^22 voxels.  floor -> int without a second conversion instruction: for |fl| < 2^22,
+// fl + 1.5 * 2^23 holds the integer in its low mantissa bits.
 __device__ __forceinline__ bool warp_cell(float dx, float dy, float dz, const WarpGrid& wg, int x, int y, int z,
                                           int& cx, int& cy, int& cz, float& fx, float& fy, float& fz)
 {
     const float tx = __fmul_rn(dx, wg.inv_hx), ty = __fmul_rn(dy, wg.inv_hy), tz = __fmul_rn(dz, wg.inv_hz);
     // the comparison is false for NaN, so it rejects NaN and inf as well
     const bool ok = (fabsf(tx) < 4194304.f) && (fabsf(ty) < 4194304.f) && (fabsf(tz) < 4194304.f);
-    const float flx = floorf(tx), fly = floorf(ty), flz = floorf(tz);
-    fx = ok ? tx - flx : 0.f; fy = ok ? ty - fly : 0.f; fz = ok ? tz - flz : 0.f;
+    float flx = floorf(tx), fly = floorf(ty), flz = floorf(tz);
+    fx = tx - flx; fy = ty - fly; fz = tz - flz;
+    if (wg.inexact && ok) {
+        constexpr float kEps = 2.0e-6f, kBig = 8.f;                 // 2^-23 * 8 = 9.5e-7 < kEps
+        if (wg.inexact & 1) if (fx < kEps || fx > 1.f - kEps || fabsf(tx) >= kBig) settle_cell(dx, wg.hx, tx, flx, fx);
+        if (wg.inexact & 2) if (fy < kEps || fy > 1.f - kEps || fabsf(ty) >= kBig) settle_cell(dy, wg.hy, ty, fly, fy);
+        if (wg.inexact & 4) if (fz < kEps || fz > 1.f - kEps || fabsf(tz) >= kBig) settle_cell(dz, wg.hz, tz, flz, fz);
+    }
+    fx = ok ? fx : 0.f; fy = ok ? fy : 0.f; fz = ok ? fz : 0.f;
     const int ix = __float_as_int(flx + 12582912.f) - 0x4B400000, iy = __float_as_int(fly + 12582912.f) - 0x4B400000;
     const int iz = __float_as_int(flz + 12582912.f) - 0x4B400000;
     cx = ok ? x + ix : x; cy = ok ? y + iy : y; cz = ok ? z + iz : z;
@@ -242,6 +260,12 @@ static int warp_grid(const gsvox_grid* g, int32_t B, WarpGrid* wg)
     wg->nx = g->dims[0]; wg->ny = g->dims[1]; wg->nz = g->dims[2];
     wg->hx = g->spacing[0]; wg->hy = g->spacing[1]; wg->hz = g->spacing[2];
     wg->inv_hx = 1.f / g->spacing[0]; wg->inv_hy = 1.f / g->spacing[1]; wg->inv_hz = 1.f / g->spacing[2];
+    wg->inexact = 0;
+    for (int k = 0; k < 3; ++k) {
+        int e; const float m = frexpf(g->spacing[k], &e);           // power of two <=> mantissa 0.5: then d * (1/h) is exact
+        const float inv = 1.f / g->spacing[k];
+        if (m != 0.5f || !(inv > 1.17549435e-38f) || !(inv < 3.0e38f)) wg->inexact |= 1 << k;
+    }
     if ((long long)wg->nx * wg->ny * wg->nz >= (1LL << 31)) return GSVOX_ELIMIT;     // 32-bit voxel indices
     return GSVOX_OK;
 }
