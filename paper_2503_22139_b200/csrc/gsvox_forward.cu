@@ -1,6 +1,10 @@
 // gsvox_forward.cu — step a3: per-brick forward accumulation (Eq. 5).
 //
-// One CTA of 64 threads per 8^3 brick; thread t owns the x-row (y = t&7, z = t>>3) of the brick,
+// Two kernels: k_forward<CH> (CH = 3, 9: the motion-basis fields, channel groups of a wider C) described here, and
+// k_forward_b1 (C = 1: the CBCT volume, the headline configuration) further down, which re-cuts the same row
+// arithmetic around what actually limits it — operand delivery through shared memory.
+//
+// k_forward<CH>: one CTA of 64 threads per 8^3 brick; thread t owns the x-row (y = t&7, z = t>>3) of the brick,
 // i.e. 8 consecutive voxels per channel, accumulated in registers and written once.  The brick's
 // keys are staged 64 at a time into shared memory: each thread gathers one 64-byte Gaussian
 // record (four LDG.128, L2-resident: a record is shared by ~20 bricks), rebases the centre to
@@ -18,7 +22,6 @@
 // take the direct path, one EX2 per voxel: the recurrence would lose accuracy and could
 // underflow there (error budget).  Direct keys are class 0 of the brick's
 // key range, so which path a staged key takes is known from bin_start, not from its data.
-#include <cstdlib>
 #include "gsvox_internal.cuh"
 
 namespace gsvox {
@@ -249,27 +252,25 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
 // rows (y, z) and (y, z + 4).  The row setup runs once for both rows in packed f32x2 instructions whose
 // key operands are scalar registers broadcast to both halves (SASS: the .F32 operand form), so the staged
 // record needs no interleaving; the three exponents per row then feed the centre-out recurrence of
-// k_forward.  Per key: 5 LDS.128, ~13 setup + 2 x 16 row instructions, 6 EX2; the FP32 pipe is the limit
-// (packed instructions take two pipe cycles).  A half (4 z-layers) no row of which lies in the box skips
-// its recurrence.  The batch's 64-byte records (and weights) arrive by cp.async, issued one batch ahead;
-// single-warp CTAs need no __syncthreads, 32 of them are resident per SM.
-// "Slow" keys (c stored negative) take a scalar route: direct-exponential keys (A > 1, class 0) and keys
+// k_forward.  Per key: 5 LDS.128, ~12 setup + 2 x 13 row instructions, 6 EX2; shared-memory path, issue slots and
+// the FP32 pipe (packed instructions take two pipe cycles) are about equally busy.  The batch's 64-byte records arrive
+// by cp.async, issued one batch ahead; single-warp CTAs need no
+// __syncthreads, 32 of them are resident per SM.
+// Keys are staged class by class — slow | both z-halves | lower half only | upper half only — so each class runs
+// its own branch-free loop (a half no row of which lies in the box is never evaluated).  "Slow" keys take a scalar route: direct-exponential keys (A > 1, class 0) and keys
 // whose first ratio 2^Lf, 2^Lb could overflow on some row of the brick (A (1 + 2 max|t3|) >= 120: the fast
 // path has no clamp — such rows hold nothing but zeros, yet inf * 0 must not be formed).
 // ==========================================================================================
 constexpr int kB1Batch = 32;
-constexpr int kB1Words = 20;                        // staged record; also the stride of the raw copy (16 + weight, padded): conflict-free 128-bit per-lane access
+constexpr int kB1Words = 20;                        // staged record; also the stride of the raw copy (16 words, padded): conflict-free 128-bit per-lane access
 
 __device__ __forceinline__ void cp_async16(uint32_t saddr, const void* g)
 { asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" :: "r"(saddr), "l"(g) : "memory"); }
-__device__ __forceinline__ void cp_async4(uint32_t saddr, const void* g)
-{ asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(saddr), "l"(g) : "memory"); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // staged record (floats):  0 cx3  1 ncy  2 ncz  3 negA | 4 l01  5 l02  6 l12  7 nD1 | 8 nD2  9 +-c  10 mask(z 0..3)  11 mask(z 4..7)
 //                          12..19  w * [k inside the box in x] (fast keys: * c^{0,0,1,1,3,3,6,6}) in the order k = 3,4, 2,5 | 1,6, 0,7
-//                          c < 0 marks a slow key
 // cx3 = 3 - cx, ncy = -cy, ncz = -cz, l01 = +l01, l02 = +l02:  t3 = 3 - xs = cx3 + l01 dy + l02 dz.
 
 // One row from its two exponents: E3 (value at k = 3) and Lf = E(4) - E(3).  The row is the parabola
@@ -320,23 +321,27 @@ __device__ __forceinline__ void eval_row_slow(const float* __restrict__ r, bool 
     for (int k = 0; k < 8; ++k) acc[k] = fmaf(G[k], r[12 + k], acc[k]);
 }
 
-__device__ __forceinline__ void eval_key_b1(const float* __restrict__ r, uint32_t lanebit, float fy, float fz,
-                                            float (&acc0)[8], float (&acc1)[8])
+// A slow key (direct exponentials, or a recurrence that needs its clamps): scalar, row by row.
+__device__ __forceinline__ void eval_key_slow(const float* __restrict__ r, uint32_t lanebit, float fy, float fz,
+                                              float (&acc0)[8], float (&acc1)[8])
+{
+    const uint32_t m0 = __float_as_uint(r[10]), m1 = __float_as_uint(r[11]);
+    if (m0) eval_row_slow(r, (m0 & lanebit) != 0u, fy, fz, acc0);
+    if (m1) eval_row_slow(r, (m1 & lanebit) != 0u, fy, fz + 4.0f, acc1);
+}
+
+// A fast key that reaches both z-halves: setup of both rows at once, (row z, row z + 4) in the two halves of
+// a packed register, the key's scalars broadcast.
+__device__ __forceinline__ void eval_key_both(const float* __restrict__ r, uint32_t lanebit, float fy, f32x2 fz2,
+                                              float (&acc0)[8], float (&acc1)[8])
 {
     const float4 q0 = *reinterpret_cast<const float4*>(r);
     const float4 q1 = *reinterpret_cast<const float4*>(r + 4);
     const float4 q2 = *reinterpret_cast<const float4*>(r + 8);
-    const uint32_t m0 = __float_as_uint(q2.z), m1 = __float_as_uint(q2.w);
-    if (q2.y < 0.f) {                                               // slow key (warp-uniform)
-        if (m0) eval_row_slow(r, (m0 & lanebit) != 0u, fy, fz, acc0);
-        if (m1) eval_row_slow(r, (m1 & lanebit) != 0u, fy, fz + 4.0f, acc1);
-        return;
-    }
     const float4 wa = *reinterpret_cast<const float4*>(r + 12);
     const float4 wb = *reinterpret_cast<const float4*>(r + 16);
-    // setup of both rows at once: (row z, row z + 4) in the two halves of a packed register
     const float dy = fy + q0.y;
-    const f32x2 dz = add2(pk2(fz, fz + 4.0f), pk2(q0.z, q0.z));
+    const f32x2 dz = add2(fz2, pk2(q0.z, q0.z));
     const f32x2 u1 = fma2(pk2(q1.z, q1.z), dz, pk2(dy, dy));
     const float tA = fmaf(q1.x, dy, q0.x);
     const f32x2 t3 = fma2(pk2(q1.y, q1.y), dz, pk2(tA, tA));
@@ -347,18 +352,35 @@ __device__ __forceinline__ void eval_key_b1(const float* __restrict__ r, uint32_
     const f32x2 Lf = fma2(nAt, pk2(2.0f, 2.0f), negA);
     float E3a, E3b, Lfa, Lfb;
     upk2(E3, E3a, E3b); upk2(Lf, Lfa, Lfb);
-    if (m0) {
-        E3a = (m0 & lanebit) ? E3a : -1.0e30f;                      // rows outside the box contribute exact zeros
-        recur_accumulate(E3a, Lfa, wa, wb, acc0);
-    }
-    if (m1) {
-        E3b = (m1 & lanebit) ? E3b : -1.0e30f;
-        recur_accumulate(E3b, Lfb, wa, wb, acc1);
-    }
+    E3a = (__float_as_uint(q2.z) & lanebit) ? E3a : -1.0e30f;        // rows outside the box contribute exact zeros
+    E3b = (__float_as_uint(q2.w) & lanebit) ? E3b : -1.0e30f;
+    recur_accumulate(E3a, Lfa, wa, wb, acc0);
+    recur_accumulate(E3b, Lfb, wa, wb, acc1);
+}
+
+// A fast key that reaches one z-half only: one row per thread, scalar setup.  HI: the half z = 4..7.
+template <bool HI>
+__device__ __forceinline__ void eval_key_half(const float* __restrict__ r, uint32_t lanebit, float fy, float fzh,
+                                              float (&acc)[8])
+{
+    const float4 q0 = *reinterpret_cast<const float4*>(r);
+    const float4 q1 = *reinterpret_cast<const float4*>(r + 4);
+    const float4 q2 = *reinterpret_cast<const float4*>(r + 8);
+    const float4 wa = *reinterpret_cast<const float4*>(r + 12);
+    const float4 wb = *reinterpret_cast<const float4*>(r + 16);
+    const float dy = fy + q0.y, dz = fzh + q0.z;
+    const float u1 = fmaf(q1.z, dz, dy);
+    const float t3 = fmaf(q1.y, dz, fmaf(q1.x, dy, q0.x));
+    const float Es = fmaf(q2.x * dz, dz, (q1.w * u1) * u1);
+    const float nAt = q0.w * t3;
+    float E3 = fmaf(nAt, t3, Es);
+    const float Lf = fmaf(nAt, 2.0f, q0.w);
+    E3 = (__float_as_uint(HI ? q2.w : q2.z) & lanebit) ? E3 : -1.0e30f;
+    recur_accumulate(E3, Lf, wa, wb, acc);
 }
 
 template <bool VEC>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32, 32)
 k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
              const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
              const float* __restrict__ weight, int wstride, int c0,
@@ -373,6 +395,7 @@ k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_sta
     const int b0x = bx * kBrick, b0y = by * kBrick, b0z = bz * kBrick;
     const int ry = lane & 7, rz = lane >> 3;                        // rows (ry, rz) and (ry, rz + 4)
     const float fy = (float)ry, fz = (float)rz;
+    const f32x2 fz2 = pk2(fz, fz + 4.0f);
     const uint32_t lanebit = 1u << lane;
 
     float acc0[8], acc1[8];                         // acc[2j], acc[2j+1] = voxels 3 - j, 4 + j
@@ -383,24 +406,32 @@ k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_sta
     if (!status->overflow) { kbeg = bin_start[b * kNumClasses]; kend = bin_start[(b + 1) * kNumClasses]; }
 
     const uint32_t raw_addr = (uint32_t)__cvta_generic_to_shared(s_raw + lane * kB1Words);
-    auto fetch = [&](uint32_t gid) {                // this lane's record + weight -> s_raw, asynchronously
+    auto fetch = [&](uint32_t gid) {                // this lane's record -> s_raw, asynchronously
         const char* rp = reinterpret_cast<const char*>(rec + gid);
         cp_async16(raw_addr, rp); cp_async16(raw_addr + 16, rp + 16);
         cp_async16(raw_addr + 32, rp + 32); cp_async16(raw_addr + 48, rp + 48);
-        cp_async4(raw_addr + 64, weight + (size_t)gid * wstride + c0);
     };
     uint32_t gid_next = 0;
-    if (kbeg + lane < kend) fetch(keys[kbeg + lane]);
+    float w_cur = 0.f, w_next = 0.f;
+    if (kbeg + lane < kend) {
+        const uint32_t gid = keys[kbeg + lane];
+        fetch(gid);
+        w_cur = __ldg(weight + (size_t)gid * wstride + c0);
+    }
     cp_async_commit();
     if (kbeg + kB1Batch + lane < kend) gid_next = keys[kbeg + kB1Batch + lane];
 
     for (uint32_t base = kbeg; base < kend; base += kB1Batch) {
         cp_async_wait_all();
         __syncwarp();                               // the previous batch's records have been read by every lane
+        // ---- stage: lane l turns key l into brick-local form and classifies it; keys are stored class by class
+        //      (slow | both halves | lower half only | upper half only) so that each class runs a branch-free loop
+        int cls = -1;
+        float4 o0, o1, o2, o3, o4;
         if (base + lane < kend) {
             const float4* rp = reinterpret_cast<const float4*>(s_raw + lane * kB1Words);
             const float4 a = rp[0], bq = rp[1], c = rp[2], d = rp[3];
-            const float w = s_raw[lane * kB1Words + 16];
+            const float w = w_cur;
             const int w1i = __float_as_int(d.y), w2i = __float_as_int(d.z), w3i = __float_as_int(d.w);
             const int lox = (int16_t)(w1i & 0xffff), loy = (int16_t)(w1i >> 16), loz = (int16_t)(w2i & 0xffff);
             const int hix = (int16_t)(w2i >> 16), hiy = (int16_t)(w3i & 0xffff), hiz = (int16_t)(w3i >> 16);
@@ -425,24 +456,41 @@ k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_sta
                                 fabsf(l02) * fmaxf(fabsf(cz), fabsf(7.0f - cz));
             const bool slow = (-negA > kRecurrenceMaxA) || !(-negA * fmaf(2.0f, t3max, 1.0f) < 120.f);
             const float cc = fabsf(a.w);
-            float4* o = reinterpret_cast<float4*>(s_rec + lane * kB1Words);
-            o[0] = make_float4(cx3, -cy, -cz, negA);
-            o[1] = make_float4(l01, l02, c.z, c.w);
-            o[2] = make_float4(d.x, slow ? -fmaxf(cc, 1.0e-30f) : cc,       // c = 2^-2A underflows to 0 for A > 63: -0 would not read as slow
-                               __uint_as_float(rep & sel0), __uint_as_float(rep & sel1));
+            cls = slow ? 0 : ((zm & 0x0fu) == 0u ? 3 : ((zm & 0xf0u) == 0u ? 2 : 1));
+            o0 = make_float4(cx3, -cy, -cz, negA);
+            o1 = make_float4(l01, l02, c.z, c.w);
+            o2 = make_float4(d.x, cc, __uint_as_float(rep & sel0), __uint_as_float(rep & sel1));
             // fast keys: the key-and-k part of the row profile, c^((k-3)(k-4)/2), goes into the weights (recur_accumulate)
             const float w1 = slow ? w : w * cc, c3 = cc * cc * cc, w3 = slow ? w : w * c3, w6 = slow ? w : w * (c3 * c3);
-            o[3] = make_float4((xm & 8u) ? w : 0.f, (xm & 16u) ? w : 0.f, (xm & 4u) ? w1 : 0.f, (xm & 32u) ? w1 : 0.f);
-            o[4] = make_float4((xm & 2u) ? w3 : 0.f, (xm & 64u) ? w3 : 0.f, (xm & 1u) ? w6 : 0.f, (xm & 128u) ? w6 : 0.f);
+            o3 = make_float4((xm & 8u) ? w : 0.f, (xm & 16u) ? w : 0.f, (xm & 4u) ? w1 : 0.f, (xm & 32u) ? w1 : 0.f);
+            o4 = make_float4((xm & 2u) ? w3 : 0.f, (xm & 64u) ? w3 : 0.f, (xm & 1u) ? w6 : 0.f, (xm & 128u) ? w6 : 0.f);
+        }
+        const uint32_t b0 = __ballot_sync(0xffffffffu, cls == 0), b1 = __ballot_sync(0xffffffffu, cls == 1),
+                       b2 = __ballot_sync(0xffffffffu, cls == 2), b3 = __ballot_sync(0xffffffffu, cls == 3);
+        const int n0 = __popc(b0), n1 = n0 + __popc(b1), n2 = n1 + __popc(b2), n3 = n2 + __popc(b3);
+        if (cls >= 0) {
+            const uint32_t mine = cls == 0 ? b0 : (cls == 1 ? b1 : (cls == 2 ? b2 : b3));
+            const int slot = (cls == 0 ? 0 : (cls == 1 ? n0 : (cls == 2 ? n1 : n2))) + __popc(mine & (lanebit - 1u));
+            float4* o = reinterpret_cast<float4*>(s_rec + slot * kB1Words);
+            o[0] = o0; o[1] = o1; o[2] = o2; o[3] = o3; o[4] = o4;
         }
         __syncwarp();
         // next batch's records on their way while this one is evaluated
-        if (base + kB1Batch + lane < kend) fetch(gid_next);
+        if (base + kB1Batch + lane < kend) {
+            fetch(gid_next);
+            w_next = __ldg(weight + (size_t)gid_next * wstride + c0);
+        }
         cp_async_commit();
+        w_cur = w_next;
         if (base + 2 * kB1Batch + lane < kend) gid_next = keys[base + 2 * kB1Batch + lane];
-        const int nb = (int)min((uint32_t)kB1Batch, kend - base);
+        int j = 0;
+        for (; j < n0; ++j) eval_key_slow(s_rec + j * kB1Words, lanebit, fy, fz, acc0, acc1);
         #pragma unroll 1
-        for (int j = 0; j < nb; ++j) eval_key_b1(s_rec + j * kB1Words, lanebit, fy, fz, acc0, acc1);
+        for (; j < n1; ++j) eval_key_both(s_rec + j * kB1Words, lanebit, fy, fz2, acc0, acc1);
+        #pragma unroll 1
+        for (; j < n2; ++j) eval_key_half<false>(s_rec + j * kB1Words, lanebit, fy, fz, acc0);
+        #pragma unroll 1
+        for (; j < n3; ++j) eval_key_half<true>(s_rec + j * kB1Words, lanebit, fy, fz + 4.0f, acc1);
     }
 
     // write the two rows once (zeros for empty bricks); x fastest
@@ -505,8 +553,7 @@ int launch_forward(gsvox_plan* p, const float* weight, int channels, float* out,
         int left = channels - c0;
         if (left >= 9)      { rc = launch_fwd_ch<9>(p, weight, channels, c0, out, st); c0 += 9; }
         else if (left >= 3) { rc = launch_fwd_ch<3>(p, weight, channels, c0, out, st); c0 += 3; }
-        else                { rc = (getenv("GSVOX_FWD_OLD") ? launch_fwd_ch<1>(p, weight, channels, c0, out, st)
-                                                            : launch_fwd_b1(p, weight, channels, c0, out, st)); c0 += 1; }
+        else                { rc = launch_fwd_b1(p, weight, channels, c0, out, st); c0 += 1; }
     }
     return rc;
 }
