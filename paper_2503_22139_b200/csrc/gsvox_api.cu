@@ -57,7 +57,7 @@ static bool grid_ok(const gsvox_grid* g)
     return true;
 }
 
-struct Layout { size_t status, rec, aux, bin_count, bin_start, scan_partial, keys, acc, total; int nbins, nbricks, nb[3]; };
+struct Layout { size_t status, rec, aux, bin_count, bin_start, scan_partial, keys, split, acc, total; int nbins, nbricks, nb[3], split_cap; };
 
 static size_t up256(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -82,6 +82,8 @@ static int make_layout(int64_t n_max, int32_t max_channels, const gsvox_grid* g,
     size_t sblocks = (size_t)((nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock);
     L->scan_partial = off; off += up256(sizeof(uint32_t) * (sblocks + 1));
     L->keys = off;         off += up256(sizeof(uint32_t) * (size_t)key_capacity);
+    L->split_cap = (int)(key_capacity / kSplitKeys) + 1;              // sum over bricks of floor(keys / kSplitKeys) <= this
+    L->split = off;        off += up256(sizeof(uint2) * (size_t)L->split_cap);
     L->acc = off;          off += up256(sizeof(float) * (size_t)n_max * (size_t)acc_stride(max_channels));
     L->total = off;
     return GSVOX_OK;
@@ -124,6 +126,7 @@ extern "C" int gsvox_plan_create(int64_t n_max, int32_t max_channels, const gsvo
     p->bin_count = (uint32_t*)(w + L.bin_count); p->bin_start = (uint32_t*)(w + L.bin_start);
     p->scan_partial = (uint32_t*)(w + L.scan_partial); p->keys = (uint32_t*)(w + L.keys);
     p->acc = (float*)(w + L.acc);
+    p->split_list = (uint2*)(w + L.split); p->split_cap = L.split_cap;
     p->nbins = L.nbins;
     *plan = p;
     return GSVOX_OK;

@@ -22,6 +22,9 @@
 namespace gsvox {
 
 constexpr int kBwdThreads = 128;
+// A CTA of the first launch takes up to 4 segments of kSplitKeys keys (16 keys per thread); dense-but-even fields
+// (config 3: ~1000 keys in every brick) then run as one launch, only truly hot bricks spill into the second.
+constexpr int kBwdMainSegments = 4;
 
 __device__ __forceinline__ float ex2b(float x)
 {
@@ -134,18 +137,13 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
     }
 }
 
+// Keys [kbeg, kend) of brick b (a whole brick, or one kSplitKeys segment of a hot one): gradient tile, then thread per key.
 template <int CH, bool SINGLE>
-__global__ void __launch_bounds__(kBwdThreads)
-k_backward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
-           const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
-           const float* __restrict__ weight, int wstride, int c0,
-           const float* __restrict__ grad_out, float* __restrict__ acc, int astride, GridDev gd)
+__device__ __forceinline__ void backward_brick(const GsRec* __restrict__ rec, const uint32_t* __restrict__ keys,
+                                               const float* __restrict__ weight, int wstride, int c0,
+                                               const float* __restrict__ grad_out, float* __restrict__ acc, int astride,
+                                               const GridDev& gd, float* __restrict__ s_g, int b, uint32_t kbeg, uint32_t kend)
 {
-    __shared__ __align__(16) float s_g[CH * kBrickVox];
-    if (status->overflow) return;
-    const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];      // z-slab of this plan
-    const uint32_t kbeg = bin_start[b * kNumClasses], kend = bin_start[(b + 1) * kNumClasses];
-    if (kbeg == kend) return;
     const int tid = threadIdx.x;
     const int bx = b % gd.nb[0], by = (b / gd.nb[0]) % gd.nb[1], bz = b / (gd.nb[0] * gd.nb[1]);
     const int b0x = bx * kBrick, b0y = by * kBrick, b0z = bz * kBrick;
@@ -224,6 +222,45 @@ k_backward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start
     }
 }
 
+// First launch: one CTA per brick, segment 0 of its key range.
+template <int CH, bool SINGLE>
+__global__ void __launch_bounds__(kBwdThreads)
+k_backward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
+           const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
+           const float* __restrict__ weight, int wstride, int c0,
+           const float* __restrict__ grad_out, float* __restrict__ acc, int astride, GridDev gd)
+{
+    __shared__ __align__(16) float s_g[CH * kBrickVox];
+    if (status->overflow) return;
+    const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];      // z-slab of this plan
+    const uint32_t kbeg = bin_start[b * kNumClasses];
+    const uint32_t kend = min(bin_start[(b + 1) * kNumClasses], kbeg + (uint32_t)(kBwdMainSegments * kSplitKeys));
+    if (kbeg == kend) return;
+    backward_brick<CH, SINGLE>(rec, keys, weight, wstride, c0, grad_out, acc, astride, gd, s_g, b, kbeg, kend);
+}
+
+// Second launch: the later segments of hot bricks (a2's item list), a fixed grid striding over the items.
+template <int CH, bool SINGLE>
+__global__ void __launch_bounds__(kBwdThreads)
+k_backward_extra(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
+                 const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
+                 const uint2* __restrict__ split_list, int split_cap,
+                 const float* __restrict__ weight, int wstride, int c0,
+                 const float* __restrict__ grad_out, float* __restrict__ acc, int astride, GridDev gd)
+{
+    __shared__ __align__(16) float s_g[CH * kBrickVox];
+    if (status->overflow) return;
+    const uint32_t nitems = min(status->nsplit, (uint32_t)split_cap);
+    for (uint32_t i = blockIdx.x; i < nitems; i += gridDim.x) {
+        const uint2 item = split_list[i];
+        if (item.y < (uint32_t)kBwdMainSegments) continue;          // the first launch took these (CTA-uniform)
+        const uint32_t kbeg = bin_start[item.x * kNumClasses] + item.y * (uint32_t)kSplitKeys;
+        const uint32_t kend = min(bin_start[(item.x + 1) * kNumClasses], kbeg + (uint32_t)kSplitKeys);
+        __syncthreads();                                            // the previous item's tile is no longer read
+        backward_brick<CH, SINGLE>(rec, keys, weight, wstride, c0, grad_out, acc, astride, gd, s_g, (int)item.x, kbeg, kend);
+    }
+}
+
 template <int CH, bool SINGLE>
 static int launch_bwd_ch(gsvox_plan* p, const float* weight, int C, int c0, const float* grad_out,
                          int astride, cudaStream_t st)
@@ -233,6 +270,11 @@ static int launch_bwd_ch(gsvox_plan* p, const float* weight, int C, int c0, cons
     LaunchScope ls(p, GSVOX_K_BACKWARD, st);
     k_backward<CH, SINGLE><<<nblocks, kBwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight,
                                                                   C, c0, grad_out, p->acc, astride, p->gd);
+    GSVOX_CUDA(cudaGetLastError());
+    p->launches[GSVOX_K_BACKWARD] += 1;              // the hot-brick launch
+    k_backward_extra<CH, SINGLE><<<kSplitGrid / 2, kBwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status,
+                                                                         p->split_list, p->split_cap, weight, C, c0,
+                                                                         grad_out, p->acc, astride, p->gd);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }

@@ -264,6 +264,10 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
 constexpr int kB1Batch = 32;
 constexpr int kB1Words = 20;                        // staged record; also the stride of the raw copy (16 words, padded): conflict-free 128-bit per-lane access
 
+__device__ __forceinline__ void red_add_v4f(float* addr, float a, float b, float c, float d)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" :: "l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
 __device__ __forceinline__ void cp_async16(uint32_t saddr, const void* g)
 { asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" :: "r"(saddr), "l"(g) : "memory"); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
@@ -379,18 +383,15 @@ __device__ __forceinline__ void eval_key_half(const float* __restrict__ r, uint3
     recur_accumulate(E3, Lf, wa, wb, acc);
 }
 
-template <bool VEC>
-__global__ void __launch_bounds__(32, 32)
-k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
-             const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
-             const float* __restrict__ weight, int wstride, int c0,
-             float* __restrict__ out, GridDev gd)
+// Keys [kbeg, kend) of brick b.  ADD = false: the brick's rows are stored (segment 0; zeros for an empty brick);
+// ADD = true: a later segment of a hot brick, added atomically to what segment 0 stored.
+template <bool VEC, bool ADD>
+__device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const uint32_t* __restrict__ keys,
+                                         const float* __restrict__ weight, int wstride, int c0, float* __restrict__ out,
+                                         const GridDev& gd, float* __restrict__ s_raw, float* __restrict__ s_rec,
+                                         int b, uint32_t kbeg, uint32_t kend)
 {
-    __shared__ __align__(16) float s_raw[kB1Batch * kB1Words];
-    __shared__ __align__(16) float s_rec[kB1Batch * kB1Words];
-
     const int lane = threadIdx.x;
-    const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];
     const int bx = b % gd.nb[0], by = (b / gd.nb[0]) % gd.nb[1], bz = b / (gd.nb[0] * gd.nb[1]);
     const int b0x = bx * kBrick, b0y = by * kBrick, b0z = bz * kBrick;
     const int ry = lane & 7, rz = lane >> 3;                        // rows (ry, rz) and (ry, rz + 4)
@@ -401,9 +402,6 @@ k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_sta
     float acc0[8], acc1[8];                         // acc[2j], acc[2j+1] = voxels 3 - j, 4 + j
     #pragma unroll
     for (int j = 0; j < 8; ++j) { acc0[j] = 0.f; acc1[j] = 0.f; }
-
-    uint32_t kbeg = 0, kend = 0;
-    if (!status->overflow) { kbeg = bin_start[b * kNumClasses]; kend = bin_start[(b + 1) * kNumClasses]; }
 
     const uint32_t raw_addr = (uint32_t)__cvta_generic_to_shared(s_raw + lane * kB1Words);
     auto fetch = [&](uint32_t gid) {                // this lane's record -> s_raw, asynchronously
@@ -493,7 +491,7 @@ k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_sta
         for (; j < n3; ++j) eval_key_half<true>(s_rec + j * kB1Words, lanebit, fy, fz + 4.0f, acc1);
     }
 
-    // write the two rows once (zeros for empty bricks); x fastest
+    // write (or add) the two rows; x fastest
     const size_t plane = (size_t)gd.dims[0] * gd.dims[1] * gd.dims[2];
     #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -505,14 +503,60 @@ k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_sta
             for (int j = 0; j < 4; ++j) { v[3 - j] = h ? acc1[2 * j] : acc0[2 * j]; v[4 + j] = h ? acc1[2 * j + 1] : acc0[2 * j + 1]; }
             float* o = out + (size_t)c0 * plane + rowoff;
             if (VEC) {
-                if (b0x + 3 < gd.dims[0]) __stcs(reinterpret_cast<float4*>(o), make_float4(v[0], v[1], v[2], v[3]));
-                if (b0x + 7 < gd.dims[0]) __stcs(reinterpret_cast<float4*>(o) + 1, make_float4(v[4], v[5], v[6], v[7]));
+                if (ADD) {
+                    if (b0x + 3 < gd.dims[0]) red_add_v4f(o, v[0], v[1], v[2], v[3]);
+                    if (b0x + 7 < gd.dims[0]) red_add_v4f(o + 4, v[4], v[5], v[6], v[7]);
+                } else {
+                    if (b0x + 3 < gd.dims[0]) __stcs(reinterpret_cast<float4*>(o), make_float4(v[0], v[1], v[2], v[3]));
+                    if (b0x + 7 < gd.dims[0]) __stcs(reinterpret_cast<float4*>(o) + 1, make_float4(v[4], v[5], v[6], v[7]));
+                }
             } else {
                 #pragma unroll
                 for (int k2 = 0; k2 < 8; ++k2)
-                    if (b0x + k2 < gd.dims[0]) o[k2] = v[k2];
+                    if (b0x + k2 < gd.dims[0]) { if (ADD) atomicAdd(o + k2, v[k2]); else o[k2] = v[k2]; }
             }
         }
+    }
+}
+
+// First launch: one warp per brick, segment 0 of its key range.
+template <bool VEC>
+__global__ void __launch_bounds__(32, 32)
+k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
+             const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
+             const float* __restrict__ weight, int wstride, int c0,
+             float* __restrict__ out, GridDev gd)
+{
+    __shared__ __align__(16) float s_raw[kB1Batch * kB1Words];
+    __shared__ __align__(16) float s_rec[kB1Batch * kB1Words];
+    const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];
+    uint32_t kbeg = 0, kend = 0;
+    if (!status->overflow) {
+        kbeg = bin_start[b * kNumClasses];
+        kend = min(bin_start[(b + 1) * kNumClasses], kbeg + (uint32_t)kSplitKeys);
+    }
+    b1_brick<VEC, false>(rec, keys, weight, wstride, c0, out, gd, s_raw, s_rec, b, kbeg, kend);
+}
+
+// Second launch: the later segments of hot bricks, a fixed grid striding over a2's item list.
+template <bool VEC>
+__global__ void __launch_bounds__(32, 32)
+k_forward_b1_extra(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
+                   const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
+                   const uint2* __restrict__ split_list, int split_cap,
+                   const float* __restrict__ weight, int wstride, int c0,
+                   float* __restrict__ out, GridDev gd)
+{
+    __shared__ __align__(16) float s_raw[kB1Batch * kB1Words];
+    __shared__ __align__(16) float s_rec[kB1Batch * kB1Words];
+    if (status->overflow) return;
+    const uint32_t nitems = min(status->nsplit, (uint32_t)split_cap);
+    for (uint32_t i = blockIdx.x; i < nitems; i += gridDim.x) {
+        const uint2 item = split_list[i];
+        const uint32_t kbeg = bin_start[item.x * kNumClasses] + item.y * (uint32_t)kSplitKeys;
+        const uint32_t kend = min(bin_start[(item.x + 1) * kNumClasses], kbeg + (uint32_t)kSplitKeys);
+        __syncwarp();
+        b1_brick<VEC, true>(rec, keys, weight, wstride, c0, out, gd, s_raw, s_rec, (int)item.x, kbeg, kend);
     }
 }
 
@@ -524,6 +568,12 @@ static int launch_fwd_b1(gsvox_plan* p, const float* weight, int C, int c0, floa
     if (nblocks <= 0) return GSVOX_OK;
     if (vec) k_forward_b1<true><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd);
     else     k_forward_b1<false><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd);
+    GSVOX_CUDA(cudaGetLastError());
+    p->launches[GSVOX_K_FORWARD] += 1;               // the hot-brick launch
+    if (vec) k_forward_b1_extra<true><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
+                                                                 p->split_cap, weight, C, c0, out, p->gd);
+    else     k_forward_b1_extra<false><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
+                                                                  p->split_cap, weight, C, c0, out, p->gd);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }

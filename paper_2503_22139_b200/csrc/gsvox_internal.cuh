@@ -50,6 +50,8 @@ struct DevStatus {
     unsigned int overflow;
     unsigned long long culled;        // keys dropped by the conservative q_min > 64 test (reading A15)
     unsigned long long pairs_exec;    // P_exec: pairs of the kept keys
+    unsigned int nsplit;              // extra key-range segments of hot bricks (entries of the split list)
+    unsigned int pad_;
 };
 
 struct GridDev {
@@ -64,7 +66,19 @@ struct GridDev {
 constexpr int kBrick = GSVOX_BRICK;
 constexpr int kBrickVox = kBrick * kBrick * kBrick;
 constexpr int kScanItemsPerBlock = 2048;     // k_scan_*: 256 threads x 8 items
-constexpr float kRecurrenceMaxA = 1.0f;      // rows with A > 1 (narrow along x) take one EX2 per voxel
+// Rows with A > kRecurrenceMaxA (narrower than ~0.54 voxel along x, conditional sigma) take one EX2 per voxel; the
+// others the multiplicative recurrence.  2.5 is what the recurrence's own safety argument allows: the start value
+// G(3) can underflow while another voxel of the row is still above 2^-20 only if (106 - 16 A)^2 / (64 A) < 20, i.e.
+// A > 2.8; the un-damped geometric chain of a3 peaks at 2^(12 A) = 2^30.  (Round 1 used 1.0: config 5's blobs,
+// scales log-uniform 0.5-2, then had 38 % direct keys at ~3x the cost; at 2.5 it is 5 %.)
+constexpr float kRecurrenceMaxA = 2.5f;
+// Hot bricks (SURVEY section 7 hard part 6; config 5: 1.9e4 keys in one brick against a mean of ~100): a brick's CTA
+// of a3 (C = 1) and a4 walks at most kSplitKeys keys, segment 0 of the brick's key range; the segments beyond are
+// listed by a2 as (brick, segment) items and worked off by a second, grid-stride launch whose CTAs accumulate
+// atomically (a3: red.global.add into the volume the first launch wrote; a4 accumulates atomically anyway).
+// No CTA then carries more than kSplitKeys keys, whatever the density.
+constexpr int kSplitKeys = 512;
+constexpr int kSplitGrid = 148 * 16;         // CTAs of the second launch (each strides over the item list)
 
 // Bins of the counting sort are (brick, class): inside a brick, keys are ordered so that the 32
 // keys a backward warp works on have similar trip counts (a4 runs one THREAD per key and walks
@@ -127,6 +141,8 @@ struct gsvox_plan {
     uint32_t* bin_start;       // [nbins+1]  exclusive scan of counts
     uint32_t* scan_partial;    // [scan blocks]
     uint32_t* keys;            // [key_capacity] Gaussian id per key, grouped by brick
+    uint2* split_list;         // [split_cap] (brick, segment >= 1) items of hot bricks
+    int split_cap;
     float* acc;                // [n_max * acc_stride(max_channels)] backward accumulators
     int nbins;
     // timing

@@ -190,9 +190,23 @@ __device__ __forceinline__ bool key_negligible(const GsRec* __restrict__ rec, co
 template <int MODE>
 __global__ void __launch_bounds__(256, 6)       // <= 40 registers: the kernel lives on atomics in flight, i.e. on resident warps
 k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, GridDev gd,
-       uint32_t* __restrict__ bin_count, uint32_t* __restrict__ keys, DevStatus* __restrict__ status)
+       uint32_t* __restrict__ bin_count, uint32_t* __restrict__ keys, DevStatus* __restrict__ status,
+       const uint32_t* __restrict__ bin_start, uint2* __restrict__ split_list, int split_cap)
 {
     if (MODE == 1 && status->overflow) return;
+    if (MODE == 1) {
+        // the scan is done: list the key-range segments beyond the first of every hot brick (kSplitKeys)
+        const int b_lo = gd.slab0 * gd.nb[0] * gd.nb[1], b_hi = gd.slab1 * gd.nb[0] * gd.nb[1];
+        for (int b = b_lo + blockIdx.x * blockDim.x + threadIdx.x; b < b_hi; b += gridDim.x * blockDim.x) {
+            const uint32_t nk = bin_start[(b + 1) * kNumClasses] - bin_start[b * kNumClasses];
+            if (nk > (uint32_t)kSplitKeys) {
+                const uint32_t extra = (nk - 1u) / (uint32_t)kSplitKeys;
+                const uint32_t at = atomicAdd(&status->nsplit, extra);
+                for (uint32_t sgm = 0; sgm < extra; ++sgm)
+                    if (at + sgm < (uint32_t)split_cap) split_list[at + sgm] = make_uint2((uint32_t)b, sgm + 1u);
+            }
+        }
+    }
     __shared__ unsigned long long s_pairs;
     __shared__ unsigned int s_culled;
     if (MODE == 0) {
@@ -385,7 +399,8 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
     int kblocks = (int)((n * 8 + 255) / 256);
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_COUNT, st);
-        k_keys<0><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status);
+        k_keys<0><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status,
+                                           p->bin_start, p->split_list, p->split_cap);
         GSVOX_CUDA(cudaGetLastError());
     }
     { LaunchScope ls(p, GSVOX_K_SCAN, st);
@@ -395,7 +410,8 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
       if (rc != GSVOX_OK) return rc; }
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_SCATTER, st);
-        k_keys<1><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status);
+        k_keys<1><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status,
+                                           p->bin_start, p->split_list, p->split_cap);
         GSVOX_CUDA(cudaGetLastError());
     }
     return GSVOX_OK;

@@ -23,6 +23,8 @@
 #include "gsvox_internal.cuh"
 
 namespace gsvox {
+constexpr float kSplatRecurrenceMaxA = 1.0f;   // footprints narrower than ~0.85 pixel along a row: one EX2 per pixel
+
 
 constexpr int kSplatTile = 16;
 constexpr int kSplatMaxBatch = 64;
@@ -296,7 +298,7 @@ k_splat_forward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* 
             t.cx = (float)(r.ciu - ox) + r.cfu; t.cy = (float)(r.civ - oy) + r.cfv;
             t.A = r.A; t.Bq = r.Bq; t.Dq = r.Dq; t.cc = ex2s(2.f * r.A);
             t.rowmask = ((2u << y1) - (1u << y0)) & 0xffffu;
-            t.direct = (-r.A > kRecurrenceMaxA) ? 1u : 0u;
+            t.direct = (-r.A > kSplatRecurrenceMaxA) ? 1u : 0u;
             const uint32_t xm = ((2u << x1) - (1u << x0)) & 0xffffu;
             #pragma unroll
             for (int s2 = 0; s2 < 2; ++s2)

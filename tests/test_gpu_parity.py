@@ -180,7 +180,7 @@ def test_single_isolated_gaussians_worst_case_tolerance(pkg):
     row recurrence.  Sweeps sub-voxel offsets, scales around the recurrence/direct switch, rotations."""
     rng = np.random.default_rng(5)
     dims = (40, 40, 40)
-    for s0 in (0.5, 0.8, 0.84, 0.86, 1.0, 1.3, 2.0, 4.5):
+    for s0 in (0.45, 0.5, 0.52, 0.535, 0.54, 0.56, 0.6, 0.7, 0.84, 1.0, 1.3, 2.0, 4.5):
         for rep in range(4):
             case = gsvox_inputs.config1(n=1, dims=dims, seed=1000 + rep)
             case.pos[:] = (19.5 + rng.uniform(-4, 4, 3)).astype(np.float32)
