@@ -158,9 +158,13 @@ k_preprocess(const float* __restrict__ pos, const float* __restrict__ scale,
 // pay nothing (unflagged: 0.23 ms of binning at config 4; testing every key cost 0.31 ms).
 // ------------------------------------------------------------------------------------------
 
-// The brick test of one flagged Gaussian (everything recomputed per brick: only needles get here).
-__device__ __forceinline__ bool key_negligible(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int g,
-                                            float h0, float h1, float h2, int bx, int by, int bz)
+// The brick test of one flagged Gaussian, in two parts.  cull_setup (once per Gaussian and pass): each principal
+// coordinate t_k of a brick centre is affine in the brick's offset (tx, ty, tz) from the first brick of the box,
+//     c_k = c0_k + tx ax_k + ty ay_k + tz az_k,     and spans +- half_k over the brick;
+// 15 floats, kept in shared memory (one set per 8-lane group).  key_negligible (per brick): 9 FMA + 3 x 4.
+// (Round 1 rebuilt R from the quaternion for every brick: ~70 instructions per test, 2.9e7 tests per pass at config 5.)
+__device__ __forceinline__ void cull_setup(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int g,
+                                           float h0, float h1, float h2, int bx0, int by0, int bz0, float* __restrict__ cq)
 {
     const int4* rp = reinterpret_cast<const int4*>(rec + g);
     const int4 w0 = __ldg(rp), w1 = __ldg(rp + 1);                        // cf, cexp | ci, negA
@@ -173,15 +177,25 @@ __device__ __forceinline__ bool key_negligible(const GsRec* __restrict__ rec, co
                           2.f * (x * y + r * z) * h1, (1.f - 2.f * (x * x + z * z)) * h1, 2.f * (y * z - r * x) * h1,
                           2.f * (x * z - r * y) * h2, 2.f * (y * z + r * x) * h2, (1.f - 2.f * (x * x + y * y)) * h2 };
     const float is[3] = { 1.f / sa.x, 1.f / sa.y, 1.f / sa.z };
-    const float d0 = (float)(8 * bx - w1.x) + (3.5f - __int_as_float(w0.x));
-    const float d1 = (float)(8 * by - w1.y) + (3.5f - __int_as_float(w0.y));
-    const float d2 = (float)(8 * bz - w1.z) + (3.5f - __int_as_float(w0.z));
+    const float d0 = (float)(8 * bx0 - w1.x) + (3.5f - __int_as_float(w0.x));      // centre of the first brick
+    const float d1 = (float)(8 * by0 - w1.y) + (3.5f - __int_as_float(w0.y));
+    const float d2 = (float)(8 * bz0 - w1.z) + (3.5f - __int_as_float(w0.z));
+    #pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        cq[5 * k + 0] = (Rm[k] * d0 + Rm[3 + k] * d1 + Rm[6 + k] * d2) * is[k];
+        cq[5 * k + 1] = 8.f * Rm[k] * is[k]; cq[5 * k + 2] = 8.f * Rm[3 + k] * is[k]; cq[5 * k + 3] = 8.f * Rm[6 + k] * is[k];
+        cq[5 * k + 4] = 3.5f * (fabsf(Rm[k]) + fabsf(Rm[3 + k]) + fabsf(Rm[6 + k])) * is[k];
+    }
+}
+
+__device__ __forceinline__ bool key_negligible(const float* __restrict__ cq, int tx, int ty, int tz)
+{
+    const float fx = (float)tx, fy = (float)ty, fz = (float)tz;
     float qmin = 0.f;
     #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        const float c = (Rm[k] * d0 + Rm[3 + k] * d1 + Rm[6 + k] * d2) * is[k];
-        const float half = 3.5f * (fabsf(Rm[k]) + fabsf(Rm[3 + k]) + fabsf(Rm[6 + k])) * is[k];
-        const float dist = fmaxf(fabsf(c) - half, 0.f);
+        const float c = fmaf(fz, cq[5 * k + 3], fmaf(fy, cq[5 * k + 2], fmaf(fx, cq[5 * k + 1], cq[5 * k])));
+        const float dist = fmaxf(fabsf(c) - cq[5 * k + 4], 0.f);
         qmin = fmaf(dist, dist, qmin);
     }
     return qmin > kCullQ;
@@ -233,6 +247,21 @@ k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, Grid
         }
         cullable = (total > 1) && (__ldg(reinterpret_cast<const int*>(rec + g) + 3) < 0);   // sign bit of cexp
     }
+    // Flagged Gaussians (needles: boxes of hundreds of bricks, most of them culled) are not walked by their own 8
+    // lanes while the other 24 lanes of the warp sit idle behind a 1-trip neighbour: their parameters are parked in
+    // shared memory and, after the ordinary keys, the whole warp walks them one after another, 32 bricks per trip.
+    __shared__ float s_cull[32][16];
+    __shared__ int s_par[32][12];
+    if (cullable && sub == 0) {
+        cull_setup(rec, aux, g, (float)gd.spacing[0], (float)gd.spacing[1], (float)gd.spacing[2], bx0, by0, bz0,
+                   s_cull[threadIdx.x >> 3]);
+        int* sp = s_par[threadIdx.x >> 3];
+        sp[0] = g; sp[1] = total; sp[2] = lox; sp[3] = loy; sp[4] = loz; sp[5] = hix; sp[6] = hiy; sp[7] = hiz;
+        sp[8] = bx0 | (by0 << 16); sp[9] = bz0; sp[10] = ex | (ey << 16); sp[11] = direct ? 1 : 0;
+    }
+    uint32_t parked = __ballot_sync(0xffffffffu, cullable && sub == 0);
+    if (cullable) total = 0;
+    __syncwarp();
     // t -> (tx, ty, tz) by reciprocal multiplies with a +-1 fix-up (exact while total < 2^23); the two
     // integer div/mod pairs were ~half of the 147 thread instructions per key ncu counted in this kernel
     const float inv_ex = __frcp_rn((float)ex), inv_ey = __frcp_rn((float)ey);
@@ -249,8 +278,6 @@ k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, Grid
             if (ty < 0) { --tz; ty += ey; }
         } else { tx = t % ex; r = t / ex; ty = r % ey; tz = r / ey; }
         const int bx = bx0 + tx, by = by0 + ty, bz = bz0 + tz;
-        if (cullable && key_negligible(rec, aux, g, (float)gd.spacing[0], (float)gd.spacing[1], (float)gd.spacing[2],
-                                       bx, by, bz)) { my_culled += 1u; return -1; }
         const int x0 = max(lox - 8 * bx, 0), x1 = min(hix - 8 * bx, 7), y0 = max(loy - 8 * by, 0), y1 = min(hiy - 8 * by, 7);
         const int z0 = max(loz - 8 * bz, 0), z1 = min(hiz - 8 * bz, 7);
         if (MODE == 0) my_pairs += (unsigned)((x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1));
@@ -268,6 +295,26 @@ k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, Grid
             if (b1 >= 0) s1 = atomicAdd(&bin_count[b1], 1u);
             if (b0 >= 0) keys[s0] = (uint32_t)g;
             if (b1 >= 0) keys[s1] = (uint32_t)g;
+        }
+    }
+    // the parked (flagged) Gaussians of this warp, one after another, 32 bricks per trip
+    while (parked) {                                     // warp-uniform
+        const int grp = (threadIdx.x >> 5) * 4 + ((__ffs(parked) - 1) >> 3);
+        parked &= parked - 1u;
+        const int* sp = s_par[grp];
+        const float* cq = s_cull[grp];
+        const int pg = sp[0], ptotal = sp[1], pex = sp[10] & 0xffff, pey = sp[10] >> 16;
+        const bool pdirect = sp[11] != 0;
+        for (int t = (int)(threadIdx.x & 31); t < ptotal; t += 32) {
+            const int tx = t % pex, r = t / pex, ty = r % pey, tz = r / pey;
+            if (key_negligible(cq, tx, ty, tz)) { my_culled += 1u; continue; }
+            const int bx = (sp[8] & 0xffff) + tx, by = (sp[8] >> 16) + ty, bz = sp[9] + tz;
+            const int x0 = max(sp[2] - 8 * bx, 0), x1 = min(sp[5] - 8 * bx, 7), y0 = max(sp[3] - 8 * by, 0), y1 = min(sp[6] - 8 * by, 7);
+            const int z0 = max(sp[4] - 8 * bz, 0), z1 = min(sp[7] - 8 * bz, 7);
+            if (MODE == 0) my_pairs += (unsigned)((x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1));
+            const int bin = ((bz * gd.nb[1] + by) * gd.nb[0] + bx) * kNumClasses + key_class(pdirect, x0, x1, y0, y1, z0, z1);
+            if (MODE == 0) atomicAdd(&bin_count[bin], 1u);
+            else keys[atomicAdd(&bin_count[bin], 1u)] = (uint32_t)pg;
         }
     }
     if (MODE == 0) {
