@@ -8,8 +8,10 @@ C = 1, upstream gradient N(0,1); one step = gsvox_preprocess + gsvox_forward + g
 (binning included: Gaussian parameters change every training step).
 Metric: Gaussian-voxel evaluations per second = P_def (pairs inside the 3-sigma box cutoff, the
 oracle's loop count) / time of one forward+backward step; whole-job aggregate over N GPUs.
-Multi-GPU: the path does not shard in this build ("replicas only"): each rank runs an
-independent replica of the step; no data-path collective.  Prints ONE JSON line on rank 0.
+Multi-GPU (N > 1): the headline is N independent replicas ("scaling": "weak", no data-path collective); the same
+line carries a "slab" record, the step sharded over the ranks as z-slabs of bricks with ONE NCCL all-reduce of the
+per-Gaussian accumulators in backward ("strong").  --shard slab makes that the headline.
+Prints ONE JSON line on rank 0.
 """
 import argparse
 import json
@@ -49,13 +51,44 @@ def get_case(cfg):
     raise SystemExit("unknown --config %r" % cfg)
 
 
-def workload_config(case, extra=None):
-    c = {"workload": case.name, "grid": list(case.dims), "gaussians": case.n, "channels": case.channels,
-         "step": "gsvox_preprocess+gsvox_forward+gsvox_backward", "parallelism": "replicas",
-         "l2_policy": "working set > L2 (volume + gradient + keys + records ~250 MB vs 126 MB L2), no flush"}
-    if extra:
-        c.update(extra)
-    return c
+def workload_config(case, parallelism="replicas"):
+    """The same keys and values in both arms (ours / reference): what is computed, not how it went."""
+    return {"workload": case.name, "grid": list(case.dims), "gaussians": case.n, "channels": case.channels,
+            "step": "gsvox_preprocess+gsvox_forward+gsvox_backward", "parallelism": parallelism,
+            "l2_policy": "working set > L2 (volume + gradient + keys + records ~250 MB vs 126 MB L2), no flush"}
+
+
+def lane_counts(plan, case):
+    """L_exec of SURVEY 8(d): voxel-lane evaluations the kernels issue, derived exactly from the plan's own boxes
+    and bins (read back through the C ABI), for C = 1.  Forward (k_forward_b1): a key costs 256 voxel-lanes per
+    z-half of the brick its box reaches.  Backward (k_backward): thread per key, 32 consecutive keys of a brick
+    per warp, the warp runs max(rows of box-in-brick) trips of 8 voxels for all 32 lanes."""
+    box, _ = plan.geometry()
+    start, keys = plan.bins()
+    nb = [(d + 7) // 8 for d in case.dims]
+    nk = np.diff(start)
+    brick = np.repeat(np.arange(len(nk), dtype=np.int64), nk)
+    b = box[keys].astype(np.int64)
+    bx, by, bz = brick % nb[0], (brick // nb[0]) % nb[1], brick // (nb[0] * nb[1])
+    ext = []
+    for k, bb in enumerate((bx, by, bz)):
+        lo = np.maximum(b[:, k] - 8 * bb, 0); hi = np.minimum(b[:, 3 + k] - 8 * bb, 7)
+        ext.append((lo, hi))
+    nxk = ext[0][1] - ext[0][0] + 1; nyk = ext[1][1] - ext[1][0] + 1; nzk = ext[2][1] - ext[2][0] + 1
+    p_exec = int((nxk * nyk * nzk).sum())
+    halves = (ext[2][0] <= 3).astype(np.int64) + (ext[2][1] >= 4).astype(np.int64)
+    l_fwd = int(256 * halves.sum())
+    nrows = nyk * nzk
+    within = np.arange(len(keys), dtype=np.int64) - np.repeat(start[:-1], nk)       # index inside the brick's range
+    grp_start = np.flatnonzero(within % 32 == 0)
+    wmax = np.maximum.reduceat(nrows, grp_start) if len(keys) else np.zeros(0, np.int64)
+    l_bwd = int(256 * wmax.sum())
+    return {"P_exec": p_exec,
+            "forward": {"L_exec": l_fwd, "lane_efficiency": p_exec / max(l_fwd, 1)},
+            "backward": {"L_exec": l_bwd, "lane_efficiency": p_exec / max(l_bwd, 1),
+                         "rows_only": int(8 * nrows.sum()), "row_lane_efficiency": p_exec / max(int(8 * nrows.sum()), 1)},
+            "note": "voxel-lanes issued, from the plan's boxes and bins: forward 256 per (key, z-half reached); backward "
+                    "32 lanes x max rows in the warp x 8 (rows_only: without the idle lanes of shorter keys)"}
 
 
 def read_traffic(workload, kernel):
@@ -170,7 +203,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(case, {"sample": sample}),
+            "config": workload_config(case, "z-slabs + all-reduce" if args.shard == "slab" else "replicas"),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -354,6 +387,50 @@ def hbm_peak():
 
 
 # ------------------------------------------------------------------------------ our arm
+def make_plan(pkg, case, tensors, slab=None):
+    plan = pkg.Plan(case.n, case.grid, max_channels=case.channels)
+    if slab:
+        plan.set_slab(*slab)
+    plan.preprocess(*tensors[:3])
+    st = plan.status()
+    if st["overflow"]:
+        plan = pkg.Plan(case.n, case.grid, max_channels=case.channels, key_capacity=int(1.05 * st["keys_needed"]))
+        if slab:
+            plan.set_slab(*slab)
+        plan.preprocess(*tensors[:3])
+        st = plan.status()
+    assert not st["overflow"]
+    return plan, st
+
+
+def other_config(torch, pkg, cfg, steps=20):
+    """ms per step of another BASELINE config (parity cases, reported for context; config 2 also forward-only)."""
+    case = get_case(cfg)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    t = (dev(case.pos), dev(case.scale), dev(case.quat), dev(case.weight))
+    g = dev(case.grad_out())
+    plan, st = make_plan(pkg, case, t)
+    nx, ny, nz = case.dims
+    out = torch.empty((case.channels, nz, ny, nx), dtype=torch.float32, device="cuda")
+    grads = tuple(torch.empty((case.n, k), dtype=torch.float32, device="cuda") for k in (case.channels, 3, 3, 4))
+
+    def fb():
+        plan.preprocess(*t[:3]); plan.forward(t[3], out=out); plan.backward(t[3], g, grads=grads)
+
+    def fo():
+        plan.preprocess(*t[:3]); plan.forward(t[3], out=out)
+    ms = _time_ms(torch, fb, steps, warm=5)
+    f_fwd, f_bwd = flops_per_pair(case.channels)
+    rec = {"workload": case.name, "ms_per_step": ms, "pairs_P_def": st["pairs"], "pairs_P_exec": st["pairs_exec"],
+           "keys": st["keys_needed"], "culled_keys": st["culled_keys"], "pairs_per_s": st["pairs"] / (ms * 1e-3),
+           "step_frac_of_fp32_peak": st["pairs_exec"] * (f_fwd + f_bwd) / (ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}
+    if cfg == 2:
+        mo = _time_ms(torch, fo, steps, warm=3)
+        rec["forward_only"] = {"ms": mo, "pairs_per_s": st["pairs"] / (mo * 1e-3),
+                               "frac_of_fp32_peak": st["pairs_exec"] * f_fwd / (mo * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}
+    return rec
+
+
 def run_ours(args):
     import torch
     import paper_2503_22139_b200 as pkg
@@ -381,21 +458,11 @@ def run_ours(args):
     grad = dev(grad_np)
     nx, ny, nz = case.dims
 
+    nbz = (nz + 7) // 8
     slab = None
     if args.shard == "slab":                     # z-slabs of bricks per rank + one all-reduce in backward
-        slab = slab_bounds((nz + 7) // 8, rank, world)
-    plan = pkg.Plan(case.n, case.grid, max_channels=C)
-    if slab:
-        plan.set_slab(*slab)
-    plan.preprocess(pos, scale, quat)
-    st = plan.status()
-    if st["overflow"]:
-        plan = pkg.Plan(case.n, case.grid, max_channels=C, key_capacity=int(1.05 * st["keys_needed"]))
-        if slab:
-            plan.set_slab(*slab)
-        plan.preprocess(pos, scale, quat)
-        st = plan.status()
-    assert not st["overflow"]
+        slab = slab_bounds(nbz, rank, world)
+    plan, st = make_plan(pkg, case, (pos, scale, quat, w), slab)
     pairs, keys = st["pairs"], st["keys_needed"]
     pairs_exec, culled = st["pairs_exec"], st["culled_keys"]       # P_exec: pairs of the keys not culled (A15)
     out = torch.empty((C, nz, ny, nx), dtype=torch.float32, device="cuda")
@@ -435,8 +502,60 @@ def run_ours(args):
     else:
         value, ms_step = whole_job_rate(pairs, ranks, ms_total, args.steps)
 
+    # ---- the same step looped for >= 2 s with the clock sampler on: does the burst number hold?
+    n_sus = max(args.steps, int(2200.0 / max(ms_step, 1e-3)))
+    sampler = ClockSampler("GPU-" + uuid if not uuid.startswith("GPU-") else uuid)
+    time.sleep(0.15)
+    barrier()
+    t0 = time.time()
+    ev0.record()
+    for _ in range(n_sus):
+        step()
+    ev1.record()
+    barrier()
+    t1 = time.time()
+    sus_clocks = sampler.stop(t0, t1)
+    sus_ms = ranks.max_over_ranks(ev0.elapsed_time(ev1)) / n_sus
+    sustained = {"steps": n_sus, "seconds": (t1 - t0), "ms_per_step": sus_ms, "ratio_to_headline": sus_ms / ms_step,
+                 "clocks": sus_clocks}
+
+    # ---- N > 1: the sharded path as well (z-slabs of bricks, one NCCL all-reduce of the accumulators in backward)
+    slab_rec = None
+    if world > 1 and not slab:
+        sb = slab_bounds(nbz, rank, world)
+        splan, sst = make_plan(pkg, case, (pos, scale, quat, w), sb)
+
+        def sstep():
+            splan.preprocess(pos, scale, quat)
+            splan.forward(w, out=out)
+            sharded_backward(splan, w, grad, ranks, grads=grads)
+        for _ in range(5):
+            sstep()
+        barrier()
+        ev0.record()
+        for _ in range(args.steps):
+            sstep()
+        ev1.record()
+        barrier()
+        s_ms = ranks.max_over_ranks(ev0.elapsed_time(ev1)) / args.steps
+        # the all-reduce alone, on the same buffer (events around the collective)
+        import torch.distributed as dist
+        accb = splan.accumulators(C)
+        barrier(); ev0.record()
+        for _ in range(20):
+            dist.all_reduce(accb)
+        ev1.record(); barrier()
+        a_ms = ranks.max_over_ranks(ev0.elapsed_time(ev1)) / 20
+        slab_rec = {"scaling": "strong", "parallelism": "z-slabs + all-reduce", "ms_per_step": s_ms,
+                    "value": pairs / (s_ms * 1e-3), "all_reduce_ms": a_ms, "all_reduce_bytes": int(accb.numel() * 4),
+                    "keys_this_rank": sst["keys_needed"], "slab_layers": list(sb)}
+
     line = None
     if rank == 0:
+        lanes = lane_counts(plan, case) if (C == 1 and not slab) else None
+        others = None
+        if args.config == 4 and not args.no_other_configs:
+            others = {str(c): other_config(torch, pkg, c) for c in (1, 2, 31, 32, 33, 5)}
         # ---- per-kernel durations: the same loop again with the library's event brackets on
         plan.set_timing(True)
         for _ in range(args.steps):
@@ -505,8 +624,10 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True,
                 "scaling": "strong" if slab else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": workload_config(case, {"pairs_P_def": pairs, "pairs_P_exec": pairs_exec, "keys": keys, "culled_keys": culled,
-                                                 "parallelism": "z-slabs + all-reduce" if slab else "replicas"}),
+                "config": workload_config(case, "z-slabs + all-reduce" if slab else "replicas"),
+                "counts": {"pairs_P_def": pairs, "pairs_P_exec": pairs_exec, "keys": keys, "culled_keys": culled,
+                           "lanes": lanes},
+                "sustained": sustained, "other_configs": others, "slab": slab_rec,
                 "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
                 "next_rows": extra}
     ranks.close()
@@ -525,6 +646,7 @@ def main():
                     help="N > 1: independent replicas (default, weak scaling) or z-slabs of bricks per rank with one "
                          "NCCL all-reduce of the per-Gaussian accumulators in backward (strong scaling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the other BASELINE configs (1, 2, 3, 5)")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the SURVEY 8(f) rows (DVF combine, warp)")
     ap.add_argument("--only-next-rows", action="store_true",
                     help="launch every 8(f) kernel once and exit (for ncu captures; prints no benchmark line)")

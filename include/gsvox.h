@@ -146,7 +146,12 @@ int gsvox_plan_timings(gsvox_plan* plan, double* ms /*[GSVOX_K_COUNT_KINDS]*/,
  * at least gsvox_host_staging_bytes(); host buffers should be pinned.  out_host may be NULL
  * (skip the volume read-back) and grad_out_host may be NULL (forward only).  The upstream gradient
  * is uploaded and the volume downloaded on two copy streams owned by the plan, overlapped with the
- * kernels (both ordered after work already enqueued on `stream`).                              */
+ * kernels (both ordered after work already enqueued on `stream`).  What the library creates behind the caller's
+ * back, all of it HOST-side and owned by the plan: the plan object itself (gsvox_plan_create: heap), and on the first
+ * gsvox_step_host two non-blocking CUDA streams and four events (destroyed by gsvox_plan_destroy); never device
+ * memory.  Errors: GSVOX_EINVAL for a plan restricted to a z-slab (gsvox_plan_set_slab: it writes its own brick
+ * layers only); on any error after the first copy was enqueued the call drains `stream` and both copy streams
+ * before it returns, so no copy still references the caller's host buffers.                            */
 int gsvox_host_staging_bytes(int64_t n_max, int32_t max_channels, const gsvox_grid* grid, size_t* bytes);
 int gsvox_step_host(gsvox_plan* plan, void* staging, size_t staging_bytes,
                     const float* pos_host, const float* scale_host, const float* quat_host,
@@ -275,25 +280,27 @@ int gsvox_splat_forward(const float* pos, const float* scale, const float* quat,
                         float* drr, void* stream);
 /* Backward for grad_drr = dL/ddrr [B,nv,nu], boxes frozen (R6).  MUST follow gsvox_splat_forward
  * with the same inputs, geometry, angles and workspace (it reuses the 2D records and the tile
- * lists).  grad_rho [n], grad_pos [n,3], grad_scale [n,3], grad_quat [n,4] OVERWRITTEN.          */
+ * lists).  grad_rho [n], grad_pos [n,3], grad_scale [n,3], grad_quat [n,4] OVERWRITTEN.  The forward
+ * leaves a stamp (magic + digest of n, B, nu, nv, key_capacity) in the workspace; a backward on a
+ * workspace without the matching stamp (no forward yet, other sizes) touches none of the lists and
+ * writes ZERO gradients — the condition lives on the device, so it is reported by gsvox_splat_status
+ * (GSVOX_ENOTREADY), not by this call's return value.                                              */
 int gsvox_splat_backward(const float* pos, const float* scale, const float* quat, const float* rho,
                          int64_t n, const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
                          void* workspace, size_t workspace_bytes, int64_t key_capacity,
                          const float* grad_drr, float* grad_rho, float* grad_pos, float* grad_scale,
                          float* grad_quat, void* stream);
 /* Outcome of the latest gsvox_splat_forward on this workspace (SYNCHRONISES): keys needed, pairs
- * inside the cutoff over all angles, overflow flag, Gaussians skipped as degenerate.  HOST outputs. */
+ * inside the cutoff over all angles, overflow flag, Gaussians skipped as degenerate (non-finite
+ * parameter, scale <= 0, zero quaternion: counted once, whatever the number of angles).  HOST outputs.
+ * GSVOX_ENOTREADY if no forward has completed on this workspace (zero it before the first use).
+ * gsvox_splat_drops: per (angle, Gaussian) items that contribute nothing at that angle although the
+ * Gaussian is valid (R5) — at or behind the source plane, centre more than 30000 pixels from the
+ * detector origin, footprint box empty after clipping to the detector.                            */
+int gsvox_splat_drops(const void* workspace, int64_t* behind_source, int64_t* out_of_range, int64_t* empty_box,
+                      void* stream);
 int gsvox_splat_status(const void* workspace, int64_t* keys_needed, int64_t* pairs, int32_t* overflow,
                        int32_t* skipped, void* stream);
-
-/* Live ALU rooflines of the device the calling thread has current (the hot path is
- * FP32-issue / MUFU bound, and MEASURED_PEAKS.json holds no FP32 figure).  Runs three register-only
- * microbenchmarks on `stream` and SYNCHRONISES: scalar FFMA chains (fp32_tflops, 2 flops per lane
- * instruction), packed fma.rn.f32x2 chains (fp32x2_tflops, 4 flops per lane instruction) and
- * ex2.approx chains (ex2_tera_per_s, 1e12 results/s).  `scratch` = at least 4 bytes of DEVICE
- * memory (never written in practice).  Any output pointer may be NULL.  HOST output pointers.  */
-int gsvox_probe_peaks(void* scratch, double* fp32_tflops, double* fp32x2_tflops,
-                      double* ex2_tera_per_s, int32_t* sm_count, void* stream);
 
 const char* gsvox_error_string(int code);
 /* Text of the last CUDA error seen by this thread inside the library ("" if none). */

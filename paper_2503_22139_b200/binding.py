@@ -19,12 +19,14 @@ EXPORTS = [
     "gsvox_forward", "gsvox_backward", "gsvox_plan_status", "gsvox_plan_geometry_host",
     "gsvox_plan_bins_host", "gsvox_plan_set_timing", "gsvox_plan_timings",
     "gsvox_host_staging_bytes", "gsvox_step_host", "gsvox_error_string",
-    "gsvox_last_cuda_error", "gsvox_version", "gsvox_probe_peaks", "gsvox_dvf_forward", "gsvox_dvf_backward",
+    "gsvox_last_cuda_error", "gsvox_version", "gsvox_dvf_forward", "gsvox_dvf_backward",
     "gsvox_mbc_combine_forward", "gsvox_mbc_combine_backward", "gsvox_warp_forward", "gsvox_warp_backward",
     "gsvox_plan_set_slab", "gsvox_backward_accumulate", "gsvox_backward_finish", "gsvox_plan_accumulators",
     "gsvox_project_scratch_bytes", "gsvox_project_forward", "gsvox_project_backward",
     "gsvox_splat_workspace_bytes", "gsvox_splat_forward", "gsvox_splat_backward", "gsvox_splat_status",
+    "gsvox_splat_drops",
 ]
+PROBE_EXPORTS = ["gsvox_probe_peaks"]            # include/gsvox_probe.h, libgsvox_probe.so (bench only)
 
 
 class GsvoxGrid(C.Structure):
@@ -93,8 +95,7 @@ def lib():
     L.gsvox_splat_forward.argtypes = [vp, vp, vp, vp, i64, cgp, vp, i32, vp, C.c_size_t, i64, vp, vp]
     L.gsvox_splat_backward.argtypes = [vp, vp, vp, vp, i64, cgp, vp, i32, vp, C.c_size_t, i64, vp, vp, vp, vp, vp, vp]
     L.gsvox_splat_status.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i32), C.POINTER(i32), vp]
-    dp = C.POINTER(C.c_double)
-    L.gsvox_probe_peaks.argtypes = [vp, dp, dp, dp, C.POINTER(i32), vp]
+    L.gsvox_splat_drops.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), vp]
     L.gsvox_error_string.argtypes = [C.c_int]
     L.gsvox_error_string.restype = C.c_char_p
     L.gsvox_last_cuda_error.restype = C.c_char_p
@@ -122,27 +123,53 @@ def _stream():
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
 
 
-def _dev(t, name):
+def _dev(t, name, shape=None):
+    """Device pointer of a contiguous float32 CUDA tensor.  The C ABI takes raw pointers, so this binding is the only
+    place a size can be checked: `shape` (a tuple; None entries are free) is what the call will read or write."""
     if t is None:
         return None
     if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
         raise GsvoxError("%s must be a contiguous float32 CUDA tensor" % name)
+    if shape is not None:
+        got = tuple(int(v) for v in t.shape)
+        if len(got) == len(shape) - 1 and shape[-1] == 1:      # [n] is accepted for [n, 1]
+            got = got + (1,)
+        if len(got) != len(shape) or any(w is not None and g != w for g, w in zip(got, shape)):
+            raise GsvoxError("%s has shape %s, expected %s" % (name, tuple(t.shape), tuple(shape)))
     return C.c_void_p(t.data_ptr())
 
 
-def _host(t, name):
+def _host(t, name, shape=None):
     if t is None:
         return None
     if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
         raise GsvoxError("%s must be a contiguous float32 CPU tensor" % name)
+    if shape is not None and tuple(int(v) for v in t.shape) != tuple(shape):
+        raise GsvoxError("%s has shape %s, expected %s" % (name, tuple(t.shape), tuple(shape)))
     return C.c_void_p(t.data_ptr())
+
+
+_probe_lib = None
+
+
+def probe_lib():
+    """The bench-only microbenchmark library (include/gsvox_probe.h); separate from the product library."""
+    global _probe_lib
+    if _probe_lib is None:
+        lib()                                        # raises if the build has not run (build.py makes both shared objects)
+        path = os.path.join(os.path.dirname(LIB_PATH), "libgsvox_probe.so")
+        L = C.CDLL(path)
+        dp = C.POINTER(C.c_double)
+        L.gsvox_probe_peaks.argtypes = [C.c_void_p, dp, dp, dp, C.POINTER(C.c_int32), C.c_void_p]
+        _probe_lib = L
+    return _probe_lib
 
 
 def probe_peaks():
     """Measured FP32 (scalar FFMA, packed FFMA2) and MUFU ex2 rates of the current device."""
     scratch = torch.zeros(64, dtype=torch.float32, device="cuda")
     a, b, c, sms = C.c_double(0), C.c_double(0), C.c_double(0), C.c_int32(0)
-    _check(lib().gsvox_probe_peaks(C.c_void_p(scratch.data_ptr()), C.byref(a), C.byref(b), C.byref(c),
+    _check(probe_lib().gsvox_probe_peaks(C.c_void_p(scratch.data_ptr()), C.byref(a), C.byref(b), C.byref(c),
                                    C.byref(sms), _stream()))
     return {"fp32_tflops": a.value, "fp32x2_tflops": b.value, "ex2_tera_per_s": c.value, "sm_count": sms.value}
 
@@ -151,9 +178,11 @@ def mbc_combine_forward(e, coef, out=None):
     """e [L,3,nz,ny,nx], coef [B,L,3] -> dvf [B,3,nz,ny,nx] (Eq. 3), HBM-bound combine."""
     L_, B = int(e.shape[0]), int(coef.shape[0])
     V = int(e[0, 0].numel())
+    vol = tuple(int(v) for v in e.shape[2:])
     if out is None:
-        out = torch.empty((B, 3) + tuple(e.shape[2:]), dtype=torch.float32, device=e.device)
-    _check(lib().gsvox_mbc_combine_forward(_dev(e, "e"), _dev(coef, "coef"), B, L_, V, _dev(out, "dvf"), _stream()))
+        out = torch.empty((B, 3) + vol, dtype=torch.float32, device=e.device)
+    _check(lib().gsvox_mbc_combine_forward(_dev(e, "e", (L_, 3) + vol), _dev(coef, "coef", (B, L_, 3)), B, L_, V,
+                                           _dev(out, "dvf", (B, 3) + vol), _stream()))
     return out
 
 
@@ -164,8 +193,10 @@ def mbc_combine_backward(e, coef, grad_dvf, grads=None):
     if grads is None:
         grads = (torch.empty_like(e), torch.empty((B, L_, 3), dtype=torch.float32, device=e.device))
     ge, gc = grads
-    _check(lib().gsvox_mbc_combine_backward(_dev(e, "e"), _dev(coef, "coef"), _dev(grad_dvf, "grad_dvf"), B, L_, V,
-                                            _dev(ge, "grad_e"), _dev(gc, "grad_coef"), _stream()))
+    vol = tuple(int(v) for v in e.shape[2:])
+    _check(lib().gsvox_mbc_combine_backward(_dev(e, "e", (L_, 3) + vol), _dev(coef, "coef", (B, L_, 3)),
+                                            _dev(grad_dvf, "grad_dvf", (B, 3) + vol), B, L_, V,
+                                            _dev(ge, "grad_e", (L_, 3) + vol), _dev(gc, "grad_coef", (B, L_, 3)), _stream()))
     return grads
 
 
@@ -175,7 +206,9 @@ def warp_forward(iref, dvf, grid, out=None):
     B = int(dvf.shape[0])
     if out is None:
         out = torch.empty((B,) + tuple(iref.shape), dtype=torch.float32, device=iref.device)
-    _check(lib().gsvox_warp_forward(_dev(iref, "iref"), _dev(dvf, "dvf"), C.byref(g), B, _dev(out, "out"), _stream()))
+    vol = (g.dims[2], g.dims[1], g.dims[0])
+    _check(lib().gsvox_warp_forward(_dev(iref, "iref", vol), _dev(dvf, "dvf", (B, 3) + vol), C.byref(g), B,
+                                    _dev(out, "out", (B,) + vol), _stream()))
     return out
 
 
@@ -186,8 +219,10 @@ def warp_backward(iref, dvf, grid, grad_out, grads=None):
     if grads is None:
         grads = (torch.empty_like(iref), torch.empty_like(dvf))
     gi, gd = grads
-    _check(lib().gsvox_warp_backward(_dev(iref, "iref"), _dev(dvf, "dvf"), C.byref(g), B, _dev(grad_out, "grad_out"),
-                                     _dev(gi, "grad_iref"), _dev(gd, "grad_dvf"), _stream()))
+    vol = (g.dims[2], g.dims[1], g.dims[0])
+    _check(lib().gsvox_warp_backward(_dev(iref, "iref", vol), _dev(dvf, "dvf", (B, 3) + vol), C.byref(g), B,
+                                     _dev(grad_out, "grad_out", (B,) + vol), _dev(gi, "grad_iref", vol),
+                                     _dev(gd, "grad_dvf", (B, 3) + vol), _stream()))
     return grads
 
 
@@ -218,8 +253,14 @@ def project_forward(vol, grid, geom, angles, out=None, scratch=None):
     if scratch is None:
         scratch = _project_scratch(g, B, vol.device)
     V = int(vol[0].numel()) if not shared else int(vol.numel())
-    _check(lib().gsvox_project_forward(_dev(vol, "vol"), 0 if shared else V, C.byref(g), C.byref(cg), ang, B,
-                                       _dev(scratch, "scratch"), _dev(out, "drr"), _stream()))
+    vshape = (g.dims[2], g.dims[1], g.dims[0])
+    nb = C.c_size_t(0)
+    _check(lib().gsvox_project_scratch_bytes(C.byref(g), B, C.byref(nb)))
+    if scratch.numel() * 4 < int(nb.value):
+        raise GsvoxError("project scratch holds %d bytes, %d needed" % (scratch.numel() * 4, int(nb.value)))
+    _check(lib().gsvox_project_forward(_dev(vol, "vol", vshape if shared else (B,) + vshape), 0 if shared else V,
+                                       C.byref(g), C.byref(cg), ang, B, _dev(scratch, "scratch"),
+                                       _dev(out, "drr", (B, cg.nv, cg.nu)), _stream()))
     return out
 
 
@@ -232,8 +273,13 @@ def project_backward(grad_drr, grid, geom, angles, out=None, scratch=None):
         out = torch.empty((B, g.dims[2], g.dims[1], g.dims[0]), dtype=torch.float32, device=grad_drr.device)
     if scratch is None:
         scratch = _project_scratch(g, B, grad_drr.device)
-    _check(lib().gsvox_project_backward(_dev(grad_drr, "grad_drr"), C.byref(g), C.byref(cg), ang, B,
-                                        _dev(scratch, "scratch"), _dev(out, "grad_vol"), _stream()))
+    nb = C.c_size_t(0)
+    _check(lib().gsvox_project_scratch_bytes(C.byref(g), B, C.byref(nb)))
+    if scratch.numel() * 4 < int(nb.value):
+        raise GsvoxError("project scratch holds %d bytes, %d needed" % (scratch.numel() * 4, int(nb.value)))
+    _check(lib().gsvox_project_backward(_dev(grad_drr, "grad_drr", (B, cg.nv, cg.nu)), C.byref(g), C.byref(cg), ang, B,
+                                        _dev(scratch, "scratch"),
+                                        _dev(out, "grad_vol", (B, g.dims[2], g.dims[1], g.dims[0])), _stream()))
     return out
 
 
@@ -250,8 +296,9 @@ class Splatter:
         nb = C.c_size_t(0)
         _check(lib().gsvox_splat_workspace_bytes(self.n_max, C.byref(self.cg), self.batch, self.key_capacity, C.byref(nb)))
         self.workspace_bytes = int(nb.value)
-        self._ws = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        self._ws = torch.zeros(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)   # zeroed: no stale stamp
         self._base = (self._ws.data_ptr() + 255) & ~255
+        self._n_fwd = None                                    # Gaussians of the latest forward
 
     def _angles(self, angles):
         if len(angles) != self.batch:
@@ -260,30 +307,43 @@ class Splatter:
 
     def forward(self, pos, scale, quat, rho, angles, out=None):
         n = int(pos.shape[0])
+        if n > self.n_max:
+            raise GsvoxError("%d Gaussians, the Splatter was sized for %d" % (n, self.n_max))
         if out is None:
             out = torch.empty((self.batch, self.cg.nv, self.cg.nu), dtype=torch.float32, device=self.device)
-        _check(lib().gsvox_splat_forward(_dev(pos, "pos"), _dev(scale, "scale"), _dev(quat, "quat"), _dev(rho, "rho"), n,
+        _check(lib().gsvox_splat_forward(_dev(pos, "pos", (n, 3)), _dev(scale, "scale", (n, 3)), _dev(quat, "quat", (n, 4)),
+                                         _dev(rho, "rho", (n, 1)), n,
                                          C.byref(self.cg), self._angles(angles), self.batch, C.c_void_p(self._base),
-                                         self.workspace_bytes, self.key_capacity, _dev(out, "drr"), _stream()))
+                                         self.workspace_bytes, self.key_capacity,
+                                         _dev(out, "drr", (self.batch, self.cg.nv, self.cg.nu)), _stream()))
+        self._n_fwd = n
         return out
 
     def backward(self, pos, scale, quat, rho, angles, grad_drr, grads=None):
         n = int(pos.shape[0])
+        if self._n_fwd is None or n != self._n_fwd:
+            raise GsvoxError("Splatter.backward must follow Splatter.forward with the same Gaussians "
+                             "(forward saw %s, backward %d)" % (self._n_fwd, n))
         if grads is None:
             mk = lambda *sh: torch.empty(sh, dtype=torch.float32, device=self.device)
             grads = (mk(n), mk(n, 3), mk(n, 3), mk(n, 4))
         gr, gp, gs, gq = grads
-        _check(lib().gsvox_splat_backward(_dev(pos, "pos"), _dev(scale, "scale"), _dev(quat, "quat"), _dev(rho, "rho"), n,
+        _check(lib().gsvox_splat_backward(_dev(pos, "pos", (n, 3)), _dev(scale, "scale", (n, 3)), _dev(quat, "quat", (n, 4)),
+                                          _dev(rho, "rho", (n, 1)), n,
                                           C.byref(self.cg), self._angles(angles), self.batch, C.c_void_p(self._base),
-                                          self.workspace_bytes, self.key_capacity, _dev(grad_drr, "grad_drr"),
-                                          _dev(gr, "grad_rho"), _dev(gp, "grad_pos"), _dev(gs, "grad_scale"),
-                                          _dev(gq, "grad_quat"), _stream()))
+                                          self.workspace_bytes, self.key_capacity,
+                                          _dev(grad_drr, "grad_drr", (self.batch, self.cg.nv, self.cg.nu)),
+                                          _dev(gr, "grad_rho", (n, 1)), _dev(gp, "grad_pos", (n, 3)),
+                                          _dev(gs, "grad_scale", (n, 3)), _dev(gq, "grad_quat", (n, 4)), _stream()))
         return grads
 
     def status(self):
         k, p, o, sk = C.c_int64(0), C.c_int64(0), C.c_int32(0), C.c_int32(0)
         _check(lib().gsvox_splat_status(C.c_void_p(self._base), C.byref(k), C.byref(p), C.byref(o), C.byref(sk), _stream()))
-        return {"keys_needed": int(k.value), "pairs": int(p.value), "overflow": bool(o.value), "skipped": int(sk.value)}
+        a, b, c = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        _check(lib().gsvox_splat_drops(C.c_void_p(self._base), C.byref(a), C.byref(b), C.byref(c), _stream()))
+        return {"keys_needed": int(k.value), "pairs": int(p.value), "overflow": bool(o.value), "skipped": int(sk.value),
+                "dropped_behind_source": int(a.value), "dropped_out_of_range": int(b.value), "dropped_empty_box": int(c.value)}
 
 
 class Plan:
@@ -329,16 +389,24 @@ class Plan:
     # --- the three hot-path calls -----------------------------------------------------
     def preprocess(self, pos, scale, quat):
         n = int(pos.shape[0])
-        _check(lib().gsvox_preprocess(self._h, _dev(pos, "pos"), _dev(scale, "scale"), _dev(quat, "quat"),
-                                      n, _stream()))
+        if n > self.n_max:
+            raise GsvoxError("%d Gaussians, the plan was sized for %d" % (n, self.n_max))
+        _check(lib().gsvox_preprocess(self._h, _dev(pos, "pos", (n, 3)), _dev(scale, "scale", (n, 3)),
+                                      _dev(quat, "quat", (n, 4)), n, _stream()))
         self.n = n
+
+    def _need_n(self):
+        if self.n is None:
+            raise GsvoxError("no preprocess on this plan yet")
+        return self.n
 
     def forward(self, weight, out=None):
         ch = int(weight.shape[1])
         nx, ny, nz = self.dims
         if out is None:
             out = torch.empty((ch, nz, ny, nx), dtype=torch.float32, device=self.device)
-        _check(lib().gsvox_forward(self._h, _dev(weight, "weight"), ch, _dev(out, "out"), _stream()))
+        _check(lib().gsvox_forward(self._h, _dev(weight, "weight", (self._need_n(), ch)), ch,
+                                   _dev(out, "out", (ch, nz, ny, nx)), _stream()))
         return out
 
     def backward(self, weight, grad_out, grads=None):
@@ -347,9 +415,11 @@ class Plan:
             mk = lambda k: torch.empty((n, k), dtype=torch.float32, device=self.device)
             grads = (mk(ch), mk(3), mk(3), mk(4))
         gw, gp, gs, gq = grads
-        _check(lib().gsvox_backward(self._h, _dev(weight, "weight"), ch, _dev(grad_out, "grad_out"),
-                                    _dev(gw, "grad_weight"), _dev(gp, "grad_pos"), _dev(gs, "grad_scale"),
-                                    _dev(gq, "grad_quat"), _stream()))
+        nx, ny, nz = self.dims
+        n = self._need_n()
+        _check(lib().gsvox_backward(self._h, _dev(weight, "weight", (n, ch)), ch, _dev(grad_out, "grad_out", (ch, nz, ny, nx)),
+                                    _dev(gw, "grad_weight", (n, ch)), _dev(gp, "grad_pos", (n, 3)),
+                                    _dev(gs, "grad_scale", (n, 3)), _dev(gq, "grad_quat", (n, 4)), _stream()))
         return grads
 
     # --- CUDA graph of one training step ----------------------------------------------
@@ -385,7 +455,9 @@ class Plan:
 
     def backward_accumulate(self, weight, grad_out):
         ch = int(weight.shape[1])
-        _check(lib().gsvox_backward_accumulate(self._h, _dev(weight, "weight"), ch, _dev(grad_out, "grad_out"), _stream()))
+        nx, ny, nz = self.dims
+        _check(lib().gsvox_backward_accumulate(self._h, _dev(weight, "weight", (self._need_n(), ch)), ch,
+                                               _dev(grad_out, "grad_out", (ch, nz, ny, nx)), _stream()))
 
     def accumulators(self, channels):
         """torch view (no copy) of the [n, round4(9 + C)] accumulators: the all-reduce payload."""
@@ -400,8 +472,10 @@ class Plan:
             mk = lambda k: torch.empty((n, k), dtype=torch.float32, device=self.device)
             grads = (mk(channels), mk(3), mk(3), mk(4))
         gw, gp, gs, gq = grads
-        _check(lib().gsvox_backward_finish(self._h, int(channels), _dev(gw, "grad_weight"), _dev(gp, "grad_pos"),
-                                           _dev(gs, "grad_scale"), _dev(gq, "grad_quat"), _stream()))
+        n = self._need_n()
+        _check(lib().gsvox_backward_finish(self._h, int(channels), _dev(gw, "grad_weight", (n, int(channels))),
+                                           _dev(gp, "grad_pos", (n, 3)), _dev(gs, "grad_scale", (n, 3)),
+                                           _dev(gq, "grad_quat", (n, 4)), _stream()))
         return grads
 
     # --- 8(f) rank 1: fused MBC -> DVF ------------------------------------------------
@@ -425,8 +499,11 @@ class Plan:
         if out is None:
             out = torch.empty((B, 3, nz, ny, nx), dtype=torch.float32, device=self.device)
         mixed, _ = self._dvf_scratch(n, 3 * B)
-        _check(lib().gsvox_dvf_forward(self._h, _dev(feat, "feat"), self._dev_i32(level, "level"), _dev(coef, "coef"),
-                                       B, L, _dev(mixed, "mixed"), _dev(out, "dvf"), _stream()))
+        if n != self._need_n() or int(level.numel()) != n:
+            raise GsvoxError("feat / level must have one row per preprocessed Gaussian (%d)" % self.n)
+        _check(lib().gsvox_dvf_forward(self._h, _dev(feat, "feat", (n, 3)), self._dev_i32(level, "level"),
+                                       _dev(coef, "coef", (B, L, 3)), B, L, _dev(mixed, "mixed"),
+                                       _dev(out, "dvf", (B, 3, nz, ny, nx)), _stream()))
         return out
 
     def dvf_backward(self, feat, level, coef, grad_dvf, grads=None):
@@ -436,10 +513,15 @@ class Plan:
             grads = (mk(n, 3), mk(B, L, 3), mk(n, 3), mk(n, 3), mk(n, 4))
         gf, gc, gp, gs, gq = grads
         mixed, gmixed = self._dvf_scratch(n, 3 * B)
-        _check(lib().gsvox_dvf_backward(self._h, _dev(feat, "feat"), self._dev_i32(level, "level"), _dev(coef, "coef"),
-                                        B, L, _dev(mixed, "mixed"), _dev(grad_dvf, "grad_dvf"), _dev(gmixed, "grad_mixed"),
-                                        _dev(gf, "grad_feat"), _dev(gc, "grad_coef"), _dev(gp, "grad_pos"),
-                                        _dev(gs, "grad_scale"), _dev(gq, "grad_quat"), _stream()))
+        nx, ny, nz = self.dims
+        if n != self._need_n() or int(level.numel()) != n:
+            raise GsvoxError("feat / level must have one row per preprocessed Gaussian (%d)" % self.n)
+        _check(lib().gsvox_dvf_backward(self._h, _dev(feat, "feat", (n, 3)), self._dev_i32(level, "level"),
+                                        _dev(coef, "coef", (B, L, 3)), B, L, _dev(mixed, "mixed"),
+                                        _dev(grad_dvf, "grad_dvf", (B, 3, nz, ny, nx)), _dev(gmixed, "grad_mixed"),
+                                        _dev(gf, "grad_feat", (n, 3)), _dev(gc, "grad_coef", (B, L, 3)),
+                                        _dev(gp, "grad_pos", (n, 3)), _dev(gs, "grad_scale", (n, 3)),
+                                        _dev(gq, "grad_quat", (n, 4)), _stream()))
         return grads
 
     # --- synchronising helpers --------------------------------------------------------
@@ -491,10 +573,12 @@ class Plan:
         gw = gp = gs = gq = None
         if grad_out is not None:
             gw, gp, gs, gq = grads
+        nx, ny, nz = self.dims
+        vol = (ch, nz, ny, nx)
         _check(lib().gsvox_step_host(self._h, C.c_void_p(base), self._staging_bytes,
-                                     _host(pos, "pos"), _host(scale, "scale"), _host(quat, "quat"),
-                                     _host(weight, "weight"), n, ch, _host(grad_out, "grad_out"), _host(out, "out"),
-                                     _host(gw, "grad_weight"), _host(gp, "grad_pos"), _host(gs, "grad_scale"),
-                                     _host(gq, "grad_quat"), _stream()))
+                                     _host(pos, "pos", (n, 3)), _host(scale, "scale", (n, 3)), _host(quat, "quat", (n, 4)),
+                                     _host(weight, "weight", (n, ch)), n, ch, _host(grad_out, "grad_out", vol),
+                                     _host(out, "out", vol), _host(gw, "grad_weight", (n, ch)), _host(gp, "grad_pos", (n, 3)),
+                                     _host(gs, "grad_scale", (n, 3)), _host(gq, "grad_quat", (n, 4)), _stream()))
         self.n = n
         return out, grads

@@ -144,13 +144,39 @@ extern "C" int gsvox_host_staging_bytes(int64_t n_max, int32_t max_channels, con
     return rc;
 }
 
+static int step_host_enqueue(gsvox_plan* p, void* staging, size_t staging_bytes,
+                             const float* pos_h, const float* scale_h, const float* quat_h,
+                             const float* weight_h, int64_t n, int32_t C,
+                             const float* grad_out_h, float* out_h,
+                             float* gw_h, float* gp_h, float* gs_h, float* gq_h, void* stream);
+
 extern "C" int gsvox_step_host(gsvox_plan* p, void* staging, size_t staging_bytes,
                                const float* pos_h, const float* scale_h, const float* quat_h,
                                const float* weight_h, int64_t n, int32_t C,
                                const float* grad_out_h, float* out_h,
                                float* gw_h, float* gp_h, float* gs_h, float* gq_h, void* stream)
 {
+    int rc = step_host_enqueue(p, staging, staging_bytes, pos_h, scale_h, quat_h, weight_h, n, C, grad_out_h, out_h,
+                               gw_h, gp_h, gs_h, gq_h, stream);
+    if (rc != GSVOX_OK && p && p->side_ready) {
+        // an error after the first enqueue: copies that reference the caller's host buffers may still be in flight
+        // on the two copy streams and on the caller's stream — drain them before control returns
+        cudaStreamSynchronize(p->side[0]); cudaStreamSynchronize(p->side[1]);
+        cudaStreamSynchronize((cudaStream_t)stream);
+        (void)cudaGetLastError();
+    }
+    return rc;
+}
+
+static int step_host_enqueue(gsvox_plan* p, void* staging, size_t staging_bytes,
+                             const float* pos_h, const float* scale_h, const float* quat_h,
+                             const float* weight_h, int64_t n, int32_t C,
+                             const float* grad_out_h, float* out_h,
+                             float* gw_h, float* gp_h, float* gs_h, float* gq_h, void* stream)
+{
     if (!p || !staging || n < 0 || n > p->n_max || C < 1 || C > p->max_channels) return GSVOX_EINVAL;
+    // a z-slab plan writes its own brick layers only: the whole-volume copy below would hand out the rest unwritten
+    if (p->gd.slab0 != 0 || p->gd.slab1 != p->gd.nb[2]) return GSVOX_EINVAL;
     if (n > 0 && (!pos_h || !scale_h || !quat_h || !weight_h)) return GSVOX_EINVAL;
     if (grad_out_h && n > 0 && (!gw_h || !gp_h || !gs_h || !gq_h)) return GSVOX_EINVAL;
     Staging S;

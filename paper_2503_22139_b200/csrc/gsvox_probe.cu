@@ -5,7 +5,11 @@
 //   FFMA2  packed fma.rn.f32x2 (sm_100 family)       (4 flops / lane-instruction)
 //   EX2    MUFU ex2.approx.ftz.f32                    (1 result / lane-instruction)
 // Grid = SM count x 8 CTAs of 256 threads; timed with CUDA events on the caller's stream.
+// Bench-only: built into libgsvox_probe.so (include/gsvox_probe.h), not into the product library.
 #include "gsvox_internal.cuh"
+#include "../../include/gsvox_probe.h"
+#undef GSVOX_CUDA
+#define GSVOX_CUDA(call) do { if ((call) != cudaSuccess) { (void)cudaGetLastError(); return GSVOX_ECUDA; } } while (0)
 
 namespace gsvox {
 
@@ -95,7 +99,7 @@ extern "C" int gsvox_probe_peaks(void* scratch, double* fp32_tflops, double* fp3
             else                k_probe_ex2<<<grid, kProbeThreads, 0, st>>>(sink, -0.001f);
             cudaEventRecord(e1, st);
             cudaError_t e = cudaEventSynchronize(e1);
-            if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return cuda_fail(e, "probe"); }
+            if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); (void)cudaGetLastError(); return GSVOX_ECUDA; }
             float ms = 0.f;
             cudaEventElapsedTime(&ms, e0, e1);
             const double per_s = lane_inst / (ms * 1e-3);

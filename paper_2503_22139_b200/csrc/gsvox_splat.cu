@@ -41,7 +41,23 @@ struct __align__(16) Splat2D {
 };
 static_assert(sizeof(Splat2D) == 48, "Splat2D must be 48 bytes");
 
-struct SplatStatus { unsigned long long keys_needed, pairs; unsigned int overflow, skipped; };
+// `stamp` is written by the LAST kernel of gsvox_splat_forward: magic + a digest of (n, B, nu, nv, key_capacity).  A
+// backward or status call on a workspace without it (no forward yet, or a forward with other sizes: every sub-buffer
+// would sit elsewhere) does nothing / reports GSVOX_ENOTREADY instead of reading garbage.
+struct SplatStatus {
+    unsigned long long keys_needed, pairs; unsigned int overflow, skipped;
+    unsigned long long stamp;
+    unsigned int drop_behind, drop_range, drop_empty, pad_;      // per (angle, Gaussian): t2 <= 0 | centre beyond +-30000 px | empty box
+};
+constexpr unsigned long long kSplatMagic = 0x67735370ull << 32;     // "gsSp"
+static unsigned long long splat_stamp(long long n, int B, int nu, int nv, long long key_capacity)
+{
+    unsigned long long h = 1469598103934665603ull;
+    const unsigned long long v[5] = { (unsigned long long)n, (unsigned long long)B, (unsigned long long)nu,
+                                      (unsigned long long)nv, (unsigned long long)key_capacity };
+    for (int i = 0; i < 5; ++i) { h ^= v[i]; h *= 1099511628211ull; }
+    return kSplatMagic | (h & 0xffffffffull);
+}
 
 struct SplatParams {
     int n, B, nu, nv, ntx, nty;
@@ -57,6 +73,7 @@ struct SplatWs {            // views into the caller's workspace
 // Everything Eq. 8-9 needs for one (angle, Gaussian), fp64.
 struct SplatTerms {
     bool valid;
+    int why;                 // when !valid: 1 degenerate parameters (any angle), 2 at or behind the source plane, 3 numerically singular
     double R[9], Sig[9], t[3], ell, T[9], St[9], det_t, det_h, amp_over_rho, P[3], dp, cu, cv;
 };
 
@@ -83,7 +100,7 @@ __device__ void splat_terms(const SplatParams& P, int b, const float* __restrict
     const double p[3] = { pos[3 * g], pos[3 * g + 1], pos[3 * g + 2] };
     const double s[3] = { scale[3 * g], scale[3 * g + 1], scale[3 * g + 2] };
     const double q[4] = { quat[4 * g], quat[4 * g + 1], quat[4 * g + 2], quat[4 * g + 3] };
-    o.valid = false;
+    o.valid = false; o.why = 1;
     bool bad = false;
     for (int k = 0; k < 3; ++k) bad |= !isfinite(p[k]) || !isfinite(s[k]) || !(s[k] > 0.0);
     for (int k = 0; k < 4; ++k) bad |= !isfinite(q[k]);
@@ -103,7 +120,9 @@ __device__ void splat_terms(const SplatParams& P, int b, const float* __restrict
     const double d[3] = { p[0] - src[0], p[1] - src[1], p[2] - src[2] };
     for (int i = 0; i < 3; ++i) o.t[i] = W[3 * i] * d[0] + W[3 * i + 1] * d[1] + W[3 * i + 2] * d[2];
     const double t0 = o.t[0], t1 = o.t[1], t2 = o.t[2];
+    o.why = 2;
     if (!(t2 > 0.0)) return;                                   // R5: at or behind the source plane
+    o.why = 3;
     o.ell = sqrt(t0 * t0 + t1 * t1 + t2 * t2);
     const double J[9] = { 1 / t2, 0, -t0 / (t2 * t2),  0, 1 / t2, -t1 / (t2 * t2),  t0 / o.ell, t1 / o.ell, t2 / o.ell };
     mat3mul(J, W, o.T);
@@ -134,7 +153,7 @@ k_splat_pre(SplatParams P, const float* __restrict__ pos, const float* __restric
     const bool live = idx < (long long)P.n * P.B;
     const int b = live ? (int)(idx / P.n) : 0, g = live ? (int)(idx - (long long)b * P.n) : 0;
     unsigned long long my_pairs = 0ull;
-    unsigned int my_skipped = 0u;
+    unsigned int my_skipped = 0u, my_drops = 0u;             // my_drops: behind | range << 10 | empty << 20 (per thread: 0/1 each)
     Splat2D r;
     r.cfu = r.cfv = r.A = r.B = r.C = r.amp = 0.f; r.ciu = r.civ = 0; r.u0 = r.v0 = 0; r.u1 = r.v1 = -1; r.Bq = r.Dq = 0.f; r.pad = 0;
     SplatTerms o;
@@ -155,25 +174,33 @@ k_splat_pre(SplatParams P, const float* __restrict__ pos, const float* __restric
             r.ciu = (int16_t)ci; r.civ = (int16_t)cj; r.cfu = (float)(o.cu - ci); r.cfv = (float)(o.cv - cj);
             r.u0 = (int16_t)u0; r.v0 = (int16_t)v0; r.u1 = (int16_t)u1; r.v1 = (int16_t)v1;
             my_pairs = (unsigned long long)((u1 - u0 + 1.0) * (v1 - v0 + 1.0));
-        }
-    } else if (live && b == 0) {
-        my_skipped = 1u;
+        } else if (!(fabs(o.cu) <= 30000.0 && fabs(o.cv) <= 30000.0)) my_drops = 1u << 10;
+        else my_drops = 1u << 20;
+    } else if (live) {
+        // degenerate Gaussians (and non-finite rho) are counted once, per-angle drops per (angle, Gaussian)
+        if (o.why == 2 && isfinite(rh)) my_drops = 1u;
+        else if (b == 0) my_skipped = 1u;
     }
     if (live) rec[idx] = r;
     // counters: warp -> CTA -> one atomic per CTA (per-item atomics on one address cost 0.15 ms)
     __shared__ unsigned long long s_pairs[4];
-    __shared__ unsigned int s_skip[4];
+    __shared__ unsigned int s_skip[4], s_drop[4];
     for (int o2 = 16; o2 > 0; o2 >>= 1) {
         my_pairs += __shfl_xor_sync(0xffffffffu, my_pairs, o2);
         my_skipped += __shfl_xor_sync(0xffffffffu, my_skipped, o2);
+        my_drops += __shfl_xor_sync(0xffffffffu, my_drops, o2);          // three 10-bit fields, <= 32 each per warp
     }
-    if ((threadIdx.x & 31) == 0) { s_pairs[threadIdx.x >> 5] = my_pairs; s_skip[threadIdx.x >> 5] = my_skipped; }
+    if ((threadIdx.x & 31) == 0) { s_pairs[threadIdx.x >> 5] = my_pairs; s_skip[threadIdx.x >> 5] = my_skipped; s_drop[threadIdx.x >> 5] = my_drops; }
     __syncthreads();
     if (threadIdx.x == 0) {
         const unsigned long long tp = s_pairs[0] + s_pairs[1] + s_pairs[2] + s_pairs[3];
         const unsigned int ts = s_skip[0] + s_skip[1] + s_skip[2] + s_skip[3];
+        const unsigned int td = s_drop[0] + s_drop[1] + s_drop[2] + s_drop[3];
         if (tp) atomicAdd(&status->pairs, tp);
         if (ts) atomicAdd(&status->skipped, ts);
+        if (td & 1023u) atomicAdd(&status->drop_behind, td & 1023u);
+        if ((td >> 10) & 1023u) atomicAdd(&status->drop_range, (td >> 10) & 1023u);
+        if (td >> 20) atomicAdd(&status->drop_empty, td >> 20);
     }
 }
 
@@ -271,8 +298,10 @@ constexpr int kSplatFwdWarps = SPLAT_FWD_WARPS;   // warps of a CTA take the til
 
 __global__ void __launch_bounds__(32 * kSplatFwdWarps)
 k_splat_forward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* __restrict__ bin_start,
-                const uint32_t* __restrict__ keys, const SplatStatus* __restrict__ status, float* __restrict__ drr)
+                const uint32_t* __restrict__ keys, SplatStatus* __restrict__ status, unsigned long long stamp,
+                float* __restrict__ drr)
 {
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) status->stamp = stamp;     // the forward got this far
     __shared__ SplatTileRec s_recs[kSplatFwdWarps][kSplatFwdBatch];
     __shared__ float s_part[kSplatFwdWarps > 1 ? kSplatFwdWarps - 1 : 1][8][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tile = blockIdx.x, b = blockIdx.y;
@@ -383,14 +412,14 @@ constexpr int kSplatBwdChunk = 1024;
 
 __global__ void __launch_bounds__(kSplatBwdThreads)
 k_splat_backward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t* __restrict__ bin_start,
-                 const uint32_t* __restrict__ keys, const SplatStatus* __restrict__ status,
+                 const uint32_t* __restrict__ keys, const SplatStatus* __restrict__ status, unsigned long long stamp,
                  const float* __restrict__ gdrr, float* __restrict__ acc)
 {
     __shared__ float s_g[kSplatTile * kSplatTile];
     __shared__ uint32_t s_key[kSplatBwdChunk], s_sorted[kSplatBwdChunk];
     __shared__ uint8_t s_cls[kSplatBwdChunk];
     __shared__ uint32_t s_hist[64];
-    if (status->overflow) return;
+    if (status->overflow || status->stamp != stamp) return;
     const int tid = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
     const uint32_t kbeg = bin_start[b * P.ntx * P.nty + tile], kend = bin_start[b * P.ntx * P.nty + tile + 1];
     if (kbeg == kend) return;
@@ -464,7 +493,7 @@ k_splat_backward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t*
 __global__ void __launch_bounds__(128, 4)
 k_splat_epilogue(SplatParams P, const float* __restrict__ pos, const float* __restrict__ scale, const float* __restrict__ quat,
                  const float* __restrict__ rho, const Splat2D* __restrict__ rec, const float* __restrict__ acc,
-                 const SplatStatus* __restrict__ status,
+                 const SplatStatus* __restrict__ status, unsigned long long stamp,
                  float* __restrict__ grho, float* __restrict__ gpos, float* __restrict__ gscale, float* __restrict__ gquat)
 {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
@@ -473,7 +502,8 @@ k_splat_epilogue(SplatParams P, const float* __restrict__ pos, const float* __re
     const double rh = (double)rho[g];
     SplatTerms o;
     o.valid = false;
-    for (int b = 0; b < P.B && !status->overflow; ++b) {
+    const bool ready = !status->overflow && status->stamp == stamp;      // else: zero gradients
+    for (int b = 0; b < P.B && ready; ++b) {
         const size_t idx = (size_t)b * P.n + g;
         if (rec[idx].u1 < rec[idx].u0) continue;               // skipped or off the detector at this angle
         splat_terms(P, b, pos, scale, quat, g, o);
@@ -637,7 +667,8 @@ extern "C" int gsvox_splat_forward(const float* pos, const float* scale, const f
         GSVOX_CUDA(cudaGetLastError());
     }
     dim3 grid((unsigned)(P.ntx * P.nty), (unsigned)B);
-    k_splat_forward<<<grid, 32 * kSplatFwdWarps, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, drr);
+    k_splat_forward<<<grid, 32 * kSplatFwdWarps, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status,
+                                                          splat_stamp(n, B, P.nu, P.nv, key_capacity), drr);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }
@@ -657,9 +688,10 @@ extern "C" int gsvox_splat_backward(const float* pos, const float* scale, const 
     cudaStream_t st = (cudaStream_t)stream;
     GSVOX_CUDA(cudaMemsetAsync(ws.acc, 0, sizeof(float) * 8 * (size_t)n * B, st));
     dim3 grid((unsigned)(P.ntx * P.nty), (unsigned)B);
-    k_splat_backward<<<grid, kSplatBwdThreads, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, grad_drr, ws.acc);
+    const unsigned long long stamp = splat_stamp(n, B, P.nu, P.nv, key_capacity);
+    k_splat_backward<<<grid, kSplatBwdThreads, 0, st>>>(P, ws.rec, ws.bin_start, ws.keys, ws.status, stamp, grad_drr, ws.acc);
     GSVOX_CUDA(cudaGetLastError());
-    k_splat_epilogue<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(P, pos, scale, quat, rho, ws.rec, ws.acc, ws.status,
+    k_splat_epilogue<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(P, pos, scale, quat, rho, ws.rec, ws.acc, ws.status, stamp,
                                                                  grad_rho, grad_pos, grad_scale, grad_quat);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
@@ -673,9 +705,25 @@ extern "C" int gsvox_splat_status(const void* workspace, int64_t* keys_needed, i
     cudaStream_t st = (cudaStream_t)stream;
     GSVOX_CUDA(cudaMemcpyAsync(&h, workspace, sizeof h, cudaMemcpyDeviceToHost, st));
     GSVOX_CUDA(cudaStreamSynchronize(st));
+    if ((h.stamp >> 32) != (kSplatMagic >> 32)) return GSVOX_ENOTREADY;      // no gsvox_splat_forward completed on this workspace
     if (keys_needed) *keys_needed = (int64_t)h.keys_needed;
     if (pairs) *pairs = (int64_t)h.pairs;
     if (overflow) *overflow = (int32_t)h.overflow;
     if (skipped) *skipped = (int32_t)h.skipped;
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_splat_drops(const void* workspace, int64_t* behind_source, int64_t* out_of_range, int64_t* empty_box,
+                                 void* stream)
+{
+    if (!workspace) return GSVOX_EINVAL;
+    SplatStatus h;
+    cudaStream_t st = (cudaStream_t)stream;
+    GSVOX_CUDA(cudaMemcpyAsync(&h, workspace, sizeof h, cudaMemcpyDeviceToHost, st));
+    GSVOX_CUDA(cudaStreamSynchronize(st));
+    if ((h.stamp >> 32) != (kSplatMagic >> 32)) return GSVOX_ENOTREADY;
+    if (behind_source) *behind_source = (int64_t)h.drop_behind;
+    if (out_of_range) *out_of_range = (int64_t)h.drop_range;
+    if (empty_box) *empty_box = (int64_t)h.drop_empty;
     return GSVOX_OK;
 }

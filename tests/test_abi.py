@@ -18,8 +18,8 @@ def pkg():
     return p
 
 
-def declared_functions():
-    text = open(os.path.join(ROOT, "include", "gsvox.h")).read()
+def declared_functions(header="gsvox.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(gsvox_[a-z_0-9]+)\s*\(", text)))
 
@@ -37,6 +37,17 @@ def test_library_exports_every_declared_symbol(pkg):
     assert pkg.lib().gsvox_version() >= 100
 
 
+def test_probe_library_is_separate_from_the_product_library(pkg):
+    """include/gsvox_probe.h (bench-only microbenchmarks) lives in libgsvox_probe.so, not in libgsvox.so."""
+    names = declared_functions("gsvox_probe.h")
+    assert names == sorted(pkg.PROBE_EXPORTS) == ["gsvox_probe_peaks"]
+    P = pkg.probe_lib()
+    for name in names:
+        assert getattr(P, name) is not None
+    with pytest.raises(AttributeError):
+        getattr(C.CDLL(pkg.LIB_PATH), "gsvox_probe_peaks")
+
+
 def test_library_is_sm100a_only_and_uses_no_tensor_cores(pkg):
     """The path is not a dense contraction (north_star): the cubin must target sm_100a."""
     import subprocess
@@ -49,8 +60,9 @@ def test_workspace_bytes_and_argument_checks(pkg):
     n = C.c_size_t(0)
     g = pkg.make_grid((0, 0, 0), (1, 1, 1), (256, 256, 256))
     assert L.gsvox_workspace_bytes(500000, 1, C.byref(g), 16_000_000, C.byref(n)) == 0
-    # records 64 B + aux 32 B + accumulators 48 B per Gaussian, 4 B per key, 8 B per (brick, class) bin
-    expect = 500000 * (64 + 32 + 48) + 16_000_000 * 4 + 32768 * 17 * 8
+    # records 64 B + aux 32 B + accumulators 48 B per Gaussian, 4 B per key, 8 B per (brick, class) bin,
+    # 8 B per hot-brick segment (one per 512 keys of capacity)
+    expect = 500000 * (64 + 32 + 48) + 16_000_000 * 4 + 32768 * 17 * 8 + (16_000_000 // 512 + 1) * 8
     assert expect <= n.value <= expect + 8192
     bad = pkg.make_grid((0, 0, 0), (1, 0, 1), (8, 8, 8))
     assert L.gsvox_workspace_bytes(10, 1, C.byref(bad), 10, C.byref(n)) == -1
