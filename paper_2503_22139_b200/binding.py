@@ -349,7 +349,8 @@ class Splatter:
 class Plan:
     """gsvox_plan + the torch-owned workspace it lives in."""
 
-    def __init__(self, n_max, grid, max_channels=1, key_capacity=None, device="cuda"):
+    def __init__(self, n_max, grid, max_channels=1, key_capacity=None, device="cuda", workspace=None):
+        """workspace: optional caller-owned uint8 CUDA tensor (>= workspace_bytes + 255) to place the plan in."""
         origin, spacing, dims = grid
         self.grid = make_grid(origin, spacing, dims)
         self.dims = tuple(int(d) for d in dims)
@@ -367,8 +368,15 @@ class Plan:
         _check(lib().gsvox_workspace_bytes(self.n_max, self.max_channels, C.byref(self.grid),
                                            self.key_capacity, C.byref(nbytes)))
         self.workspace_bytes = int(nbytes.value)
-        self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        if workspace is None:
+            workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        if not (workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.is_contiguous()):
+            raise GsvoxError("workspace must be a contiguous uint8 CUDA tensor")
+        self.workspace = workspace
         base = (self.workspace.data_ptr() + 255) & ~255
+        if base + self.workspace_bytes > self.workspace.data_ptr() + self.workspace.numel():
+            raise GsvoxError("workspace holds %d bytes, %d (+ alignment) needed" % (self.workspace.numel(), self.workspace_bytes))
+        self.workspace_offset = base - self.workspace.data_ptr()
         self._h = C.c_void_p(None)
         _check(lib().gsvox_plan_create(self.n_max, self.max_channels, C.byref(self.grid), self.key_capacity,
                                        C.c_void_p(base), self.workspace_bytes, C.byref(self._h)))
@@ -549,6 +557,13 @@ class Plan:
         _check(lib().gsvox_plan_bins_host(self._h, C.c_void_p(start.data_ptr()), C.c_void_p(keys.data_ptr()),
                                           total, _stream()))
         return start.numpy(), keys.numpy()[:total]
+
+    def layer_keys(self):
+        """Keys per brick layer along z of the latest binning (SYNCHRONISES): what dist.slab_bounds_by_keys cuts on."""
+        start, _ = self.bins()
+        nb = [(d + 7) // 8 for d in self.dims]
+        per_brick = start[1:] - start[:-1]
+        return per_brick.reshape(nb[2], nb[1] * nb[0]).sum(axis=1).tolist()
 
     def set_timing(self, on):
         _check(lib().gsvox_plan_set_timing(self._h, 1 if on else 0))

@@ -69,6 +69,34 @@ def slab_bounds(nbz, rank, world):
     return lo, lo + base + (1 if rank < extra else 0)
 
 
+def slab_bounds_by_keys(layer_keys, rank, world):
+    """Contiguous split of the brick layers balanced by KEY COUNT, not by layer count: layer_keys[l] = keys whose
+    brick lies in layer l (Plan.layer_keys() of an unsharded binning, or any work estimate).  Clustered inputs
+    (config 5's blobs) make layers very unequal: equal-layer slabs leave most ranks idle.  Rank r owns [lo, hi);
+    cut c sits at the layer boundary whose running sum is nearest to c/world of the total (ties to the left, cuts
+    never move backwards), so every layer is owned exactly once, slabs stay contiguous, and equal weights reproduce slab_bounds up to rounding.
+    All ranks must pass the same layer_keys."""
+    nbz = len(layer_keys)
+    if not (0 <= rank < world):
+        raise ValueError("slab_bounds_by_keys(rank=%r, world=%r)" % (rank, world))
+    total = float(sum(layer_keys))
+    if nbz == 0 or total <= 0:
+        return slab_bounds(nbz, rank, world)
+    prefix = [0.0]
+    for v in layer_keys:
+        prefix.append(prefix[-1] + float(v))
+    cuts = [0]
+    for c in range(1, world):                      # the boundary whose prefix sum is nearest to c/world of the total
+        target = total * c / world
+        best = cuts[-1]
+        for i in range(cuts[-1], nbz + 1):
+            if abs(prefix[i] - target) < abs(prefix[best] - target):
+                best = i
+        cuts.append(best)
+    cuts.append(nbz)
+    return cuts[rank], cuts[rank + 1]
+
+
 def sharded_backward(plan, weight, grad_out, ranks, grads=None, all_reduce=None):
     """a4 on this rank's slab -> sum of the [n, 9 + C] accumulators over ranks -> a5.  `all_reduce`
     defaults to torch.distributed.all_reduce (NCCL over NVLink/NVSwitch: 24 MB at config 4)."""

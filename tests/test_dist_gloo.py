@@ -154,3 +154,32 @@ def test_two_rank_gloo_projection_batch_sharding_and_gradient_sum():
     assert outs[0]["b"] == [0, 4] and outs[1]["b"] == [4, 8]
     for o in outs:
         assert o["g0"] == 8.0 and o["g1"] == 3.0             # sums over both ranks
+
+
+def test_slab_bounds_by_keys_partition_and_balance():
+    """Key-balanced cuts: every layer owned exactly once, contiguous; no slab holds more than total/world plus one
+    layer's keys; equal weights give the equal-layer split; a clustered profile moves the cuts into the cluster."""
+    sys.path.insert(0, ROOT)
+    import numpy as np
+    from paper_2503_22139_b200.dist import slab_bounds, slab_bounds_by_keys
+    rng = np.random.default_rng(5)
+    profiles = [[1] * 32, [0] * 8, [5], list(rng.integers(0, 1000, 32)), [0, 0, 0, 900, 50, 50, 0, 0],
+                list((1000 * np.exp(-0.5 * ((np.arange(32) - 12) / 3.0) ** 2)).astype(int))]
+    for w in profiles:
+        for world in (1, 2, 3, 4, 8):
+            cover, loads = [], []
+            for r in range(world):
+                lo, hi = slab_bounds_by_keys(w, r, world)
+                assert 0 <= lo <= hi <= len(w)
+                cover += list(range(lo, hi)); loads.append(sum(w[lo:hi]))
+            assert cover == list(range(len(w)))
+            if sum(w) > 0:
+                assert max(loads) <= sum(w) / world + max(w) + 1e-9
+    for world in (1, 2, 4, 8):
+        for r in range(world):
+            assert slab_bounds_by_keys([7] * 32, r, world) == slab_bounds(32, r, world)
+    # the Gaussian-shaped profile: equal layers would give rank 0 of 4 the layers 0..7 (few keys); key balance does not
+    w = profiles[-1]
+    eq = [sum(w[slab_bounds(32, r, 4)[0]:slab_bounds(32, r, 4)[1]]) for r in range(4)]
+    kb = [sum(w[slab_bounds_by_keys(w, r, 4)[0]:slab_bounds_by_keys(w, r, 4)[1]]) for r in range(4)]
+    assert max(kb) < 0.6 * max(eq)

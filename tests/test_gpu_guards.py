@@ -107,3 +107,92 @@ def test_splat_outputs_stay_inside_their_buffers(pkg):
     sp.backward(*a, list(sc.angles), dev(sc.grad_drr()), grads=(gr, gp, gs, gq))
     assert not sp.status()["overflow"]
     ar.check()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# compute-sanitizer is closed on this pool (profiles/sanitizer_r2.md holds the refusal); what follows stands in
+# for its three tools on the voxelizer: memcheck -> guard zones around the WORKSPACE with every sub-buffer sized
+# exactly; initcheck -> the same step on poisoned memory (NaN bytes, then zeros) must give the same results;
+# racecheck -> repeated launches on one plan must agree bit for bit where the kernel has no atomics.
+# ---------------------------------------------------------------------------------------------------------
+def _guarded_plan(pkg, case, key_capacity, poison=0xFF):
+    probe = pkg.Plan(max(case.n, 1), case.grid, max_channels=case.channels, key_capacity=key_capacity)
+    need = probe.workspace_bytes
+    guard = 1 << 16
+    arena = torch.full((need + 2 * guard + 512,), 0xA5, dtype=torch.uint8, device="cuda")
+    off = guard + ((-(arena.data_ptr() + guard)) % 256)
+    ws = arena[off:off + need]
+    ws.fill_(poison)
+    plan = pkg.Plan(max(case.n, 1), case.grid, max_channels=case.channels, key_capacity=key_capacity, workspace=ws)
+    assert plan.workspace_offset == 0
+
+    def check():
+        torch.cuda.synchronize()
+        assert bool((arena[:off] == 0xA5).all()) and bool((arena[off + need:] == 0xA5).all()), "workspace guard overwritten"
+    return plan, check
+
+
+@pytest.mark.parametrize("which", ["config1", "hot", "needles", "channels9"])
+def test_workspace_guards_with_exactly_sized_key_buffer(pkg, which):
+    """key_capacity = the exact key count: the key list, the split list and every other sub-buffer of the workspace
+    are full to the last element, and nothing may spill into the guard zones around the workspace."""
+    if which == "config1":
+        case = gsvox_inputs.config1()
+    elif which == "hot":
+        case = gsvox_inputs.config1(n=6000, dims=(16, 15, 13), seed=88)
+    elif which == "needles":
+        case = gsvox_inputs.config5(n=6000, dims=(64, 48, 40))
+    else:
+        case = gsvox_inputs.config3(3, n=900, dims=(40, 36, 28))
+    t = (dev(case.pos), dev(case.scale), dev(case.quat), dev(case.weight))
+    g = dev(case.grad_out())
+    first = pkg.Plan(case.n, case.grid, max_channels=case.channels)
+    first.preprocess(*t[:3])
+    need = first.status()["keys_needed"]
+    results = []
+    for poison in (0xFF, 0x00):
+        plan, check = _guarded_plan(pkg, case, need, poison)
+        nx, ny, nz = case.dims
+        out = torch.full((case.channels, nz, ny, nx), float("nan"), device="cuda")
+        grads = tuple(torch.full((case.n, k), float("nan"), device="cuda") for k in (case.channels, 3, 3, 4))
+        for _ in range(2):                                      # a second step on the used workspace as well
+            plan.preprocess(*t[:3])
+            plan.forward(t[3], out=out)
+            plan.backward(t[3], g, grads=grads)
+        st = plan.status()
+        assert not st["overflow"] and st["keys_needed"] == need
+        check()
+        assert torch.isfinite(out).all() and all(torch.isfinite(x).all() for x in grads)
+        results.append((out.cpu().numpy(), [x.cpu().numpy() for x in grads]))
+    (o1, g1), (o2, g2) = results
+    # poison must not reach the results: same values up to the summation order of the atomics
+    assert np.abs(o1 - o2).max() <= 1e-6 * np.abs(o1).max()
+    for a, b in zip(g1, g2):
+        assert np.linalg.norm(a - b) <= 1e-5 * np.linalg.norm(a)
+    # one key short: the overflow path must engage and still write nothing outside
+    plan, check = _guarded_plan(pkg, case, need - 1)
+    plan.preprocess(*t[:3])
+    out = plan.forward(t[3])
+    assert plan.status()["overflow"] and not out.any()
+    check()
+
+
+@pytest.mark.parametrize("channels", [1, 3, 9])
+def test_repeated_forward_on_one_plan_is_bitwise_identical(pkg, channels):
+    """The forward kernels stage keys through shared memory (C > 1: double-buffered batches behind one __syncthreads;
+    C = 1: cp.async + per-warp lists behind __syncwarp) and use no atomics below 512 keys per brick: with the bins
+    fixed, 25 launches under whatever timing must produce the same bits.  A shared-memory race would not."""
+    case = gsvox_inputs.config3(3, n=4000, dims=(64, 56, 48), channels=channels) if channels > 1 else \
+        gsvox_inputs.config4(n=12000, dims=(96, 88, 72))
+    t = (dev(case.pos), dev(case.scale), dev(case.quat), dev(case.weight))
+    plan = pkg.Plan(case.n, case.grid, max_channels=channels)
+    plan.preprocess(*t[:3])
+    start, _ = plan.bins()
+    assert np.diff(start).max() <= 512                          # no hot-brick segments: no atomics in the forward
+    ref = plan.forward(t[3]).clone()
+    busy = torch.empty(1 << 24, device="cuda")
+    for i in range(25):
+        if i % 3 == 0:
+            busy.normal_()                                      # perturb the timing
+        out = plan.forward(t[3])
+        assert torch.equal(out, ref), "forward differs between launches on the same plan (launch %d)" % i

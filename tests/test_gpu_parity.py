@@ -165,6 +165,23 @@ def test_config5_recipe_reduced_needles_and_blobs(pkg):
     full_parity(pkg, gsvox_inputs.config5(n=20000, dims=(128, 96, 64)))
 
 
+def test_hot_bricks_are_split_into_key_range_segments(pkg):
+    """6000 Gaussians on 8 bricks: ~3000 keys per brick, so a3 (C = 1) works segments 1.. of every brick in its
+    second launch (atomic adds onto what segment 0 stored) and a4 spills past its 2048-key first launch
+    (kSplitKeys = 512, gsvox_internal.cuh; SURVEY section 7 hard part 6).  Ragged grid: rows outside the grid too."""
+    case = gsvox_inputs.config1(n=6000, dims=(16, 15, 13), seed=88)
+    plan = full_parity(pkg, case)
+    start, _ = plan.bins()
+    assert np.diff(start).max() > 2048
+
+
+def test_hot_bricks_multi_channel(pkg):
+    case = gsvox_inputs.subvolume_case(n=12000, dims=(16, 16, 8), channels=3, seed=89)
+    plan = full_parity(pkg, case)
+    start, _ = plan.bins()
+    assert np.diff(start).max() > 2048
+
+
 def test_narrow_and_wide_gaussians(pkg):
     """Scales from 0.15 voxel (sub-voxel, direct-exponential path, mostly empty boxes) to 40 voxels."""
     rng = np.random.default_rng(77)
