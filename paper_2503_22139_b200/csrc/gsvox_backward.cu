@@ -64,6 +64,13 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
 {
     float dy = (float)kg.y0 - kg.cy, dz = (float)kg.z0 - kg.cz;
     const float dy0 = dy;
+    float km[8];                                                    // [k in box] c^((k-3)(k-4)/2), c = 2^-2A
+    {
+        const float c1 = kg.cc, c3 = c1 * c1 * c1, c6 = c3 * c3;
+        const float kk[8] = { c6, c3, c1, 1.f, 1.f, c1, c3, c6 };
+        #pragma unroll
+        for (int k = 0; k < 8; ++k) km[k] = (!DIRECT && (kg.xm & (1u << k))) ? kk[k] : 0.f;
+    }
     uint32_t gaddr = sbase + ((((kg.z0 << 3) + kg.y0) << 3) << 2);     // byte address of the row in the tile
     const uint32_t wrapstep = (uint32_t)(9 - kg.ny) << 5;              // last y of a slice -> y0 of the next
     int yc = kg.ny;
@@ -73,19 +80,24 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
         const float Es = fmaf(kg.nD2 * dz, dz, (kg.nD1 * u1) * u1);
         float G[8];
         if (!DIRECT) {
+            // the row is the parabola E(k) = E3 + (k - 3) Lf - A (k - 3)(k - 4):  G(k) = G3 rho^(k-3) c^((k-3)(k-4)/2).
+            // The geometric part is chained here (7 FMUL); the key-and-k part, together with the x mask of the box,
+            // sits in km[k] (per key, hoisted out of the row loop) — as in a3, where it sits in the staged weights.
             const float t3 = 3.0f - xs;
             const float nAt = kg.negA * t3;
+            const float Lf = fminf(fmaxf(fmaf(nAt, 2.0f, kg.negA), -120.f), 120.f);      // 2^+-Lf stay finite; beyond, G3 is 0
             G[3] = ex2b(fmaf(nAt, t3, Es));
-            float rf = ex2b(fminf(fmaf(nAt, 2.0f, kg.negA), 120.f));
-            float rb = ex2b(fminf(fmaf(nAt, -2.0f, kg.negA), 120.f));
-            G[4] = G[3] * rf; rf *= kg.cc; G[5] = G[4] * rf; rf *= kg.cc; G[6] = G[5] * rf; rf *= kg.cc; G[7] = G[6] * rf;
-            G[2] = G[3] * rb; rb *= kg.cc; G[1] = G[2] * rb; rb *= kg.cc; G[0] = G[1] * rb;
+            const float rf = ex2b(Lf), rb = ex2b(-Lf);
+            G[4] = G[3] * rf; G[5] = G[4] * rf; G[6] = G[5] * rf; G[7] = G[6] * rf;
+            G[2] = G[3] * rb; G[1] = G[2] * rb; G[0] = G[1] * rb;
+            #pragma unroll
+            for (int k = 0; k < 8; ++k) G[k] *= km[k];
         } else {
             #pragma unroll
             for (int k = 0; k < 8; ++k) { const float t = (float)k - xs; G[k] = ex2b(fmaf(kg.negA * t, t, Es)); }
+            #pragma unroll
+            for (int k = 0; k < 8; ++k) G[k] = (kg.xm & (1u << k)) ? G[k] : 0.f;      // voxels outside the box in x
         }
-        #pragma unroll
-        for (int k = 0; k < 8; ++k) G[k] = (kg.xm & (1u << k)) ? G[k] : 0.f;      // voxels outside the box in x
         // a_k = (sum_c g_c w_c) G_k  (w factored out when SINGLE)
         float av[8];
         if (SINGLE) {
