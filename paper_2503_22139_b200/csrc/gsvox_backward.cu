@@ -107,9 +107,10 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
         } else {
             #pragma unroll
             for (int k = 0; k < 8; ++k) av[k] = 0.f;
+            const uint32_t ga0 = gaddr ^ ((gaddr >> 3) & 16u), ga1 = ga0 ^ 16u;   // rows with y >= 4 hold their halves swapped (stage loop)
             #pragma unroll
             for (int ch = 0; ch < CH; ++ch) {
-                const float4 g0 = lds_v4(gaddr + ch * kBrickVox * 4), g1 = lds_v4(gaddr + ch * kBrickVox * 4 + 16);
+                const float4 g0 = lds_v4(ga0 + ch * kBrickVox * 4), g1 = lds_v4(ga1 + ch * kBrickVox * 4);
                 const float gv[8] = { g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w };
                 float d = 0.f;
                 #pragma unroll
@@ -169,7 +170,11 @@ __device__ __forceinline__ void backward_brick(const GsRec* __restrict__ rec, co
             float val = 0.f;
             if (gx < gd.dims[0] && gy < gd.dims[1] && gz < gd.dims[2])
                 val = __ldg(grad_out + (size_t)(c0 + ch) * plane + ((size_t)gz * gd.dims[1] + gy) * gd.dims[0] + gx);
-            s_g[e] = val;
+            // 16-byte chunk c = 2 row + half goes to chunk c ^ (bit 2 of y): the eight rows y = 0..7 of a slice then start in
+            // eight different bank groups, not four (thread-per-key LDS.128 of different rows: ncu counted 48 % of the
+            // shared-memory wavefronts of k_backward<9> as bank conflicts, on a kernel whose l1tex pipe was 95 % busy)
+            // (C = 1 keeps the plain layout: it is issue-bound, and the two extra address instructions per row cost it 4 %)
+            s_g[CH > 1 ? ((e & ~7) | ((x & 4) ^ (y & 4)) | (x & 3)) : e] = val;
         }
     }
     __syncthreads();
@@ -242,7 +247,7 @@ k_backward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start
            const float* __restrict__ weight, int wstride, int c0,
            const float* __restrict__ grad_out, float* __restrict__ acc, int astride, GridDev gd)
 {
-    __shared__ __align__(16) float s_g[CH * kBrickVox];
+    __shared__ __align__(256) float s_g[CH * kBrickVox];
     if (status->overflow) return;
     const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];      // z-slab of this plan
     const uint32_t kbeg = bin_start[b * kNumClasses];
@@ -260,7 +265,7 @@ k_backward_extra(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin
                  const float* __restrict__ weight, int wstride, int c0,
                  const float* __restrict__ grad_out, float* __restrict__ acc, int astride, GridDev gd)
 {
-    __shared__ __align__(16) float s_g[CH * kBrickVox];
+    __shared__ __align__(256) float s_g[CH * kBrickVox];
     if (status->overflow) return;
     const uint32_t nitems = min(status->nsplit, (uint32_t)split_cap);
     for (uint32_t i = blockIdx.x; i < nitems; i += gridDim.x) {
