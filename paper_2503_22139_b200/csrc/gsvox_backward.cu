@@ -107,7 +107,8 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
         } else {
             #pragma unroll
             for (int k = 0; k < 8; ++k) av[k] = 0.f;
-            const uint32_t ga0 = gaddr ^ ((gaddr >> 3) & 16u), ga1 = ga0 ^ 16u;   // rows with y >= 4 hold their halves swapped (stage loop)
+            // rows with y >= 4 hold their halves swapped when CH > 1 (stage loop); a lone channel of a wider C keeps the plain layout
+            const uint32_t ga0 = (CH > 1) ? (gaddr ^ ((gaddr >> 3) & 16u)) : gaddr, ga1 = ga0 ^ 16u;
             #pragma unroll
             for (int ch = 0; ch < CH; ++ch) {
                 const float4 g0 = lds_v4(ga0 + ch * kBrickVox * 4), g1 = lds_v4(ga1 + ch * kBrickVox * 4);
