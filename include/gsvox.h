@@ -109,6 +109,18 @@ typedef struct {
 } gsvox_status;
 int gsvox_plan_status(gsvox_plan* plan, gsvox_status* status, void* stream);
 
+/* Deterministic forward (SURVEY.md section 7 hard part 3).  By default the keys of a (brick, class) bin stand in
+ * the order the binning's atomics produced, so two preprocess calls on the same inputs may sum a voxel's terms in
+ * different orders (results agree to ~1e-7 relative, not bit for bit).  With `enabled` != 0, gsvox_preprocess
+ * additionally sorts every bin by Gaussian id (two more launches) and gsvox_forward walks each brick's whole key
+ * list in one CTA without atomics: the forward output is then bitwise identical from run to run and from plan to
+ * plan, at the price of the sort (0.22 ms at config 4, 2.9 ms at config 5) and of no hot-brick splitting in a3 (config 5 forward 1.36 -> 2.48 ms).  The backward keeps
+ * its fp32 atomics (gradients repeatable to ~1e-6 relative, north_star allows it).  Takes effect at the next
+ * gsvox_preprocess (until then forward/backward return GSVOX_ENOTREADY).  Bins longer than 51200 keys are left
+ * unsorted and counted: gsvox_plan_unsorted_bins (SYNCHRONISES; -1 when the mode is off).                      */
+int gsvox_plan_set_deterministic(gsvox_plan* plan, int32_t enabled);
+int gsvox_plan_unsorted_bins(gsvox_plan* plan, int64_t* unsorted_bins, void* stream);
+
 /* Debug/parity read-back of the latest preprocess (SYNCHRONISES): integer voxel boxes
  * box_host [n,6] = lo_x,lo_y,lo_z,hi_x,hi_y,hi_z inclusive (0,0,0,-1,-1,-1 when empty or
  * skipped) and the inverse covariance in index units minv_host [n,6] = xx,xy,xz,yy,yz,zz

@@ -24,7 +24,7 @@ EXPORTS = [
     "gsvox_plan_set_slab", "gsvox_backward_accumulate", "gsvox_backward_finish", "gsvox_plan_accumulators",
     "gsvox_project_scratch_bytes", "gsvox_project_forward", "gsvox_project_backward",
     "gsvox_splat_workspace_bytes", "gsvox_splat_forward", "gsvox_splat_backward", "gsvox_splat_status",
-    "gsvox_splat_drops",
+    "gsvox_splat_drops", "gsvox_plan_set_deterministic", "gsvox_plan_unsorted_bins",
 ]
 PROBE_EXPORTS = ["gsvox_probe_peaks"]            # include/gsvox_probe.h, libgsvox_probe.so (bench only)
 
@@ -84,6 +84,8 @@ def lib():
     L.gsvox_warp_forward.argtypes = [vp, vp, gp, i32, vp, vp]
     L.gsvox_warp_backward.argtypes = [vp, vp, gp, i32, vp, vp, vp, vp]
     L.gsvox_plan_set_slab.argtypes = [vp, i32, i32]
+    L.gsvox_plan_set_deterministic.argtypes = [vp, i32]
+    L.gsvox_plan_unsorted_bins.argtypes = [vp, C.POINTER(i64), vp]
     L.gsvox_backward_accumulate.argtypes = [vp, vp, i32, vp, vp]
     L.gsvox_backward_finish.argtypes = [vp, i32, vp, vp, vp, vp, vp]
     L.gsvox_plan_accumulators.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(i64)]
@@ -460,6 +462,16 @@ class Plan:
     def set_slab(self, bz_begin, bz_end):
         _check(lib().gsvox_plan_set_slab(self._h, int(bz_begin), int(bz_end)))
         self.n = None
+
+    def set_deterministic(self, on=True):
+        """Sort every (brick, class) bin by Gaussian id and run a3 without atomics: bitwise repeatable forward."""
+        _check(lib().gsvox_plan_set_deterministic(self._h, 1 if on else 0))
+        self.n = None
+
+    def unsorted_bins(self):
+        v = C.c_int64(0)
+        _check(lib().gsvox_plan_unsorted_bins(self._h, C.byref(v), _stream()))
+        return int(v.value)
 
     def backward_accumulate(self, weight, grad_out):
         ch = int(weight.shape[1])

@@ -177,6 +177,14 @@ extern "C" int gsvox_backward(gsvox_plan* p, const float* weight, int32_t channe
     return launch_backward(p, weight, channels, grad_out, gw, gp, gs, gq, (cudaStream_t)stream);
 }
 
+extern "C" int gsvox_plan_set_deterministic(gsvox_plan* p, int32_t enabled)
+{
+    if (!p) return GSVOX_EINVAL;
+    p->deterministic = enabled ? 1 : 0;
+    p->n = -1;                                   // the binning in the workspace was made in the other mode
+    return GSVOX_OK;
+}
+
 // ------------------------------------------------------------------ multi-GPU z-slabs
 extern "C" int gsvox_plan_set_slab(gsvox_plan* p, int32_t bz_begin, int32_t bz_end)
 {

@@ -525,7 +525,7 @@ __global__ void __launch_bounds__(32, 32)
 k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
              const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
              const float* __restrict__ weight, int wstride, int c0,
-             float* __restrict__ out, GridDev gd)
+             float* __restrict__ out, GridDev gd, uint32_t max_keys)
 {
     __shared__ __align__(16) float s_raw[kB1Batch * kB1Words];
     __shared__ __align__(16) float s_rec[kB1Batch * kB1Words];
@@ -533,7 +533,8 @@ k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_sta
     uint32_t kbeg = 0, kend = 0;
     if (!status->overflow) {
         kbeg = bin_start[b * kNumClasses];
-        kend = min(bin_start[(b + 1) * kNumClasses], kbeg + (uint32_t)kSplitKeys);
+        kend = bin_start[(b + 1) * kNumClasses];
+        if (kend - kbeg > max_keys) kend = kbeg + max_keys;         // kSplitKeys; deterministic mode: the whole range
     }
     b1_brick<VEC, false>(rec, keys, weight, wstride, c0, out, gd, s_raw, s_rec, b, kbeg, kend);
 }
@@ -566,9 +567,12 @@ static int launch_fwd_b1(gsvox_plan* p, const float* weight, int C, int c0, floa
     const bool vec = (p->gd.dims[0] % 4 == 0) && (((uintptr_t)out & 15) == 0);
     const int nblocks = (p->gd.slab1 - p->gd.slab0) * p->gd.nb[0] * p->gd.nb[1];
     if (nblocks <= 0) return GSVOX_OK;
-    if (vec) k_forward_b1<true><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd);
-    else     k_forward_b1<false><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd);
+    // deterministic mode: one warp walks its brick's whole key list in the sorted order, no second launch, no atomics
+    const uint32_t max_keys = p->deterministic ? 0xffffffffu : (uint32_t)kSplitKeys;
+    if (vec) k_forward_b1<true><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd, max_keys);
+    else     k_forward_b1<false><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd, max_keys);
     GSVOX_CUDA(cudaGetLastError());
+    if (p->deterministic) return GSVOX_OK;
     p->launches[GSVOX_K_FORWARD] += 1;               // the hot-brick launch
     if (vec) k_forward_b1_extra<true><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
                                                                  p->split_cap, weight, C, c0, out, p->gd);

@@ -36,6 +36,18 @@ extern "C" int gsvox_plan_status(gsvox_plan* p, gsvox_status* status, void* stre
     return GSVOX_OK;
 }
 
+extern "C" int gsvox_plan_unsorted_bins(gsvox_plan* p, int64_t* unsorted_bins, void* stream)
+{
+    if (!p || !unsorted_bins) return GSVOX_EINVAL;
+    if (p->n < 0) return GSVOX_ENOTREADY;
+    cudaStream_t st = (cudaStream_t)stream;
+    DevStatus h;
+    GSVOX_CUDA(cudaMemcpyAsync(&h, p->status, sizeof h, cudaMemcpyDeviceToHost, st));
+    GSVOX_CUDA(cudaStreamSynchronize(st));
+    *unsorted_bins = p->deterministic ? (int64_t)h.unsorted : -1;
+    return GSVOX_OK;
+}
+
 extern "C" int gsvox_plan_geometry_host(gsvox_plan* p, int32_t* box_host, float* minv_host, void* stream)
 {
     if (!p) return GSVOX_EINVAL;

@@ -51,7 +51,7 @@ struct DevStatus {
     unsigned long long culled;        // keys dropped by the conservative q_min > 64 test (reading A15)
     unsigned long long pairs_exec;    // P_exec: pairs of the kept keys
     unsigned int nsplit;              // extra key-range segments of hot bricks (entries of the split list)
-    unsigned int pad_;
+    unsigned int unsorted;            // deterministic mode: (brick, class) bins too long to be sorted by Gaussian id
 };
 
 struct GridDev {
@@ -156,6 +156,7 @@ struct gsvox_plan {
     cudaStream_t side[2];
     cudaEvent_t side_ev[4];
     int side_ready;
+    int deterministic;         // gsvox_plan_set_deterministic: keys of every bin sorted by Gaussian id, a3 without atomics
 };
 
 namespace gsvox {
@@ -175,6 +176,7 @@ int cuda_fail(cudaError_t e, const char* what);          // records text, return
 int launch_preprocess(gsvox_plan* p, const float* pos, const float* scale, const float* quat,
                       int64_t n, cudaStream_t st);
 int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st);
+int launch_sort_bins(gsvox_plan* p, cudaStream_t st);
 int launch_exclusive_scan(uint32_t* cnt, int nbins, uint32_t* partial, uint32_t* start,
                           unsigned long long* keys_needed, unsigned int* overflow,
                           unsigned long long key_capacity, cudaStream_t st);

@@ -426,6 +426,76 @@ int launch_exclusive_scan(uint32_t* cnt, int nbins, uint32_t* partial, uint32_t*
     return GSVOX_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// Deterministic mode (gsvox_plan_set_deterministic; SURVEY section 7 hard part 3, section 4 test 6): the counting
+// sort leaves the keys of a (brick, class) bin in whatever order the atomics produced.  Here every bin is sorted by
+// Gaussian id, in place: the bin is loaded into shared memory, every key counts the smaller ones (ids are unique
+// inside a bin), and is written to that rank.  k_sort_bins: one CTA per brick, bins up to kSortSmall keys (config 4:
+// 18 keys per bin on average).  k_sort_bins_large: the longer bins of hot bricks (one item of the split list per
+// brick), up to kSortLarge keys in 200 KB of shared memory; anything longer stays unsorted and is counted.
+// ------------------------------------------------------------------------------------------
+constexpr int kSortSmall = 4096, kSortLarge = 51200;
+
+template <int THREADS>
+__device__ __forceinline__ void sort_bin_in_place(uint32_t* __restrict__ keys, uint32_t beg, uint32_t len, uint32_t* s_keys)
+{
+    for (uint32_t i = threadIdx.x; i < len; i += THREADS) s_keys[i] = keys[beg + i];
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < len; i += THREADS) {
+        const uint32_t mine = s_keys[i];
+        uint32_t rank = 0;
+        for (uint32_t j = 0; j < len; ++j) rank += (s_keys[j] < mine) ? 1u : 0u;
+        keys[beg + rank] = mine;
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(128)
+k_sort_bins(const uint32_t* __restrict__ bin_start, uint32_t* __restrict__ keys, const DevStatus* __restrict__ status, GridDev gd)
+{
+    __shared__ uint32_t s_keys[kSortSmall];
+    if (status->overflow) return;
+    const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];
+    for (int c = 0; c < kNumClasses; ++c) {
+        const uint32_t beg = bin_start[b * kNumClasses + c], len = bin_start[b * kNumClasses + c + 1] - beg;
+        if (len >= 2u && len <= (uint32_t)kSortSmall) sort_bin_in_place<128>(keys, beg, len, s_keys);     // CTA-uniform
+    }
+}
+
+__global__ void __launch_bounds__(1024)
+k_sort_bins_large(const uint32_t* __restrict__ bin_start, uint32_t* __restrict__ keys, DevStatus* __restrict__ status,
+                  const uint2* __restrict__ split_list, int split_cap)
+{
+    extern __shared__ uint32_t s_big[];
+    if (status->overflow) return;
+    const uint32_t nitems = min(status->nsplit, (uint32_t)split_cap);
+    for (uint32_t i = blockIdx.x; i < nitems; i += gridDim.x) {
+        const uint2 item = split_list[i];
+        if (item.y != 1u) continue;                          // one item per hot brick does the brick
+        for (int c = 0; c < kNumClasses; ++c) {
+            const uint32_t beg = bin_start[item.x * kNumClasses + c], len = bin_start[item.x * kNumClasses + c + 1] - beg;
+            if (len <= (uint32_t)kSortSmall) continue;
+            if (len <= (uint32_t)kSortLarge) sort_bin_in_place<1024>(keys, beg, len, s_big);
+            else if (threadIdx.x == 0) atomicAdd(&status->unsorted, 1u);
+        }
+    }
+}
+
+int launch_sort_bins(gsvox_plan* p, cudaStream_t st)
+{
+    const int nblocks = (p->gd.slab1 - p->gd.slab0) * p->gd.nb[0] * p->gd.nb[1];
+    if (nblocks <= 0) return GSVOX_OK;
+    LaunchScope ls(p, GSVOX_K_SCATTER, st);
+    k_sort_bins<<<nblocks, 128, 0, st>>>(p->bin_start, p->keys, p->status, p->gd);
+    GSVOX_CUDA(cudaGetLastError());
+    const size_t smem = sizeof(uint32_t) * (size_t)kSortLarge;
+    GSVOX_CUDA(cudaFuncSetAttribute(k_sort_bins_large, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_sort_bins_large<<<148, 1024, smem, st>>>(p->bin_start, p->keys, p->status, p->split_list, p->split_cap);
+    GSVOX_CUDA(cudaGetLastError());
+    p->launches[GSVOX_K_SCATTER] += 1;
+    return GSVOX_OK;
+}
+
 int launch_preprocess(gsvox_plan* p, const float* pos, const float* scale, const float* quat,
                       int64_t n, cudaStream_t st)
 {
@@ -460,6 +530,7 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
         k_keys<1><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status,
                                            p->bin_start, p->split_list, p->split_cap);
         GSVOX_CUDA(cudaGetLastError());
+        if (p->deterministic) { int rc = launch_sort_bins(p, st); if (rc != GSVOX_OK) return rc; }
     }
     return GSVOX_OK;
 }

@@ -282,6 +282,48 @@ def test_forward_is_run_to_run_stable_within_tolerance(pkg):
         assert np.linalg.norm(x - y) <= 1e-5 * np.linalg.norm(x)
 
 
+@pytest.mark.parametrize("which", ["config4_recipe", "hot_bricks", "channels3", "needles"])
+def test_deterministic_mode_gives_a_bitwise_repeatable_forward(pkg, which):
+    """gsvox_plan_set_deterministic (SURVEY section 7 hard part 3, section 4 test 6): every (brick, class) bin sorted by
+    Gaussian id and a3 without atomics.  Two INDEPENDENT plans (their counting sorts race differently) must then
+    hold identical key arrays and produce the same forward bits, also across repeated preprocess calls; parity with
+    the oracle is unchanged; the default mode is only required to agree to rounding."""
+    case = {"config4_recipe": lambda: gsvox_inputs.config4(n=20000, dims=(96, 88, 72)),
+            "hot_bricks": lambda: gsvox_inputs.config1(n=6000, dims=(16, 15, 13), seed=88),
+            "channels3": lambda: gsvox_inputs.subvolume_case(n=3000, channels=3, seed=23),
+            "needles": lambda: gsvox_inputs.config5(n=20000, dims=(128, 96, 64))}[which]()
+    t = (dev(case.pos), dev(case.scale), dev(case.quat), dev(case.weight))
+    outs, keysets = [], []
+    for rep in range(3):
+        plan = pkg.Plan(case.n, case.grid, max_channels=case.channels)
+        plan.set_deterministic(True)
+        for _ in range(1 + rep):                                   # repeated preprocess on the same plan as well
+            plan.preprocess(*t[:3])
+        assert not plan.status()["overflow"] and plan.unsorted_bins() == 0
+        outs.append(plan.forward(t[3]).clone())
+        start, keys = plan.bins()
+        keysets.append((start.copy(), keys.copy()))
+    for o in outs[1:]:
+        assert torch.equal(o, outs[0]), "deterministic forward differs between plans"
+    for st_, k_ in keysets[1:]:
+        assert np.array_equal(st_, keysets[0][0]) and np.array_equal(k_, keysets[0][1])
+    # keys of a brick are grouped by class; inside a class they ascend
+    start, keys = keysets[0]
+    ref = oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid)
+    check_forward(outs[0].cpu().numpy(), ref)
+    g = case.grad_out()
+    grads = [x.cpu().numpy() for x in plan.backward(t[3], dev(g))]
+    check_grads(grads, oracle.backward(case.pos, case.scale, case.quat, case.weight, case.grid, g), case)
+    # and the mode can be switched off again: same values to rounding
+    plan.set_deterministic(False)
+    with pytest.raises(pkg.GsvoxError):
+        plan.forward(t[3])                                         # needs a new preprocess
+    plan.preprocess(*t[:3])
+    assert plan.unsorted_bins() == -1
+    o2 = plan.forward(t[3])
+    assert float((o2 - outs[0]).abs().max()) <= 1e-5 * float(outs[0].abs().max())      # another summation order, same values
+
+
 def test_host_buffer_step_matches_device_path(pkg):
     case = gsvox_inputs.config1(n=1200, dims=(40, 32, 24), seed=6)
     g = case.grad_out()
