@@ -330,6 +330,8 @@ def cone_rays(grid, geom, angle):
     """geom = dict(sad, sdd, nu, nv, du, dv, off_u, off_v, iso[3]).  -> per-pixel [nv, nu] arrays:
     dominant axis a, and fp64 (p0, ps, q0, qs, weight) for the two in-plane axes (b, c) = the axes
     other than a in ascending order, all in voxel index units."""
+    from .splat import geom32
+    geom = geom32(geom)                                       # fp32 scalars, as gsvox_cone_geometry carries them
     o, h, dims = _grid(grid)
     o = o.astype(np.float64); h = h.astype(np.float64)
     ca, sa = np.cos(np.float64(angle)), np.sin(np.float64(angle))
@@ -431,4 +433,4 @@ def project_backward(grad_drr, grid, geom, angles):
 
 
 # Gaussian-splat X-ray rasterizer (Eq. 6-9) — oracle/splat.py (torch fp64)
-from .splat import splat_backward, splat_forward, splat_forward_at, splat_terms   # noqa: E402,F401
+from .splat import splat_backward, splat_forward, splat_forward_at, splat_forward_boxes, splat_terms   # noqa: E402,F401

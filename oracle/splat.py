@@ -30,10 +30,24 @@ def _t(a):
     return torch.as_tensor(np.ascontiguousarray(np.asarray(a, dtype=np.float32)), dtype=torch.float32).to(torch.float64)
 
 
+def geom32(geom):
+    """The scanner geometry as the boundary carries it: gsvox_cone_geometry holds fp32 scalars (sad, sdd, du, dv,
+    off_u, off_v, iso), so — like every other input ("inputs are fp32; the oracle promotes them
+    exactly") — they are rounded to fp32 once and promoted to fp64.  0.776 mm is not an fp32 number: taking it as the
+    Python double moved cu + 3 sigma by 1e-6 pixel and one box edge of 400 000 across an integer (found by the
+    every-pixel parity at the bench size)."""
+    g = dict(geom)
+    for k in ("sad", "sdd", "du", "dv", "off_u", "off_v"):
+        g[k] = float(np.float32(geom[k]))
+    g["iso"] = [float(np.float32(v)) for v in geom["iso"]]
+    return g
+
+
 def splat_terms(pos, scale, quat, rho, geom, angle, kappa=KAPPA):
     """Per-Gaussian 2D quantities for one gantry angle (torch fp64, differentiable):
     centre in pixel coordinates (cu, cv), conic (A, B, C) in pixel units, amplitude, inclusive
     integer box (u0, v0, u1, v1) and validity."""
+    geom = geom32(geom)
     qn = quat / quat.norm(dim=1, keepdim=True)
     r, x, y, z = qn[:, 0], qn[:, 1], qn[:, 2], qn[:, 3]
     R = torch.stack([1 - 2 * (y * y + z * z), 2 * (x * y - r * z), 2 * (x * z + r * y),
@@ -122,6 +136,28 @@ def splat_forward(pos, scale, quat, rho, geom, angles, kappa=KAPPA, return_pairs
             out.append(img.numpy()); pairs += k
     out = np.stack(out)
     return (out, pairs) if return_pairs else out
+
+
+def splat_forward_boxes(pos, scale, quat, rho, geom, angles, kappa=KAPPA):
+    """The same sum as splat_forward, organised per Gaussian instead of per pixel chunk: for every valid
+    (angle, Gaussian) the 2D Gaussian of Eq. 9 is added on the pixels of its inclusive box, nothing else — a plain
+    double loop with numpy rows.  Cost is proportional to the pairs inside the cutoff, so the bench size (50 000
+    Gaussians, 8 angles, 512 x 384 pixels, 1e9 pairs) takes about a minute where the masked form above would take
+    hours; tests/test_splat_oracle_pins.py pins it to splat_forward.  -> drr [B, nv, nu] fp64."""
+    p, s, q, r = _t(pos), _t(scale), _t(quat), _t(rho).reshape(-1)
+    nu, nv = int(geom["nu"]), int(geom["nv"])
+    out = np.zeros((len(np.atleast_1d(angles)), nv, nu))
+    with torch.no_grad():
+        for b, a in enumerate(np.atleast_1d(np.asarray(angles, dtype=np.float32))):
+            cu, cv, A, B, C, amp, box, valid = (x.numpy() for x in splat_terms(p, s, q, r, geom, a, kappa))
+            img = out[b]
+            for i in np.flatnonzero(valid):
+                u0, v0, u1, v1 = (int(x) for x in box[i])
+                du = np.arange(u0, u1 + 1, dtype=np.float64) - cu[i]
+                dv = np.arange(v0, v1 + 1, dtype=np.float64) - cv[i]
+                qf = A[i] * du[None, :] ** 2 + 2.0 * B[i] * du[None, :] * dv[:, None] + C[i] * dv[:, None] ** 2
+                img[v0:v1 + 1, u0:u1 + 1] += amp[i] * np.exp(-0.5 * qf)
+    return out
 
 
 def splat_forward_at(pos, scale, quat, rho, geom, angle, pixels, kappa=KAPPA):

@@ -150,6 +150,26 @@ def test_splat_full_size_sampled_pixels(pkg):
           (worst / (FWD_REL * peak + FWD_ABS), rels, st["pairs"], st["keys_needed"]))
 
 
+def test_splat_full_size_every_pixel_forward(pkg):
+    """The bench workload (50 000 Gaussians, 8 angles, 512 x 384), EVERY pixel of all eight DRRs against the oracle's
+    per-Gaussian box form (oracle.splat_forward_boxes, pinned to splat_forward on the CPU); pair count exact."""
+    case = gsvox_inputs.splat_case()
+    drr, _, st = run_gpu(pkg, case)
+    assert not st["overflow"]
+    ref = oracle.splat_forward_boxes(case.pos, case.scale, case.quat, case.rho, case.geom, case.angles)
+    t = [oracle.splat._t(x) for x in (case.pos, case.scale, case.quat)] + [oracle.splat._t(case.rho).reshape(-1)]
+    pairs = 0
+    for a in case.angles:                                        # integer work: every box identical to the oracle's
+        terms = oracle.splat_terms(*t, case.geom, a)
+        bx = terms[6][terms[7]].numpy()
+        pairs += int(((bx[:, 2] - bx[:, 0] + 1) * (bx[:, 3] - bx[:, 1] + 1)).sum())
+    assert st["pairs"] == pairs, (st["pairs"], pairs)
+    err = np.abs(drr - ref).max()
+    tol = FWD_REL * np.abs(ref).max() + FWD_ABS
+    print("splat full size, every pixel: forward err/tol %.3f (max |drr| %.1f)" % (err / tol, np.abs(ref).max()))
+    assert err <= tol
+
+
 def test_splat_single_isolated_gaussians_worst_case_tolerance(pkg):
     """One Gaussian per image, footprints around the recurrence / direct switch (sigma ~ 0.85 pixel along
     x) and up: no averaging over neighbours hides the error of the multiplicative recurrence."""
