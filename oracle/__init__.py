@@ -433,4 +433,5 @@ def project_backward(grad_drr, grid, geom, angles):
 
 
 # Gaussian-splat X-ray rasterizer (Eq. 6-9) — oracle/splat.py (torch fp64)
-from .splat import splat_backward, splat_forward, splat_forward_at, splat_forward_boxes, splat_terms   # noqa: E402,F401
+from .splat import (splat_backward, splat_backward_boxes, splat_forward, splat_forward_at, splat_forward_boxes,   # noqa: E402,F401
+                    splat_terms)

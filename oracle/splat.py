@@ -204,3 +204,41 @@ def splat_backward(pos, scale, quat, rho, geom, angles, grad_drr, kappa=KAPPA, p
             (img * gb).sum().backward()
             gr[sl] += r.grad; gp[sl] += p.grad; gs[sl] += s.grad; gq[sl] += q.grad
     return gr.numpy(), gp.numpy(), gs.numpy(), gq.numpy()
+
+
+def splat_backward_boxes(pos, scale, quat, rho, geom, angles, grad_drr, kappa=KAPPA, group=64):
+    """splat_backward over ALL pixels at a cost proportional to the pairs inside the cutoff: the same autograd of the
+    same _render_subset, but each group of Gaussians (taken in the order of their projected centre, so that a group is
+    compact on the detector) is rendered only on the union of its boxes — outside every box `inside` is false and
+    the pixel contributes nothing to the loss, so the result is that of splat_backward.  Pinned to it on the CPU
+    (tests/test_splat_oracle_pins.py).  -> (d rho [n], d pos [n,3], d scale [n,3], d quat [n,4]) fp64."""
+    P, S, Q, Rh = _t(pos), _t(scale), _t(quat), _t(rho).reshape(-1)
+    n = P.shape[0]
+    angles = np.atleast_1d(np.asarray(angles, dtype=np.float32))
+    nu, nv = int(geom["nu"]), int(geom["nv"])
+    g = torch.as_tensor(np.asarray(grad_drr, dtype=np.float32)).to(torch.float64).reshape(angles.size, nv, nu)
+    gr, gp, gs, gq = torch.zeros(n, dtype=torch.float64), torch.zeros(n, 3, dtype=torch.float64), \
+        torch.zeros(n, 3, dtype=torch.float64), torch.zeros(n, 4, dtype=torch.float64)
+    for b, a in enumerate(angles):
+        with torch.no_grad():
+            cu0, cv0, _, _, _, _, box0, valid0 = splat_terms(P, S, Q, Rh, geom, a, kappa)
+        ids_all = torch.nonzero(valid0).reshape(-1)
+        if ids_all.numel() == 0:
+            continue
+        # order by 32-pixel detector cell of the centre: neighbours on the detector end up in the same group
+        cell = (torch.floor(cv0[ids_all] / 32.0) * 4096 + torch.floor(cu0[ids_all] / 32.0))
+        ids_all = ids_all[torch.argsort(cell, stable=True)]
+        for s0 in range(0, ids_all.numel(), group):
+            ids = ids_all[s0:s0 + group]
+            bx = box0[ids]
+            u0, v0 = int(bx[:, 0].min()), int(bx[:, 1].min())
+            u1, v1 = int(bx[:, 2].max()), int(bx[:, 3].max())
+            vv, uu = torch.meshgrid(torch.arange(v0, v1 + 1, dtype=torch.float64),
+                                    torch.arange(u0, u1 + 1, dtype=torch.float64), indexing="ij")
+            p, s, q, r = (P[ids].clone().requires_grad_(True), S[ids].clone().requires_grad_(True),
+                          Q[ids].clone().requires_grad_(True), Rh[ids].clone().requires_grad_(True))
+            cu, cv, A, B_, C, amp, box, valid = splat_terms(p, s, q, r, geom, a, kappa)
+            img, _ = _render_subset(torch.arange(ids.numel()), cu, cv, A, B_, C, amp, box, uu, vv)
+            (img * g[b, v0:v1 + 1, u0:u1 + 1]).sum().backward()
+            gr[ids] += r.grad; gp[ids] += p.grad; gs[ids] += s.grad; gq[ids] += q.grad
+    return gr.numpy(), gp.numpy(), gs.numpy(), gq.numpy()

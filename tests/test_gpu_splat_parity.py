@@ -170,6 +170,19 @@ def test_splat_full_size_every_pixel_forward(pkg):
     assert err <= tol
 
 
+def test_splat_full_size_every_pixel_backward(pkg):
+    """The bench workload again, gradients of L = <g, drr> with g on EVERY pixel of all eight DRRs, against the oracle's
+    box-restricted autograd (oracle.splat_backward_boxes, pinned to splat_backward on the CPU); group relative L2 and
+    the per-Gaussian bound."""
+    case = gsvox_inputs.splat_case()
+    g = case.grad_drr()
+    _, grads, st = run_gpu(pkg, case, grad=g)
+    assert not st["overflow"]
+    refs = oracle.splat_backward_boxes(case.pos, case.scale, case.quat, case.rho, case.geom, case.angles, g)
+    res = check_grad_groups(("rho", "pos", "scale", "quat"), grads, refs, tol=GRAD_REL, label="splat full size, every pixel")
+    print("splat full size, every pixel, gradients: %s" % fmt(res))
+
+
 def test_splat_single_isolated_gaussians_worst_case_tolerance(pkg):
     """One Gaussian per image, footprints around the recurrence / direct switch (sigma ~ 0.85 pixel along
     x) and up: no averaging over neighbours hides the error of the multiplicative recurrence."""

@@ -268,3 +268,21 @@ def test_per_gaussian_box_form_equals_the_per_pixel_form():
     assert a.shape == b.shape and np.abs(a).max() > 0
     assert np.allclose(a, b, rtol=1e-13, atol=1e-13 * np.abs(a).max())
     assert np.array_equal(a == 0.0, b == 0.0)                                # the same pixels are untouched
+
+
+def test_box_restricted_backward_equals_the_full_backward():
+    """splat_backward_boxes (every-pixel gradient parity at the bench size) against splat_backward, which central
+    differences hold in place: groups smaller than the set, clipped boxes, dropped Gaussians, signed amplitudes."""
+    rng = np.random.default_rng(14)
+    n = 50
+    pos = f32(rng.uniform(-70, 70, (n, 3))); scale = f32(rng.uniform(1.0, 9.0, (n, 3)))
+    quat = f32(rng.standard_normal((n, 4))); rho = f32(rng.standard_normal(n))
+    pos[0] = (1200.0, 0.0, 0.0); pos[1] = (0.0, 0.0, 400.0)
+    angles = [0.0, 2.9, 5.1]
+    g = rng.standard_normal((3, GEOM["nv"], GEOM["nu"])).astype(np.float32)
+    full = oracle.splat_backward(pos, scale, quat, rho, GEOM, angles, g)
+    for group in (7, 64):
+        part = oracle.splat_backward_boxes(pos, scale, quat, rho, GEOM, angles, g, group=group)
+        for a, b in zip(full, part):
+            assert np.allclose(a, b, rtol=1e-11, atol=1e-13 * max(1.0, np.abs(a).max()))
+    assert np.abs(full[1]).max() > 0 and not full[1][0].any()
