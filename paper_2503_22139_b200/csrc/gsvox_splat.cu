@@ -459,27 +459,32 @@ k_splat_backward(SplatParams P, const Splat2D* __restrict__ rec, const uint32_t*
             const float4* rp = reinterpret_cast<const float4*>(rec + id);
             const float4 a = __ldg(rp), c = __ldg(rp + 1);
             const int4 w = __ldg(reinterpret_cast<const int4*>(rp + 2));
-            const float cfu = a.x, cfv = a.y, A = a.z, Bc = a.w, C = c.x;             // c.y = amp (applied in s5)
+            const float cfu = a.x, cfv = a.y, A = a.z;                                // c.y = amp (applied in s5)
+            const float Bq = __int_as_float(w.y), Dq = __int_as_float(w.z);           // row form: E = A t^2 + Dq dy^2, t = dx + Bq dy
             const int ciu = (int16_t)(__float_as_int(c.z) & 0xffff), civ = (int16_t)(__float_as_int(c.z) >> 16);
             const int u0 = (int16_t)(__float_as_int(c.w) & 0xffff), v0 = (int16_t)(__float_as_int(c.w) >> 16);
             const int u1 = (int16_t)(w.x & 0xffff), v1 = (int16_t)(w.x >> 16);
             const int x0 = max(u0 - ox, 0), x1 = min(u1 - ox, kSplatTile - 1), y0 = max(v0 - oy, 0), y1 = min(v1 - oy, kSplatTile - 1);
-            float m0 = 0.f, mx = 0.f, my = 0.f, mxx = 0.f, mxy = 0.f, myy = 0.f;
+            // Moments of g E about the centre in the SHEARED frame (t, dy), t = dx + Bq dy = distance from the row's ridge:
+            // for an elongated footprint t is the transverse coordinate, and sum g E t^2 is summed directly instead of
+            // being the small difference of raw dx/dy moments (fp32 raw moments lost (s_max/s_min)^2: a 34:1 needle seen
+            // at 240:1 in 2D had its scale/quaternion gradients off by 1.7e-4).  s5 goes back to raw moments in fp64.
+            float m0 = 0.f, mt = 0.f, my = 0.f, mtt = 0.f, mty = 0.f, myy = 0.f;
             for (int y = y0; y <= y1; ++y) {
                 const float dy = (float)(oy + y - civ) - cfv;
-                const float cy = C * dy * dy, by = 2.f * Bc * dy;
-                float r0 = 0.f, r1 = 0.f, r2 = 0.f;               // row sums of g E {1, dx, dx^2}
+                const float ey = Dq * dy * dy, sh = fmaf(Bq, dy, -cfu);
+                float r0 = 0.f, r1 = 0.f, r2 = 0.f;               // row sums of g E {1, t, t^2}
                 for (int x = x0; x <= x1; ++x) {
-                    const float dx = (float)(ox + x - ciu) - cfu;
-                    const float gE = s_g[y * kSplatTile + x] * ex2s(fmaf(A * dx, dx, fmaf(by, dx, cy)));
-                    r0 += gE; const float t = gE * dx; r1 += t; r2 = fmaf(t, dx, r2);
+                    const float t = (float)(ox + x - ciu) + sh;
+                    const float gE = s_g[y * kSplatTile + x] * ex2s(fmaf(A * t, t, ey));
+                    r0 += gE; const float q = gE * t; r1 += q; r2 = fmaf(q, t, r2);
                 }
-                m0 += r0; mx += r1; mxx += r2;
-                my = fmaf(dy, r0, my); mxy = fmaf(dy, r1, mxy); myy = fmaf(dy * dy, r0, myy);
+                m0 += r0; mt += r1; mtt += r2;
+                my = fmaf(dy, r0, my); mty = fmaf(dy, r1, mty); myy = fmaf(dy * dy, r0, myy);
             }
             float* dst = acc + (size_t)id * 8;
-            asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" :: "l"(dst), "f"(m0), "f"(mx), "f"(my), "f"(mxx) : "memory");
-            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" :: "l"(dst + 4), "f"(mxy), "f"(myy) : "memory");
+            asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" :: "l"(dst), "f"(m0), "f"(mt), "f"(my), "f"(mtt) : "memory");
+            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" :: "l"(dst + 4), "f"(mty), "f"(myy) : "memory");
         }
         __syncthreads();                                        // s_key / s_hist are reused by the next chunk
     }
@@ -511,7 +516,10 @@ k_splat_epilogue(SplatParams P, const float* __restrict__ pos, const float* __re
         splat_terms(P, b, pos, scale, quat, g, o);
         if (!o.valid) continue;
         const float* m = acc + idx * 8;
-        const double m0 = m[0], mx = m[1], my = m[2], mxx = m[3], mxy = m[4], myy = m[5];
+        // sheared-frame moments (t = dx + Bq dy, with the Bq the kernel used) -> raw moments, in fp64
+        const double bq = (double)rec[idx].Bq;
+        const double m0 = m[0], my = m[2], myy = m[5];
+        const double mx = m[1] - bq * my, mxy = m[4] - bq * myy, mxx = m[3] - 2.0 * bq * m[4] + bq * bq * myy;
         const double amp = rh * o.amp_over_rho;
         const double A = o.P[2] / o.dp, Bc = -o.P[1] / o.dp, C = o.P[0] / o.dp;
         const double g_amp = m0, gA = -0.5 * amp * mxx, gB = -amp * mxy, gC = -0.5 * amp * myy;

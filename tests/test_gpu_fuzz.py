@@ -6,8 +6,13 @@ import numpy as np
 import pytest
 
 import gsvox_inputs
+import os
+
 import oracle
 from parity_util import per_row_worst
+
+# GSVOX_FUZZ_SEEDS=n widens every sweep to n seeds (default: 24 / 8 / 8, sized for the round-end run)
+_N = int(os.environ.get("GSVOX_FUZZ_SEEDS", "0"))
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -32,7 +37,7 @@ def rel_l2(a, b):
     return np.linalg.norm(a.astype(np.float64) - b) / nb if nb > 0 else float(np.abs(a).max())
 
 
-@pytest.mark.parametrize("seed", range(24))
+@pytest.mark.parametrize("seed", range(_N or 24))
 def test_voxelizer_random_cases(pkg, seed):
     rng = np.random.default_rng(1000 + seed)
     dims = tuple(int(v) for v in rng.choice([1, 3, 7, 8, 9, 16, 23, 40], size=3))
@@ -63,14 +68,14 @@ def test_voxelizer_random_cases(pkg, seed):
     assert np.abs(out - ref).max() <= 1e-5 * np.abs(ref).max() + 1e-6, seed
     refs = oracle.backward(case.pos, case.scale, case.quat, case.weight, case.grid, g)
     for name, a, b in zip("wpsq", grads, refs):
-        if np.linalg.norm(b) > 1e-12:
+        if np.linalg.norm(b) > 1e-8:
             assert rel_l2(a, b) <= 1e-4, (seed, name, rel_l2(a, b))
             assert per_row_worst(a, b)[0] <= 1.0, (seed, name, per_row_worst(a, b))
-        else:
-            assert np.abs(a).max() <= 1e-6, (seed, name)
+        else:       # every Gaussian so far from its voxels that all terms are below e^-20 (seed 277: 6e-11 vs an exact 0)
+            assert np.abs(a - b).max() <= 1e-8, (seed, name)
 
 
-@pytest.mark.parametrize("seed", range(8))
+@pytest.mark.parametrize("seed", range(_N or 8))
 def test_warp_and_projector_random_cases(pkg, seed):
     rng = np.random.default_rng(2000 + seed)
     dims = tuple(int(v) for v in rng.choice([4, 9, 16, 21, 33], size=3))
@@ -96,7 +101,7 @@ def test_warp_and_projector_random_cases(pkg, seed):
     assert rel_l2(gv, oracle.project_backward(pc.grad_drr(), pc.grid, pc.geom, pc.angles)) <= 1e-4, seed
 
 
-@pytest.mark.parametrize("seed", range(8))
+@pytest.mark.parametrize("seed", range(_N or 8))
 def test_splat_random_cases(pkg, seed):
     rng = np.random.default_rng(3000 + seed)
     B = int(rng.choice([1, 2, 4]))
