@@ -158,9 +158,10 @@ int gsvox_plan_timings(gsvox_plan* plan, double* ms /*[GSVOX_K_COUNT_KINDS]*/,
  * at least gsvox_host_staging_bytes(); host buffers should be pinned.  out_host may be NULL
  * (skip the volume read-back) and grad_out_host may be NULL (forward only).  The upstream gradient
  * is uploaded and the volume downloaded on two copy streams owned by the plan, overlapped with the
- * kernels (both ordered after work already enqueued on `stream`).  What the library creates behind the caller's
+ * kernels (both ordered after work already enqueued on `stream`); for C = 1 the gradient travels in four pieces of whole
+ * brick layers and a4 runs piece by piece as they arrive.  What the library creates behind the caller's
  * back, all of it HOST-side and owned by the plan: the plan object itself (gsvox_plan_create: heap), and on the first
- * gsvox_step_host two non-blocking CUDA streams and four events (destroyed by gsvox_plan_destroy); never device
+ * gsvox_step_host two non-blocking CUDA streams and eight events (destroyed by gsvox_plan_destroy); never device
  * memory.  Errors: GSVOX_EINVAL for a plan restricted to a z-slab (gsvox_plan_set_slab: it writes its own brick
  * layers only); on any error after the first copy was enqueued the call drains `stream` and both copy streams
  * before it returns, so no copy still references the caller's host buffers.                            */

@@ -139,7 +139,7 @@ extern "C" void gsvox_plan_destroy(gsvox_plan* p)
     free(p->pending);
     if (p->side_ready) {
         for (int i = 0; i < 2; ++i) cudaStreamDestroy(p->side[i]);
-        for (int i = 0; i < 4; ++i) cudaEventDestroy(p->side_ev[i]);
+        for (int i = 0; i < 4 + 8; ++i) if (p->side_ev[i]) cudaEventDestroy(p->side_ev[i]);
     }
     delete p;
 }

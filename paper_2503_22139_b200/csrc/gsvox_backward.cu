@@ -317,6 +317,43 @@ int launch_backward_accumulate(gsvox_plan* p, const float* weight, int channels,
     return rc;
 }
 
+// C = 1, for gsvox_step_host: a4 in pieces.  Piece `part` of `nparts` covers a contiguous range of brick layers (whole
+// z-slices of the gradient volume), so it can start as soon as THAT part of the upstream gradient has arrived on the
+// device; the caller waits on the matching copy event before each call.  part 0 zeroes the accumulators, the last part
+// also runs the hot-brick launch (which reads any part of the gradient).
+void backward_part_layers(const gsvox_plan* p, int part, int nparts, int* z0, int* z1)
+{
+    const int nl = p->gd.slab1 - p->gd.slab0;
+    *z0 = p->gd.slab0 + (int)((long long)nl * part / nparts);
+    *z1 = p->gd.slab0 + (int)((long long)nl * (part + 1) / nparts);
+}
+
+int launch_backward_part(gsvox_plan* p, const float* weight, const float* grad_out, int part, int nparts, cudaStream_t st)
+{
+    const int astride = acc_stride(1);
+    if (part == 0) {
+        LaunchScope ls(p, GSVOX_K_MEMSET, st);
+        GSVOX_CUDA(cudaMemsetAsync(p->acc, 0, sizeof(float) * (size_t)p->n * astride, st));
+    }
+    int z0, z1;
+    backward_part_layers(p, part, nparts, &z0, &z1);
+    GridDev gd = p->gd;
+    gd.slab0 = z0; gd.slab1 = z1;
+    const int nblocks = (z1 - z0) * gd.nb[0] * gd.nb[1];
+    LaunchScope ls(p, GSVOX_K_BACKWARD, st);
+    if (nblocks > 0) {
+        k_backward<1, true><<<nblocks, kBwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, 1, 0, grad_out,
+                                                             p->acc, astride, gd);
+        GSVOX_CUDA(cudaGetLastError());
+    }
+    if (part == nparts - 1) {
+        k_backward_extra<1, true><<<kSplitGrid / 2, kBwdThreads, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
+                                                                         p->split_cap, weight, 1, 0, grad_out, p->acc, astride, p->gd);
+        GSVOX_CUDA(cudaGetLastError());
+    }
+    return GSVOX_OK;
+}
+
 int launch_backward(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
                     float* gw, float* gp, float* gs, float* gq, cudaStream_t st)
 {

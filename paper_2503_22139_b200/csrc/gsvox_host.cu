@@ -4,9 +4,12 @@
 #include <cstdlib>
 #include <cstring>
 #include <vector>
+#include <algorithm>
 #include "gsvox_internal.cuh"
 
 using namespace gsvox;
+
+constexpr int kStepParts = 4;       // pieces of the upstream gradient in gsvox_step_host (C = 1)
 
 static void drain(gsvox_plan* p)
 {
@@ -204,7 +207,7 @@ static int step_host_enqueue(gsvox_plan* p, void* staging, size_t staging_bytes,
     // large H2D) travels while a1-a3 run, the volume (the large D2H) while a4-a5 run.
     if (!p->side_ready) {
         for (int i = 0; i < 2; ++i) GSVOX_CUDA(cudaStreamCreateWithFlags(&p->side[i], cudaStreamNonBlocking));
-        for (int i = 0; i < 4; ++i) GSVOX_CUDA(cudaEventCreateWithFlags(&p->side_ev[i], cudaEventDisableTiming));
+        for (int i = 0; i < 4 + kStepParts; ++i) GSVOX_CUDA(cudaEventCreateWithFlags(&p->side_ev[i], cudaEventDisableTiming));
         p->side_ready = 1;
     }
     cudaStream_t up = p->side[0], down = p->side[1];
@@ -216,9 +219,23 @@ static int step_host_enqueue(gsvox_plan* p, void* staging, size_t staging_bytes,
         GSVOX_CUDA(cudaMemcpyAsync(d + S.quat, quat_h, nn * 16, H2D, st));
         GSVOX_CUDA(cudaMemcpyAsync(d + S.weight, weight_h, nn * C * 4, H2D, st));
     }
+    // C = 1: the upstream gradient travels in kStepParts pieces of whole brick layers, and a4 runs piece by piece as they
+    // arrive (the upload of 67 MB at config 4 takes longer than a1-a3; a4 used to wait for all of it)
+    const bool parts = grad_out_h && C == 1 && nn > 0 && p->gd.nb[2] >= kStepParts;
     if (grad_out_h) {
         GSVOX_CUDA(cudaStreamWaitEvent(up, ev_begin, 0));
-        GSVOX_CUDA(cudaMemcpyAsync(d + S.vol_grad, grad_out_h, V * C * 4, H2D, up));
+        if (parts) {
+            const size_t slice = (size_t)p->grid.dims[0] * p->grid.dims[1];
+            for (int k = 0; k < kStepParts; ++k) {
+                int z0, z1;
+                backward_part_layers(p, k, kStepParts, &z0, &z1);
+                const size_t v0 = slice * (size_t)std::min(z0 * kBrick, p->grid.dims[2]), v1 = slice * (size_t)std::min(z1 * kBrick, p->grid.dims[2]);
+                if (v1 > v0) GSVOX_CUDA(cudaMemcpyAsync(d + S.vol_grad + 4 * v0, grad_out_h + v0, 4 * (v1 - v0), H2D, up));
+                GSVOX_CUDA(cudaEventRecord(p->side_ev[4 + k], up));
+            }
+        } else {
+            GSVOX_CUDA(cudaMemcpyAsync(d + S.vol_grad, grad_out_h, V * C * 4, H2D, up));
+        }
         GSVOX_CUDA(cudaEventRecord(ev_grad, up));
     }
     rc = gsvox_preprocess(p, (float*)(d + S.pos), (float*)(d + S.scale), (float*)(d + S.quat), n, stream);
@@ -231,10 +248,19 @@ static int step_host_enqueue(gsvox_plan* p, void* staging, size_t staging_bytes,
         GSVOX_CUDA(cudaMemcpyAsync(out_h, d + S.vol_out, V * C * 4, D2H, down));
         GSVOX_CUDA(cudaEventRecord(ev_out, down));
     }
-    if (grad_out_h) GSVOX_CUDA(cudaStreamWaitEvent(st, ev_grad, 0));
+    if (grad_out_h && !parts) GSVOX_CUDA(cudaStreamWaitEvent(st, ev_grad, 0));
     if (grad_out_h && nn) {
-        rc = gsvox_backward(p, (float*)(d + S.weight), C, (float*)(d + S.vol_grad), (float*)(d + S.gw),
-                            (float*)(d + S.gp), (float*)(d + S.gs), (float*)(d + S.gq), stream);
+        if (parts) {
+            for (int k = 0; k < kStepParts; ++k) {
+                GSVOX_CUDA(cudaStreamWaitEvent(st, p->side_ev[4 + k], 0));
+                rc = launch_backward_part(p, (float*)(d + S.weight), (float*)(d + S.vol_grad), k, kStepParts, st);
+                if (rc != GSVOX_OK) return rc;
+            }
+            rc = launch_epilogue(p, 1, (float*)(d + S.gw), (float*)(d + S.gp), (float*)(d + S.gs), (float*)(d + S.gq), st);
+        } else {
+            rc = gsvox_backward(p, (float*)(d + S.weight), C, (float*)(d + S.vol_grad), (float*)(d + S.gw),
+                                (float*)(d + S.gp), (float*)(d + S.gs), (float*)(d + S.gq), stream);
+        }
         if (rc != GSVOX_OK) return rc;
         GSVOX_CUDA(cudaMemcpyAsync(gw_h, d + S.gw, nn * C * 4, D2H, st));
         GSVOX_CUDA(cudaMemcpyAsync(gp_h, d + S.gp, nn * 12, D2H, st));

@@ -154,7 +154,7 @@ struct gsvox_plan {
     int n_pending, cap_pending;
     // gsvox_step_host: copy streams (H2D of the upstream gradient, D2H of the volume) and their events, created lazily
     cudaStream_t side[2];
-    cudaEvent_t side_ev[4];
+    cudaEvent_t side_ev[4 + 8];    // [4..]: arrival of the upstream-gradient parts (gsvox_step_host, C = 1)
     int side_ready;
     int deterministic;         // gsvox_plan_set_deterministic: keys of every bin sorted by Gaussian id, a3 without atomics
 };
@@ -185,6 +185,8 @@ int launch_backward(gsvox_plan* p, const float* weight, int channels, const floa
                     float* gw, float* gp, float* gs, float* gq, cudaStream_t st);
 int launch_backward_accumulate(gsvox_plan* p, const float* weight, int channels, const float* grad_out,
                                cudaStream_t st);
+void backward_part_layers(const gsvox_plan* p, int part, int nparts, int* z0, int* z1);
+int launch_backward_part(gsvox_plan* p, const float* weight, const float* grad_out, int part, int nparts, cudaStream_t st);
 int launch_epilogue(gsvox_plan* p, int channels, float* gw, float* gp, float* gs, float* gq, cudaStream_t st);
 
 }  // namespace gsvox

@@ -324,12 +324,15 @@ def test_deterministic_mode_gives_a_bitwise_repeatable_forward(pkg, which):
     assert float((o2 - outs[0]).abs().max()) <= 1e-5 * float(outs[0].abs().max())      # another summation order, same values
 
 
-def test_host_buffer_step_matches_device_path(pkg):
-    case = gsvox_inputs.config1(n=1200, dims=(40, 32, 24), seed=6)
+@pytest.mark.parametrize("dims", [(40, 32, 24), (40, 36, 70)])
+def test_host_buffer_step_matches_device_path(pkg, dims):
+    """(40, 36, 70): 9 brick layers, ragged in z — gsvox_step_host uploads the upstream gradient in four pieces of whole
+    brick layers and runs a4 piece by piece; (40, 32, 24): 3 layers, the unsplit path."""
+    case = gsvox_inputs.config1(n=1200, dims=dims, seed=6)
     g = case.grad_out()
     plan = pkg.Plan(case.n, case.grid)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    out = torch.empty((1, 24, 32, 40)).pin_memory()
+    out = torch.empty((1, dims[2], dims[1], dims[0])).pin_memory()
     grads = tuple(torch.empty((case.n, k)).pin_memory() for k in (1, 3, 3, 4))
     plan.step_host(pin(case.pos), pin(case.scale), pin(case.quat), pin(case.weight), pin(g), out, grads)
     check_forward(out.numpy(), oracle.forward(case.pos, case.scale, case.quat, case.weight, case.grid))
