@@ -1,8 +1,10 @@
 // gsvox_forward.cu — step a3: per-brick forward accumulation (Eq. 5).
 //
-// Two kernels: k_forward<CH> (CH = 3, 9: the motion-basis fields, channel groups of a wider C) described here, and
-// k_forward_b1 (C = 1: the CBCT volume, the headline configuration) further down, which re-cuts the same row
-// arithmetic around what actually limits it — operand delivery through shared memory.
+// Two kernels: k_forward<CH> (CH = 9: the motion-basis fields, channel groups of a wider C) described here, and
+// k_forward_b1<CH> (CH = 1: the CBCT volume, the headline configuration; CH = 3: one DVF level) further down,
+// which re-cuts the same row arithmetic around what actually limits it — operand delivery through shared memory.
+// (Nine channels as three b1<3> passes measured slower than k_forward<9>: 0.75/1.0/0.98 vs 0.50/0.70/0.62 ms on
+// config 3's levels; two rows x nine channels of accumulators do not fit a thread.)
 //
 // k_forward<CH>: one CTA of 64 threads per 8^3 brick; thread t owns the x-row (y = t&7, z = t>>3) of the brick,
 // i.e. 8 consecutive voxels per channel, accumulated in registers and written once.  The brick's
@@ -242,7 +244,7 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
 
 
 // ==========================================================================================
-// C = 1 fast path: one WARP per brick, two rows per thread.
+// C = 1 and C = 3 fast path: one WARP per brick, two rows per thread.
 //
 // What binds k_forward above is not arithmetic but operand delivery: every key costs each of the brick's two
 // warps ~21 words through LDS, and a warp-wide LDS.128 occupies the SM's one shared-memory return path for
@@ -262,7 +264,11 @@ k_forward(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
 // path has no clamp — such rows hold nothing but zeros, yet inf * 0 must not be formed).
 // ==========================================================================================
 constexpr int kB1Batch = 32;
-constexpr int kB1Words = 20;                        // staged record; also the stride of the raw copy (16 words, padded): conflict-free 128-bit per-lane access
+constexpr int kB1Words = 20;                        // staged record (C = 1); also the stride of the raw copy (16 words, padded): conflict-free 128-bit per-lane access
+// CH > 1 (the motion-basis fields, groups of three channels): words 12..19 hold the key-and-k factor alone,
+// km_k = [k inside the box in x] (fast keys: * c^{0,0,1,1,3,3,6,6}), words 20.. the CH weights; 28 words keep the
+// per-lane 128-bit staging stores conflict-free (stride 24 would map eight lanes onto four bank groups).
+template <int CH> struct B1Rec { static constexpr int kWords = (CH == 1) ? kB1Words : 28; };
 
 __device__ __forceinline__ void red_add_v4f(float* addr, float a, float b, float c, float d)
 {
@@ -297,8 +303,53 @@ __device__ __forceinline__ void recur_accumulate(float E3, float Lf, const float
     fma2_acc(acc[6], acc[7], P3, pk2(wb.z, wb.w));
 }
 
+// CH > 1: the same eight values, times km (four more FMUL2), then one broadcast weight per channel.
+template <int CH>
+__device__ __forceinline__ void recur_accumulate_ch(float E3, float Lf, const float4 ka, const float4 kb,
+                                                    const float (&w)[CH], float (&acc)[CH][8])
+{
+    const float G3 = ex2f(E3), rf = ex2f(Lf), rb = ex2f(-Lf);
+    const float G4 = G3 * rf;
+    const f32x2 R = pk2(rb, rf);
+    const f32x2 P0 = pk2(G3, G4);
+    const f32x2 P1 = mul2(P0, R);
+    const f32x2 P2 = mul2(P1, R);
+    const f32x2 P3 = mul2(P2, R);
+    const f32x2 Q0 = mul2(P0, pk2(ka.x, ka.y)), Q1 = mul2(P1, pk2(ka.z, ka.w));
+    const f32x2 Q2 = mul2(P2, pk2(kb.x, kb.y)), Q3 = mul2(P3, pk2(kb.z, kb.w));
+    #pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+        const f32x2 wv = pk2(w[ch], w[ch]);
+        fma2_acc(acc[ch][0], acc[ch][1], Q0, wv);
+        fma2_acc(acc[ch][2], acc[ch][3], Q1, wv);
+        fma2_acc(acc[ch][4], acc[ch][5], Q2, wv);
+        fma2_acc(acc[ch][6], acc[ch][7], Q3, wv);
+    }
+}
+
+template <int CH> struct B1W { float w[CH == 1 ? 1 : CH]; };
+template <int CH>
+__device__ __forceinline__ B1W<CH> load_w(const float* __restrict__ r)
+{
+    B1W<CH> o;
+    if constexpr (CH == 1) o.w[0] = 0.f;
+    else {
+        #pragma unroll
+        for (int ch = 0; ch < CH; ++ch) o.w[ch] = r[20 + ch];
+    }
+    return o;
+}
+template <int CH>
+__device__ __forceinline__ void row_accumulate(float E3, float Lf, const float4 wa, const float4 wb, const B1W<CH>& w,
+                                               float (&acc)[CH][8])
+{
+    if constexpr (CH == 1) recur_accumulate(E3, Lf, wa, wb, acc[0]);
+    else recur_accumulate_ch<CH>(E3, Lf, wa, wb, w.w, acc);
+}
+
 // One row of a slow key, scalar.
-__device__ __forceinline__ void eval_row_slow(const float* __restrict__ r, bool inrow, float fy, float fz, float (&acc)[8])
+template <int CH>
+__device__ __forceinline__ void eval_row_slow(const float* __restrict__ r, bool inrow, float fy, float fz, float (&acc)[CH][8])
 {
     const float dy = fy + r[1], dz = fz + r[2];
     const float negA = r[3];
@@ -321,23 +372,36 @@ __device__ __forceinline__ void eval_row_slow(const float* __restrict__ r, bool 
         G[1] = G[0] * rf; rf *= cc; G[3] = G[1] * rf; rf *= cc; G[5] = G[3] * rf; rf *= cc; G[7] = G[5] * rf;
         G[2] = G[0] * rb; rb *= cc; G[4] = G[2] * rb; rb *= cc; G[6] = G[4] * rb;
     }
-    #pragma unroll
-    for (int k = 0; k < 8; ++k) acc[k] = fmaf(G[k], r[12 + k], acc[k]);
+    if constexpr (CH == 1) {
+        #pragma unroll
+        for (int k = 0; k < 8; ++k) acc[0][k] = fmaf(G[k], r[12 + k], acc[0][k]);
+    } else {
+        #pragma unroll
+        for (int k = 0; k < 8; ++k) G[k] *= r[12 + k];
+        #pragma unroll
+        for (int ch = 0; ch < CH; ++ch) {
+            const float w = r[20 + ch];
+            #pragma unroll
+            for (int k = 0; k < 8; ++k) acc[ch][k] = fmaf(G[k], w, acc[ch][k]);
+        }
+    }
 }
 
 // A slow key (direct exponentials, or a recurrence that needs its clamps): scalar, row by row.
+template <int CH>
 __device__ __forceinline__ void eval_key_slow(const float* __restrict__ r, uint32_t lanebit, float fy, float fz,
-                                              float (&acc0)[8], float (&acc1)[8])
+                                              float (&acc0)[CH][8], float (&acc1)[CH][8])
 {
     const uint32_t m0 = __float_as_uint(r[10]), m1 = __float_as_uint(r[11]);
-    if (m0) eval_row_slow(r, (m0 & lanebit) != 0u, fy, fz, acc0);
-    if (m1) eval_row_slow(r, (m1 & lanebit) != 0u, fy, fz + 4.0f, acc1);
+    if (m0) eval_row_slow<CH>(r, (m0 & lanebit) != 0u, fy, fz, acc0);
+    if (m1) eval_row_slow<CH>(r, (m1 & lanebit) != 0u, fy, fz + 4.0f, acc1);
 }
 
 // A fast key that reaches both z-halves: setup of both rows at once, (row z, row z + 4) in the two halves of
 // a packed register, the key's scalars broadcast.
+template <int CH>
 __device__ __forceinline__ void eval_key_both(const float* __restrict__ r, uint32_t lanebit, float fy, f32x2 fz2,
-                                              float (&acc0)[8], float (&acc1)[8])
+                                              float (&acc0)[CH][8], float (&acc1)[CH][8])
 {
     const float4 q0 = *reinterpret_cast<const float4*>(r);
     const float4 q1 = *reinterpret_cast<const float4*>(r + 4);
@@ -358,14 +422,15 @@ __device__ __forceinline__ void eval_key_both(const float* __restrict__ r, uint3
     upk2(E3, E3a, E3b); upk2(Lf, Lfa, Lfb);
     E3a = (__float_as_uint(q2.z) & lanebit) ? E3a : -1.0e30f;        // rows outside the box contribute exact zeros
     E3b = (__float_as_uint(q2.w) & lanebit) ? E3b : -1.0e30f;
-    recur_accumulate(E3a, Lfa, wa, wb, acc0);
-    recur_accumulate(E3b, Lfb, wa, wb, acc1);
+    const B1W<CH> w = load_w<CH>(r);
+    row_accumulate<CH>(E3a, Lfa, wa, wb, w, acc0);
+    row_accumulate<CH>(E3b, Lfb, wa, wb, w, acc1);
 }
 
 // A fast key that reaches one z-half only: one row per thread, scalar setup.  HI: the half z = 4..7.
-template <bool HI>
+template <int CH, bool HI>
 __device__ __forceinline__ void eval_key_half(const float* __restrict__ r, uint32_t lanebit, float fy, float fzh,
-                                              float (&acc)[8])
+                                              float (&acc)[CH][8])
 {
     const float4 q0 = *reinterpret_cast<const float4*>(r);
     const float4 q1 = *reinterpret_cast<const float4*>(r + 4);
@@ -380,12 +445,12 @@ __device__ __forceinline__ void eval_key_half(const float* __restrict__ r, uint3
     float E3 = fmaf(nAt, t3, Es);
     const float Lf = fmaf(nAt, 2.0f, q0.w);
     E3 = (__float_as_uint(HI ? q2.w : q2.z) & lanebit) ? E3 : -1.0e30f;
-    recur_accumulate(E3, Lf, wa, wb, acc);
+    row_accumulate<CH>(E3, Lf, wa, wb, load_w<CH>(r), acc);
 }
 
 // Keys [kbeg, kend) of brick b.  ADD = false: the brick's rows are stored (segment 0; zeros for an empty brick);
 // ADD = true: a later segment of a hot brick, added atomically to what segment 0 stored.
-template <bool VEC, bool ADD>
+template <int CH, bool VEC, bool ADD>
 __device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const uint32_t* __restrict__ keys,
                                          const float* __restrict__ weight, int wstride, int c0, float* __restrict__ out,
                                          const GridDev& gd, float* __restrict__ s_raw, float* __restrict__ s_rec,
@@ -399,9 +464,12 @@ __device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const ui
     const f32x2 fz2 = pk2(fz, fz + 4.0f);
     const uint32_t lanebit = 1u << lane;
 
-    float acc0[8], acc1[8];                         // acc[2j], acc[2j+1] = voxels 3 - j, 4 + j
+    constexpr int KW = B1Rec<CH>::kWords;
+    float acc0[CH][8], acc1[CH][8];                 // acc[ch][2j], acc[ch][2j+1] = voxels 3 - j, 4 + j
     #pragma unroll
-    for (int j = 0; j < 8; ++j) { acc0[j] = 0.f; acc1[j] = 0.f; }
+    for (int ch = 0; ch < CH; ++ch)
+        #pragma unroll
+        for (int j = 0; j < 8; ++j) { acc0[ch][j] = 0.f; acc1[ch][j] = 0.f; }
 
     const uint32_t raw_addr = (uint32_t)__cvta_generic_to_shared(s_raw + lane * kB1Words);
     auto fetch = [&](uint32_t gid) {                // this lane's record -> s_raw, asynchronously
@@ -410,11 +478,14 @@ __device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const ui
         cp_async16(raw_addr + 32, rp + 32); cp_async16(raw_addr + 48, rp + 48);
     };
     uint32_t gid_next = 0;
-    float w_cur = 0.f, w_next = 0.f;
+    float w_cur[CH], w_next[CH];
+    #pragma unroll
+    for (int ch = 0; ch < CH; ++ch) { w_cur[ch] = 0.f; w_next[ch] = 0.f; }
     if (kbeg + lane < kend) {
         const uint32_t gid = keys[kbeg + lane];
         fetch(gid);
-        w_cur = __ldg(weight + (size_t)gid * wstride + c0);
+        #pragma unroll
+        for (int ch = 0; ch < CH; ++ch) w_cur[ch] = __ldg(weight + (size_t)gid * wstride + c0 + ch);
     }
     cp_async_commit();
     if (kbeg + kB1Batch + lane < kend) gid_next = keys[kbeg + kB1Batch + lane];
@@ -425,11 +496,11 @@ __device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const ui
         // ---- stage: lane l turns key l into brick-local form and classifies it; keys are stored class by class
         //      (slow | both halves | lower half only | upper half only) so that each class runs a branch-free loop
         int cls = -1;
-        float4 o0, o1, o2, o3, o4;
+        float4 o0, o1, o2, o3, o4, o5;
         if (base + lane < kend) {
             const float4* rp = reinterpret_cast<const float4*>(s_raw + lane * kB1Words);
             const float4 a = rp[0], bq = rp[1], c = rp[2], d = rp[3];
-            const float w = w_cur;
+            const float w = (CH == 1) ? w_cur[0] : 1.0f;          // CH > 1: words 12..19 carry km alone
             const int w1i = __float_as_int(d.y), w2i = __float_as_int(d.z), w3i = __float_as_int(d.w);
             const int lox = (int16_t)(w1i & 0xffff), loy = (int16_t)(w1i >> 16), loz = (int16_t)(w2i & 0xffff);
             const int hix = (int16_t)(w2i >> 16), hiy = (int16_t)(w3i & 0xffff), hiz = (int16_t)(w3i >> 16);
@@ -462,6 +533,7 @@ __device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const ui
             const float w1 = slow ? w : w * cc, c3 = cc * cc * cc, w3 = slow ? w : w * c3, w6 = slow ? w : w * (c3 * c3);
             o3 = make_float4((xm & 8u) ? w : 0.f, (xm & 16u) ? w : 0.f, (xm & 4u) ? w1 : 0.f, (xm & 32u) ? w1 : 0.f);
             o4 = make_float4((xm & 2u) ? w3 : 0.f, (xm & 64u) ? w3 : 0.f, (xm & 1u) ? w6 : 0.f, (xm & 128u) ? w6 : 0.f);
+            if constexpr (CH > 1) o5 = make_float4(w_cur[0], w_cur[1], w_cur[2 % CH], 0.f);
         }
         const uint32_t b0 = __ballot_sync(0xffffffffu, cls == 0), b1 = __ballot_sync(0xffffffffu, cls == 1),
                        b2 = __ballot_sync(0xffffffffu, cls == 2), b3 = __ballot_sync(0xffffffffu, cls == 3);
@@ -469,26 +541,35 @@ __device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const ui
         if (cls >= 0) {
             const uint32_t mine = cls == 0 ? b0 : (cls == 1 ? b1 : (cls == 2 ? b2 : b3));
             const int slot = (cls == 0 ? 0 : (cls == 1 ? n0 : (cls == 2 ? n1 : n2))) + __popc(mine & (lanebit - 1u));
-            float4* o = reinterpret_cast<float4*>(s_rec + slot * kB1Words);
+            float4* o = reinterpret_cast<float4*>(s_rec + slot * KW);
             o[0] = o0; o[1] = o1; o[2] = o2; o[3] = o3; o[4] = o4;
+            if constexpr (CH > 1) o[5] = o5;
         }
         __syncwarp();
         // next batch's records on their way while this one is evaluated
         if (base + kB1Batch + lane < kend) {
             fetch(gid_next);
-            w_next = __ldg(weight + (size_t)gid_next * wstride + c0);
+            #pragma unroll
+            for (int ch = 0; ch < CH; ++ch) w_next[ch] = __ldg(weight + (size_t)gid_next * wstride + c0 + ch);
         }
         cp_async_commit();
-        w_cur = w_next;
+        #pragma unroll
+        for (int ch = 0; ch < CH; ++ch) w_cur[ch] = w_next[ch];
         if (base + 2 * kB1Batch + lane < kend) gid_next = keys[base + 2 * kB1Batch + lane];
         int j = 0;
-        for (; j < n0; ++j) eval_key_slow(s_rec + j * kB1Words, lanebit, fy, fz, acc0, acc1);
+        for (; j < n0; ++j) eval_key_slow<CH>(s_rec + j * KW, lanebit, fy, fz, acc0, acc1);
+        if constexpr (CH > 1) {
+            for (; j + 1 < n1; j += 2) {
+                eval_key_both<CH>(s_rec + j * KW, lanebit, fy, fz2, acc0, acc1);
+                eval_key_both<CH>(s_rec + (j + 1) * KW, lanebit, fy, fz2, acc0, acc1);
+            }
+        }
         #pragma unroll 1
-        for (; j < n1; ++j) eval_key_both(s_rec + j * kB1Words, lanebit, fy, fz2, acc0, acc1);
+        for (; j < n1; ++j) eval_key_both<CH>(s_rec + j * KW, lanebit, fy, fz2, acc0, acc1);
         #pragma unroll 1
-        for (; j < n2; ++j) eval_key_half<false>(s_rec + j * kB1Words, lanebit, fy, fz, acc0);
+        for (; j < n2; ++j) eval_key_half<CH, false>(s_rec + j * KW, lanebit, fy, fz, acc0);
         #pragma unroll 1
-        for (; j < n3; ++j) eval_key_half<true>(s_rec + j * kB1Words, lanebit, fy, fz + 4.0f, acc1);
+        for (; j < n3; ++j) eval_key_half<CH, true>(s_rec + j * KW, lanebit, fy, fz + 4.0f, acc1);
     }
 
     // write (or add) the two rows; x fastest
@@ -498,10 +579,12 @@ __device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const ui
         const int gy = b0y + ry, gz = b0z + rz + 4 * h;
         if (gy < gd.dims[1] && gz < gd.dims[2]) {
             const size_t rowoff = ((size_t)gz * gd.dims[1] + gy) * gd.dims[0] + b0x;
+            #pragma unroll
+            for (int ch = 0; ch < CH; ++ch) {
             float v[8];
             #pragma unroll
-            for (int j = 0; j < 4; ++j) { v[3 - j] = h ? acc1[2 * j] : acc0[2 * j]; v[4 + j] = h ? acc1[2 * j + 1] : acc0[2 * j + 1]; }
-            float* o = out + (size_t)c0 * plane + rowoff;
+            for (int j = 0; j < 4; ++j) { v[3 - j] = h ? acc1[ch][2 * j] : acc0[ch][2 * j]; v[4 + j] = h ? acc1[ch][2 * j + 1] : acc0[ch][2 * j + 1]; }
+            float* o = out + (size_t)(c0 + ch) * plane + rowoff;
             if (VEC) {
                 if (ADD) {
                     if (b0x + 3 < gd.dims[0]) red_add_v4f(o, v[0], v[1], v[2], v[3]);
@@ -515,20 +598,21 @@ __device__ __forceinline__ void b1_brick(const GsRec* __restrict__ rec, const ui
                 for (int k2 = 0; k2 < 8; ++k2)
                     if (b0x + k2 < gd.dims[0]) { if (ADD) atomicAdd(o + k2, v[k2]); else o[k2] = v[k2]; }
             }
+            }
         }
     }
 }
 
 // First launch: one warp per brick, segment 0 of its key range.
-template <bool VEC>
-__global__ void __launch_bounds__(32, 32)
+template <int CH, bool VEC>
+__global__ void __launch_bounds__(32, CH == 1 ? 32 : 16)
 k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
              const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
              const float* __restrict__ weight, int wstride, int c0,
              float* __restrict__ out, GridDev gd, uint32_t max_keys)
 {
     __shared__ __align__(16) float s_raw[kB1Batch * kB1Words];
-    __shared__ __align__(16) float s_rec[kB1Batch * kB1Words];
+    __shared__ __align__(16) float s_rec[kB1Batch * B1Rec<CH>::kWords];
     const int b = blockIdx.x + gd.slab0 * gd.nb[0] * gd.nb[1];
     uint32_t kbeg = 0, kend = 0;
     if (!status->overflow) {
@@ -536,12 +620,12 @@ k_forward_b1(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_sta
         kend = bin_start[(b + 1) * kNumClasses];
         if (kend - kbeg > max_keys) kend = kbeg + max_keys;         // kSplitKeys; deterministic mode: the whole range
     }
-    b1_brick<VEC, false>(rec, keys, weight, wstride, c0, out, gd, s_raw, s_rec, b, kbeg, kend);
+    b1_brick<CH, VEC, false>(rec, keys, weight, wstride, c0, out, gd, s_raw, s_rec, b, kbeg, kend);
 }
 
 // Second launch: the later segments of hot bricks, a fixed grid striding over a2's item list.
-template <bool VEC>
-__global__ void __launch_bounds__(32, 32)
+template <int CH, bool VEC>
+__global__ void __launch_bounds__(32, CH == 1 ? 32 : 16)
 k_forward_b1_extra(const GsRec* __restrict__ rec, const uint32_t* __restrict__ bin_start,
                    const uint32_t* __restrict__ keys, const DevStatus* __restrict__ status,
                    const uint2* __restrict__ split_list, int split_cap,
@@ -549,7 +633,7 @@ k_forward_b1_extra(const GsRec* __restrict__ rec, const uint32_t* __restrict__ b
                    float* __restrict__ out, GridDev gd)
 {
     __shared__ __align__(16) float s_raw[kB1Batch * kB1Words];
-    __shared__ __align__(16) float s_rec[kB1Batch * kB1Words];
+    __shared__ __align__(16) float s_rec[kB1Batch * B1Rec<CH>::kWords];
     if (status->overflow) return;
     const uint32_t nitems = min(status->nsplit, (uint32_t)split_cap);
     for (uint32_t i = blockIdx.x; i < nitems; i += gridDim.x) {
@@ -557,27 +641,29 @@ k_forward_b1_extra(const GsRec* __restrict__ rec, const uint32_t* __restrict__ b
         const uint32_t kbeg = bin_start[item.x * kNumClasses] + item.y * (uint32_t)kSplitKeys;
         const uint32_t kend = min(bin_start[(item.x + 1) * kNumClasses], kbeg + (uint32_t)kSplitKeys);
         __syncwarp();
-        b1_brick<VEC, true>(rec, keys, weight, wstride, c0, out, gd, s_raw, s_rec, (int)item.x, kbeg, kend);
+        b1_brick<CH, VEC, true>(rec, keys, weight, wstride, c0, out, gd, s_raw, s_rec, (int)item.x, kbeg, kend);
     }
 }
 
+template <int CH>
 static int launch_fwd_b1(gsvox_plan* p, const float* weight, int C, int c0, float* out, cudaStream_t st)
 {
+    static_assert(CH == 1 || CH == 3, "b1 staging carries one or three weights");
     LaunchScope ls(p, GSVOX_K_FORWARD, st);
     const bool vec = (p->gd.dims[0] % 4 == 0) && (((uintptr_t)out & 15) == 0);
     const int nblocks = (p->gd.slab1 - p->gd.slab0) * p->gd.nb[0] * p->gd.nb[1];
     if (nblocks <= 0) return GSVOX_OK;
     // deterministic mode: one warp walks its brick's whole key list in the sorted order, no second launch, no atomics
     const uint32_t max_keys = p->deterministic ? 0xffffffffu : (uint32_t)kSplitKeys;
-    if (vec) k_forward_b1<true><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd, max_keys);
-    else     k_forward_b1<false><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd, max_keys);
+    if (vec) k_forward_b1<CH, true><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd, max_keys);
+    else     k_forward_b1<CH, false><<<nblocks, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, weight, C, c0, out, p->gd, max_keys);
     GSVOX_CUDA(cudaGetLastError());
     if (p->deterministic) return GSVOX_OK;
     p->launches[GSVOX_K_FORWARD] += 1;               // the hot-brick launch
-    if (vec) k_forward_b1_extra<true><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
-                                                                 p->split_cap, weight, C, c0, out, p->gd);
-    else     k_forward_b1_extra<false><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
-                                                                  p->split_cap, weight, C, c0, out, p->gd);
+    if (vec) k_forward_b1_extra<CH, true><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
+                                                                     p->split_cap, weight, C, c0, out, p->gd);
+    else     k_forward_b1_extra<CH, false><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
+                                                                      p->split_cap, weight, C, c0, out, p->gd);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }
@@ -606,8 +692,8 @@ int launch_forward(gsvox_plan* p, const float* weight, int channels, float* out,
     while (c0 < channels && rc == GSVOX_OK) {
         int left = channels - c0;
         if (left >= 9)      { rc = launch_fwd_ch<9>(p, weight, channels, c0, out, st); c0 += 9; }
-        else if (left >= 3) { rc = launch_fwd_ch<3>(p, weight, channels, c0, out, st); c0 += 3; }
-        else                { rc = launch_fwd_b1(p, weight, channels, c0, out, st); c0 += 1; }
+        else if (left >= 3) { rc = launch_fwd_b1<3>(p, weight, channels, c0, out, st); c0 += 3; }
+        else                { rc = launch_fwd_b1<1>(p, weight, channels, c0, out, st); c0 += 1; }
     }
     return rc;
 }
