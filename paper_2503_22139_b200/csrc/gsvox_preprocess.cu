@@ -143,8 +143,8 @@ k_preprocess(const float* __restrict__ pos, const float* __restrict__ scale,
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: keys.  Eight lanes cooperate on one Gaussian and stride over the bricks of its box.
-// MODE 0: count keys per brick.  MODE 1: claim a slot per key and write the Gaussian id.
+// a2: keys.  A warp walks the bricks of the boxes of its (up to 32) Gaussians as one flat list (k_keys below).
+// MODE 0: count keys per (brick, class) bin.  MODE 1: claim a slot per key and write the Gaussian id.
 //
 // Negligible keys are dropped (reading A15; SURVEY.md section 7 hard part 7): the axis-aligned box
 // of a thin rotated Gaussian is mostly empty space (config 5's needles: 91 % of all pairs, 0.8 % of
@@ -161,7 +161,7 @@ k_preprocess(const float* __restrict__ pos, const float* __restrict__ scale,
 // The brick test of one flagged Gaussian, in two parts.  cull_setup (once per Gaussian and pass): each principal
 // coordinate t_k of a brick centre is affine in the brick's offset (tx, ty, tz) from the first brick of the box,
 //     c_k = c0_k + tx ax_k + ty ay_k + tz az_k,     and spans +- half_k over the brick;
-// 15 floats, kept in shared memory (one set per 8-lane group).  key_negligible (per brick): 9 FMA + 3 x 4.
+// 15 floats, kept in shared memory (one set per warp).  key_negligible (per brick): 9 FMA + 3 x 4.
 // (Round 1 rebuilt R from the quaternion for every brick: ~70 instructions per test, 2.9e7 tests per pass at config 5.)
 __device__ __forceinline__ void cull_setup(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int g,
                                            float h0, float h1, float h2, int bx0, int by0, int bz0, float* __restrict__ cq)
@@ -201,9 +201,46 @@ __device__ __forceinline__ bool key_negligible(const float* __restrict__ cq, int
     return qmin > kCullQ;
 }
 
+// One WARP takes 32 consecutive Gaussians and walks the keys of all of them as ONE flat list, 32 keys per trip:
+// lane l decodes Gaussian l (box, brick range, key count), the live ones are compacted into a shared-memory table
+// (8 words each) with the exclusive prefix sum of their key counts, and key j of the list belongs to the last
+// entry whose start is <= j.  Per trip that owner is found without a search: the starts that fall inside the
+// trip's window [j0, j0 + 32) are OR-ed into a 32-bit mask (redux.sync), so
+//     owner(lane) = #(starts <= j0) - 1 + popc(mask & bits 1..lane).
+// Every lane then has a key in every trip but the last, whatever the mix of box sizes (round 2's first scheme gave each
+// Gaussian 8 lanes: ncu counted 17 of 32 lanes active and 131 thread instructions per key, the decode replicated
+// eight times; the count pass was issue-bound at 81 %, not atomics-bound).
+constexpr int kKeysThreads = 128;
+constexpr int kKeysWarps = kKeysThreads / 32;
+
+struct KeyOwner {                      // 8 words in shared memory
+    int w_lo, w_mid, w_hi;             // the record's packed int16 box: lox|loy, loz|hix, hiy|hiz
+    int b01;                           // bx0 | by0 << 16 | direct << 31
+    int b2g;                           // bz0 | lane << 16
+    int exy;                           // ex | ey << 16
+    float inv_ex, inv_ey;
+};
+
+// Bin of key t of an owner: (brick, class).  t -> (tx, ty, tz) by reciprocal multiplies with a +-1 fix-up
+// (exact while t < 2^23; larger boxes take the parked route below).
+__device__ __forceinline__ int owner_bin(const KeyOwner& o, int t, const GridDev& gd)
+{
+    const int ex = o.exy & 0xffff, ey = o.exy >> 16;
+    int r = (int)(__int2float_rz(t) * o.inv_ex), tx = t - r * ex;
+    if (tx >= ex) { ++r; tx -= ex; }
+    if (tx < 0) { --r; tx += ex; }
+    int tz = (int)(__int2float_rz(r) * o.inv_ey), ty = r - tz * ey;
+    if (ty >= ey) { ++tz; ty -= ey; }
+    if (ty < 0) { --tz; ty += ey; }
+    const int bx = (o.b01 & 0x7fff) + tx, by = ((o.b01 >> 16) & 0x7fff) + ty, bz = (o.b2g & 0xffff) + tz;
+    const int loy = o.w_lo >> 16, loz = (int16_t)(o.w_mid & 0xffff), hiy = (int16_t)(o.w_hi & 0xffff), hiz = o.w_hi >> 16;
+    const int y0 = max(loy - 8 * by, 0), y1 = min(hiy - 8 * by, 7), z0 = max(loz - 8 * bz, 0), z1 = min(hiz - 8 * bz, 7);
+    return ((bz * gd.nb[1] + by) * gd.nb[0] + bx) * kNumClasses + key_class(o.b01 < 0, 0, 7, y0, y1, z0, z1);
+}
+
 template <int MODE>
-__global__ void __launch_bounds__(256, 6)       // <= 40 registers: the kernel lives on atomics in flight, i.e. on resident warps
-k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, GridDev gd,
+__global__ void __launch_bounds__(kKeysThreads, 10)
+k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, int gw, GridDev gd,
        uint32_t* __restrict__ bin_count, uint32_t* __restrict__ keys, DevStatus* __restrict__ status,
        const uint32_t* __restrict__ bin_start, uint2* __restrict__ split_list, int split_cap)
 {
@@ -221,117 +258,140 @@ k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, Grid
             }
         }
     }
-    __shared__ unsigned long long s_pairs;
-    __shared__ unsigned int s_culled;
-    if (MODE == 0) {
-        if (threadIdx.x == 0) { s_pairs = 0ull; s_culled = 0u; }
-        __syncthreads();
-    }
-    const int g = (blockIdx.x * blockDim.x + threadIdx.x) >> 3;
-    const int sub = threadIdx.x & 7;
-    unsigned int my_pairs = 0u, my_culled = 0u;                // per thread: < 2^32 (<= 4096^3/8 bricks x 512)
-    int total = 0, lox = 0, loy = 0, loz = 0, hix = -1, hiy = -1, hiz = -1, bx0 = 0, by0 = 0, bz0 = 0, ex = 1, ey = 1;
-    bool direct = false, cullable = false;
-    if (g < n) {
+    __shared__ __align__(16) KeyOwner s_own[kKeysWarps][32];
+    __shared__ int s_start[kKeysWarps][32];
+    __shared__ float s_cull[kKeysWarps][16];
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31, wq = threadIdx.x >> 5;
+    const int wbase = (blockIdx.x * kKeysWarps + wq) * gw;      // this warp's gw (a power of two <= 32) Gaussians
+    const int g = wbase + lane;
+    unsigned long long my_pairs = 0ull;
+    unsigned int my_culled = 0u;
+
+    // ---- decode Gaussian `lane`
+    int total = 0;
+    bool park = false;
+    KeyOwner me;
+    me.w_lo = me.w_mid = 0; me.w_hi = -1; me.b01 = 0; me.b2g = lane << 16; me.exy = 1 | (1 << 16); me.inv_ex = me.inv_ey = 1.f;
+    if (lane < gw && g < n) {
         const int4* rp = reinterpret_cast<const int4*>(rec + g);
         const int4 w3 = __ldg(rp + 3);                      // bytes 48..63: nD2, lo[3], hi[3]
-        direct = -__int_as_float(__ldg(rp + 1).w) > kRecurrenceMaxA;      // negA at byte 28
-        lox = (int16_t)(w3.y & 0xffff); loy = (int16_t)(w3.y >> 16);
-        loz = (int16_t)(w3.z & 0xffff); hix = (int16_t)(w3.z >> 16);
-        hiy = (int16_t)(w3.w & 0xffff); hiz = (int16_t)(w3.w >> 16);
+        const bool direct = -__int_as_float(__ldg(rp + 1).w) > kRecurrenceMaxA;      // negA at byte 28
+        const int lox = (int16_t)(w3.y & 0xffff), loy = w3.y >> 16, loz = (int16_t)(w3.z & 0xffff);
+        const int hix = w3.z >> 16, hiy = (int16_t)(w3.w & 0xffff), hiz = w3.w >> 16;
         if (hix >= lox) {
-            bx0 = lox >> 3; by0 = loy >> 3; bz0 = max(loz >> 3, gd.slab0);          // z-slab of this plan only
-            ex = (hix >> 3) - bx0 + 1; ey = (hiy >> 3) - by0 + 1;
+            const int bx0 = lox >> 3, by0 = loy >> 3, bz0 = max(loz >> 3, gd.slab0);          // z-slab of this plan only
+            const int ex = (hix >> 3) - bx0 + 1, ey = (hiy >> 3) - by0 + 1;
             const int ez = min(hiz >> 3, gd.slab1 - 1) - bz0 + 1;
-            total = (ez > 0) ? ex * ey * ez : 0;
+            if (ez > 0) {
+                const int tot = ex * ey * ez;                 // < 2^31: nbricks is an int
+                const bool cullable = (tot > 1) && (__ldg(reinterpret_cast<const int*>(rec + g) + 3) < 0);   // sign bit of cexp
+                park = cullable || tot >= (1 << 23);
+                total = park ? 0 : tot;
+                me.w_lo = w3.y; me.w_mid = w3.z; me.w_hi = w3.w;
+                me.b01 = bx0 | (by0 << 16) | (direct ? (int)0x80000000u : 0);
+                me.b2g = bz0 | (lane << 16);
+                me.exy = ex | (ey << 16);
+                me.inv_ex = __frcp_rn((float)ex); me.inv_ey = __frcp_rn((float)ey);
+                if (MODE == 0 && !park) {                   // every key of an unflagged Gaussian is kept: P_exec = its box (in this slab)
+                    const int zl = max(loz, 8 * gd.slab0), zh = min(hiz, 8 * gd.slab1 - 1);
+                    my_pairs = (unsigned long long)((hix - lox + 1) * (hiy - loy + 1)) * (unsigned long long)(zh - zl + 1);
+                }
+            }
         }
-        cullable = (total > 1) && (__ldg(reinterpret_cast<const int*>(rec + g) + 3) < 0);   // sign bit of cexp
     }
-    // Flagged Gaussians (needles: boxes of hundreds of bricks, most of them culled) are not walked by their own 8
-    // lanes while the other 24 lanes of the warp sit idle behind a 1-trip neighbour: their parameters are parked in
-    // shared memory and, after the ordinary keys, the whole warp walks them one after another, 32 bricks per trip.
-    __shared__ float s_cull[32][16];
-    __shared__ int s_par[32][12];
-    if (cullable && sub == 0) {
-        cull_setup(rec, aux, g, (float)gd.spacing[0], (float)gd.spacing[1], (float)gd.spacing[2], bx0, by0, bz0,
-                   s_cull[threadIdx.x >> 3]);
-        int* sp = s_par[threadIdx.x >> 3];
-        sp[0] = g; sp[1] = total; sp[2] = lox; sp[3] = loy; sp[4] = loz; sp[5] = hix; sp[6] = hiy; sp[7] = hiz;
-        sp[8] = bx0 | (by0 << 16); sp[9] = bz0; sp[10] = ex | (ey << 16); sp[11] = direct ? 1 : 0;
+    // ---- compact the live Gaussians, prefix-sum their key counts
+    const unsigned live_mask = __ballot_sync(full, total > 0);
+    const int nlive = __popc(live_mask);
+    int incl = total;
+    #pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(full, incl, o); if (lane >= o) incl += v; }
+    const int T = __shfl_sync(full, incl, 31);
+    if (total > 0) {
+        const int c = __popc(live_mask & ((1u << lane) - 1u));
+        int4* dst = reinterpret_cast<int4*>(&s_own[wq][c]);
+        dst[0] = make_int4(me.w_lo, me.w_mid, me.w_hi, me.b01);
+        dst[1] = make_int4(me.b2g, me.exy, __float_as_int(me.inv_ex), __float_as_int(me.inv_ey));
+        s_start[wq][c] = incl - total;
     }
-    uint32_t parked = __ballot_sync(0xffffffffu, cullable && sub == 0);
-    if (cullable) total = 0;
+    unsigned parked = __ballot_sync(full, park);
     __syncwarp();
-    // t -> (tx, ty, tz) by reciprocal multiplies with a +-1 fix-up (exact while total < 2^23); the two
-    // integer div/mod pairs were ~half of the 147 thread instructions per key ncu counted in this kernel
-    const float inv_ex = __frcp_rn((float)ex), inv_ey = __frcp_rn((float)ey);
-    const bool small = total < (1 << 23);
-    // bin of key t of this Gaussian, or -1 when the key is culled
-    auto bin_of = [&](int t) -> int {
-        int tx, r, ty, tz;
-        if (small) {
-            r = (int)(__int2float_rz(t) * inv_ex); tx = t - r * ex;
-            if (tx >= ex) { ++r; tx -= ex; }
-            if (tx < 0) { --r; tx += ex; }
-            tz = (int)(__int2float_rz(r) * inv_ey); ty = r - tz * ey;
-            if (ty >= ey) { ++tz; ty -= ey; }
-            if (ty < 0) { --tz; ty += ey; }
-        } else { tx = t % ex; r = t / ex; ty = r % ey; tz = r / ey; }
-        const int bx = bx0 + tx, by = by0 + ty, bz = bz0 + tz;
-        const int x0 = max(lox - 8 * bx, 0), x1 = min(hix - 8 * bx, 7), y0 = max(loy - 8 * by, 0), y1 = min(hiy - 8 * by, 7);
-        const int z0 = max(loz - 8 * bz, 0), z1 = min(hiz - 8 * bz, 7);
-        if (MODE == 0) my_pairs += (unsigned)((x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1));
-        return ((bz * gd.nb[1] + by) * gd.nb[0] + bx) * kNumClasses + key_class(direct, x0, x1, y0, y1, z0, z1);
-    };
-    // two keys per trip: both slot-returning atomics of the scatter pass are in flight before the stores
-    // (the count pass has no returning atomics to wait for and is faster one key at a time: 89 vs 94 us)
-    for (int t = sub; t < total; t += (MODE == 0 ? 8 : 16)) {
-        const int b0 = bin_of(t), b1 = (MODE == 1 && t + 8 < total) ? bin_of(t + 8) : -1;
+    const int start_c = (lane < nlive) ? s_start[wq][lane] : 0x7fffffff;
+    // ---- the flat key list, 32 keys per trip (scatter pass: two trips at once, so that both slot-returning atomics
+    //      of a lane are in flight before the stores)
+    constexpr int kTrips = (MODE == 0) ? 1 : 2;
+    for (int j0 = 0; j0 < T; j0 += 32 * kTrips) {
+        int bin[kTrips], gid[kTrips];
+        #pragma unroll
+        for (int u = 0; u < kTrips; ++u) {
+            const int jb = j0 + 32 * u, j = jb + lane;
+            const unsigned m = __reduce_or_sync(full, (start_c > jb && start_c < jb + 32) ? (1u << (start_c - jb)) : 0u);
+            const int first = __popc(__ballot_sync(full, start_c <= jb)) - 1;
+            bin[u] = -1; gid[u] = 0;
+            if (j < T) {
+                const int owner = first + __popc(m & (0xffffffffu >> (31 - lane)));
+                const int4* src = reinterpret_cast<const int4*>(&s_own[wq][owner]);
+                const int4 a = src[0], b = src[1];
+                KeyOwner o;
+                o.w_lo = a.x; o.w_mid = a.y; o.w_hi = a.z; o.b01 = a.w; o.b2g = b.x; o.exy = b.y;
+                o.inv_ex = __int_as_float(b.z); o.inv_ey = __int_as_float(b.w);
+                bin[u] = owner_bin(o, j - s_start[wq][owner], gd);
+                gid[u] = wbase + (o.b2g >> 16);
+            }
+        }
         if (MODE == 0) {
-            if (b0 >= 0) atomicAdd(&bin_count[b0], 1u);
+            if (bin[0] >= 0) atomicAdd(&bin_count[bin[0]], 1u);
         } else {
-            uint32_t s0 = 0u, s1 = 0u;
-            if (b0 >= 0) s0 = atomicAdd(&bin_count[b0], 1u);
-            if (b1 >= 0) s1 = atomicAdd(&bin_count[b1], 1u);
-            if (b0 >= 0) keys[s0] = (uint32_t)g;
-            if (b1 >= 0) keys[s1] = (uint32_t)g;
+            uint32_t slot[kTrips];
+            #pragma unroll
+            for (int u = 0; u < kTrips; ++u) slot[u] = (bin[u] >= 0) ? atomicAdd(&bin_count[bin[u]], 1u) : 0u;
+            #pragma unroll
+            for (int u = 0; u < kTrips; ++u) if (bin[u] >= 0) keys[slot[u]] = (uint32_t)gid[u];
         }
     }
-    // the parked (flagged) Gaussians of this warp, one after another, 32 bricks per trip
+    // ---- the parked Gaussians of this warp (flagged needles: boxes of hundreds of bricks, most of them culled; and
+    //      boxes of 2^23 bricks or more), one after another, 32 bricks per trip
     while (parked) {                                     // warp-uniform
-        const int grp = (threadIdx.x >> 5) * 4 + ((__ffs(parked) - 1) >> 3);
+        const int pl = __ffs(parked) - 1;
         parked &= parked - 1u;
-        const int* sp = s_par[grp];
-        const float* cq = s_cull[grp];
-        const int pg = sp[0], ptotal = sp[1], pex = sp[10] & 0xffff, pey = sp[10] >> 16;
-        const bool pdirect = sp[11] != 0;
-        for (int t = (int)(threadIdx.x & 31); t < ptotal; t += 32) {
+        const int pg = wbase + pl;
+        const int4* rp = reinterpret_cast<const int4*>(rec + pg);
+        const int4 w3 = __ldg(rp + 3);
+        const bool pdirect = -__int_as_float(__ldg(rp + 1).w) > kRecurrenceMaxA;
+        const bool flagged = __ldg(reinterpret_cast<const int*>(rec + pg) + 3) < 0;
+        const int lox = (int16_t)(w3.y & 0xffff), loy = w3.y >> 16, loz = (int16_t)(w3.z & 0xffff);
+        const int hix = w3.z >> 16, hiy = (int16_t)(w3.w & 0xffff), hiz = w3.w >> 16;
+        const int bx0 = lox >> 3, by0 = loy >> 3, bz0 = max(loz >> 3, gd.slab0);
+        const int pex = (hix >> 3) - bx0 + 1, pey = (hiy >> 3) - by0 + 1;
+        const int ptotal = pex * pey * (min(hiz >> 3, gd.slab1 - 1) - bz0 + 1);      // < 2^31: nbricks is an int
+        if (flagged) {
+            if (lane == 0) cull_setup(rec, aux, pg, (float)gd.spacing[0], (float)gd.spacing[1], (float)gd.spacing[2],
+                                      bx0, by0, bz0, s_cull[wq]);
+            __syncwarp();
+        }
+        const float* cq = s_cull[wq];
+        for (int t = lane; t < ptotal; t += 32) {
             const int tx = t % pex, r = t / pex, ty = r % pey, tz = r / pey;
-            if (key_negligible(cq, tx, ty, tz)) { my_culled += 1u; continue; }
-            const int bx = (sp[8] & 0xffff) + tx, by = (sp[8] >> 16) + ty, bz = sp[9] + tz;
-            const int x0 = max(sp[2] - 8 * bx, 0), x1 = min(sp[5] - 8 * bx, 7), y0 = max(sp[3] - 8 * by, 0), y1 = min(sp[6] - 8 * by, 7);
-            const int z0 = max(sp[4] - 8 * bz, 0), z1 = min(sp[7] - 8 * bz, 7);
-            if (MODE == 0) my_pairs += (unsigned)((x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1));
+            if (flagged && key_negligible(cq, tx, ty, tz)) { my_culled += 1u; continue; }
+            const int bx = bx0 + tx, by = by0 + ty, bz = bz0 + tz;
+            const int x0 = max(lox - 8 * bx, 0), x1 = min(hix - 8 * bx, 7), y0 = max(loy - 8 * by, 0), y1 = min(hiy - 8 * by, 7);
+            const int z0 = max(loz - 8 * bz, 0), z1 = min(hiz - 8 * bz, 7);
+            if (MODE == 0) my_pairs += (unsigned long long)((x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1));
             const int bin = ((bz * gd.nb[1] + by) * gd.nb[0] + bx) * kNumClasses + key_class(pdirect, x0, x1, y0, y1, z0, z1);
             if (MODE == 0) atomicAdd(&bin_count[bin], 1u);
             else keys[atomicAdd(&bin_count[bin], 1u)] = (uint32_t)pg;
         }
+        __syncwarp();                                    // s_cull is rewritten for the next parked Gaussian
     }
     if (MODE == 0) {
-        // P_exec and the culled count: warp -> CTA (shared) -> ONE global atomic pair per CTA
-        unsigned long long wp = my_pairs;
+        // P_exec and the culled count: warp -> ONE global atomic pair per warp that has something to add
         for (int o = 16; o > 0; o >>= 1) {
-            wp += __shfl_xor_sync(0xffffffffu, wp, o);
-            my_culled += __shfl_xor_sync(0xffffffffu, my_culled, o);
+            my_pairs += __shfl_xor_sync(full, my_pairs, o);
+            my_culled += __shfl_xor_sync(full, my_culled, o);
         }
-        if ((threadIdx.x & 31) == 0) {
-            if (wp) atomicAdd(&s_pairs, wp);
-            if (my_culled) atomicAdd(&s_culled, my_culled);
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            if (s_pairs) atomicAdd(&status->pairs_exec, s_pairs);
-            if (s_culled) atomicAdd(&status->culled, (unsigned long long)s_culled);
+        if (lane == 0) {
+            if (my_pairs) atomicAdd(&status->pairs_exec, my_pairs);
+            if (my_culled) atomicAdd(&status->culled, (unsigned long long)my_culled);
         }
     }
 }
@@ -513,10 +573,17 @@ int launch_preprocess(gsvox_plan* p, const float* pos, const float* scale, const
 
 int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
 {
-    int kblocks = (int)((n * 8 + 255) / 256);
+    // Gaussians per warp: 32 when that still leaves >= 8192 warps, fewer otherwise, down to one warp per Gaussian
+    // (measured count + scatter: config 4, 500 k Gaussians x 20 keys, 0.188 / 0.195 / 0.214 / 0.256 ms at 32 / 16 / 8 / 4;
+    //  config 3 level 1, 1000 Gaussians x 1336 keys, 0.91 / 0.25 / 0.138 / 0.065 ms at 32 / 8 / 4 / 1;
+    //  level 3, 64 k x 31 keys, 0.069 / 0.062 / 0.073 at 32 / 4 / 2)
+    int gw = 32;
+    while (gw > 1 && n / gw < 8192) gw >>= 1;
+    const int64_t kwarps = (n + gw - 1) / gw;
+    const int kblocks = (int)((kwarps + kKeysWarps - 1) / kKeysWarps);
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_COUNT, st);
-        k_keys<0><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status,
+        k_keys<0><<<kblocks, kKeysThreads, 0, st>>>(p->rec, p->aux, (int)n, gw, p->gd, p->bin_count, p->keys, p->status,
                                            p->bin_start, p->split_list, p->split_cap);
         GSVOX_CUDA(cudaGetLastError());
     }
@@ -527,7 +594,7 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
       if (rc != GSVOX_OK) return rc; }
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_SCATTER, st);
-        k_keys<1><<<kblocks, 256, 0, st>>>(p->rec, p->aux, (int)n, p->gd, p->bin_count, p->keys, p->status,
+        k_keys<1><<<kblocks, kKeysThreads, 0, st>>>(p->rec, p->aux, (int)n, gw, p->gd, p->bin_count, p->keys, p->status,
                                            p->bin_start, p->split_list, p->split_cap);
         GSVOX_CUDA(cudaGetLastError());
         if (p->deterministic) { int rc = launch_sort_bins(p, st); if (rc != GSVOX_OK) return rc; }

@@ -35,6 +35,9 @@ class Stage3Step:
         self.g_warped, self.g_dvf = f(batch, nz, ny, nx), f(batch, 3, nz, ny, nx)
         self.g_iref, self.g_e = f(1, nz, ny, nx), f(self.L, 3, nz, ny, nx)
         self.g_coef = f(batch, self.L, 3)
+        # parameter gradients, allocated once: (d feat | d rho, d pos, d scale, d quat) per plan
+        gset = lambda n, c: (f(n, c), f(n, 3), f(n, 3), f(n, 4))
+        self.g_ref, self.g_levels = gset(n_ref, 1), [gset(n, 3) for n in n_levels]
         self.scratch = B_._project_scratch(B_.make_grid(*grid), batch, dev)
         self._saved = None
         # the four voxelizers are independent: each runs on its own stream so that the small binning kernels of one
@@ -85,18 +88,16 @@ class Stage3Step:
 
     def backward(self, grad_drr):
         """dL/dDRR [B,nv,nu] -> dict(ref=(d rho, d pos, d scale, d quat), levels=[(d feat, d pos, d scale, d quat)],
-        coef=dL/dcoef [B,L,3]).  Must follow forward() of the same step."""
+        coef=dL/dcoef [B,L,3]), buffers owned by this object (overwritten by the next call).  Must follow forward() of
+        the same step."""
         ref, levels, coef, angles = self._saved
         B_.project_backward(grad_drr, self.grid, self.geom, angles, out=self.g_warped, scratch=self.scratch)
         B_.warp_backward(self.iref[0], self.dvf, self.grid, self.g_warped, grads=(self.g_iref[0], self.g_dvf))
         B_.mbc_combine_backward(self.e, coef, self.g_dvf, grads=(self.g_e, self.g_coef))
         main = self._fork()
-        g_levels = []
         for i, lv in enumerate(levels):
             with torch.cuda.stream(self._side[i]):
-                g_levels.append(self.plans[i].backward(lv[3], self.g_e[i]))
-                for t in g_levels[-1]:
-                    t.record_stream(main)          # allocated on the side stream, consumed on the caller's
-        g_ref = self.plan_ref.backward(ref[3], self.g_iref)
+                self.plans[i].backward(lv[3], self.g_e[i], grads=self.g_levels[i])
+        self.plan_ref.backward(ref[3], self.g_iref, grads=self.g_ref)
         self._join(main)
-        return {"ref": g_ref, "levels": g_levels, "coef": self.g_coef}
+        return {"ref": self.g_ref, "levels": self.g_levels, "coef": self.g_coef}
