@@ -217,6 +217,22 @@ def test_far_grid_coordinates_keep_accuracy(pkg):
     full_parity(pkg, case)
 
 
+def test_longest_axis_the_boundary_allows(pkg):
+    """GSVOX_MAX_DIM = 32760 voxels along one axis (the record packs box corners as int16, bricks 4095 wide): Gaussians at
+    both ends and one 2000-voxel-long needle along the axis; one voxel more is refused."""
+    for axis in range(3):
+        dims = [9, 11, 10]; dims[axis] = 32760
+        case = gsvox_inputs.config1(n=240, dims=tuple(dims), seed=60 + axis)
+        case.pos[:80, axis] = np.linspace(32700.0, 32761.5, 80, dtype=np.float32)       # the far end, some beyond it
+        case.pos[80:120, axis] = np.linspace(-1.5, 40.0, 40, dtype=np.float32)
+        case.scale[200] = 1.0; case.scale[200, axis] = 333.0; case.quat[200] = (1, 0, 0, 0)
+        case.pos[200, axis] = 20000.3
+        full_parity(pkg, case)
+    bad = ((0.0, 0.0, 0.0), (1.0, 1.0, 1.0), (32761, 8, 8))
+    with pytest.raises(pkg.GsvoxError):
+        pkg.Plan(10, bad, max_channels=1)
+
+
 # --------------------------------------------------------------------------- edge cases
 def test_degenerate_empty_and_outside(pkg):
     case = gsvox_inputs.config1(n=64, dims=(24, 20, 18), seed=3)
