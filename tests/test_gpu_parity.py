@@ -146,9 +146,10 @@ def test_subvolume_anisotropic_spacing_three_channels(pkg):
     full_parity(pkg, gsvox_inputs.subvolume_case())
 
 
-@pytest.mark.parametrize("channels", [2, 4, 5, 9, 13])
+@pytest.mark.parametrize("channels", [2, 4, 5, 9, 13, 96])
 def test_channel_counts(pkg, channels):
-    full_parity(pkg, gsvox_inputs.subvolume_case(n=300, channels=channels, seed=20 + channels))
+    """Channel groups of 9, 3 and 1 in every mix up to GSVOX_MAX_CHANNELS = 96 (ten groups of 9 and two of 3)."""
+    full_parity(pkg, gsvox_inputs.subvolume_case(n=300 if channels < 96 else 120, channels=channels, seed=20 + channels))
 
 
 @pytest.mark.parametrize("level,n", [(1, 60), (2, 400), (3, 3000)])
