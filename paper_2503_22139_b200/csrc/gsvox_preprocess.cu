@@ -397,7 +397,8 @@ k_keys(const GsRec* __restrict__ rec, const GsAux* __restrict__ aux, int n, int 
 }
 
 // ------------------------------------------------------------------------------------------
-// Exclusive scan over the nbins counters, three launches (reduce, scan of partials, apply).
+// Exclusive scan over the nbins counters: reduce, then apply (each tile sums the tile totals before it); beyond
+// kScanFusedTiles tiles a single-block scan of the tile totals runs in between.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_scan_reduce(const uint32_t* __restrict__ cnt, int nbins, uint32_t* __restrict__ partial)
@@ -444,12 +445,31 @@ k_scan_partials(uint32_t* __restrict__ partial, int nblocks, unsigned long long*
     }
 }
 
+// SUMMED = false: partial[] already holds the exclusive prefix of the tile sums (k_scan_partials ran).
+// SUMMED = true: partial[] holds the tile sums themselves and every CTA adds up the ones before it (two launches
+// instead of three; quadratic in the tile count, so only for up to kScanFusedTiles tiles); the last CTA reports the total.
+constexpr int kScanFusedTiles = 4096;
+template <bool SUMMED>
 __global__ void __launch_bounds__(256)
 k_scan_apply(uint32_t* __restrict__ cnt, int nbins, const uint32_t* __restrict__ partial,
-             uint32_t* __restrict__ start)
+             uint32_t* __restrict__ start, unsigned long long* __restrict__ keys_needed,
+             unsigned int* __restrict__ overflow, unsigned long long key_capacity)
 {
     // 256 threads x 8 consecutive items; counts are replaced by write cursors (= start)
     __shared__ uint32_t sh[8];
+    __shared__ unsigned long long sh_off[8];
+    unsigned long long tile_off = 0ull;
+    if (SUMMED) {
+        unsigned long long a = 0ull;
+        for (int k = threadIdx.x; k < (int)blockIdx.x; k += 256) a += partial[k];
+        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+        if ((threadIdx.x & 31) == 0) sh_off[threadIdx.x >> 5] = a;
+        __syncthreads();
+        #pragma unroll
+        for (int k = 0; k < 8; ++k) tile_off += sh_off[k];
+    } else {
+        tile_off = partial[blockIdx.x];
+    }
     int base = blockIdx.x * kScanItemsPerBlock + threadIdx.x * 8;
     uint32_t v[8]; uint32_t s = 0;
     #pragma unroll
@@ -461,14 +481,23 @@ k_scan_apply(uint32_t* __restrict__ cnt, int nbins, const uint32_t* __restrict__
     __syncthreads();
     uint32_t woff = 0;
     for (int k = 0; k < w; ++k) woff += sh[k];
-    uint32_t run = partial[blockIdx.x] + woff + inc - s;
+    uint32_t run = (uint32_t)tile_off + woff + inc - s;       // 32-bit cursors: a total beyond 2^32 - 16 is an overflow
     #pragma unroll
     for (int k = 0; k < 8; ++k) {
         if (base + k < nbins) { start[base + k] = run; cnt[base + k] = run; }
         run += v[k];
     }
     // sentinel start[nbins] = total
-    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 255) start[nbins] = run;
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 255) {
+        start[nbins] = run;
+        if (SUMMED) {
+            uint32_t mine = 0;
+            for (int k = 0; k < 8; ++k) mine += sh[k];
+            const unsigned long long total = tile_off + mine;
+            *keys_needed = total;
+            *overflow = (total > key_capacity || total > 0xfffffff0ull) ? 1u : 0u;
+        }
+    }
 }
 
 // cnt[nbins] -> start[nbins + 1] (exclusive scan, start[nbins] = total); cnt is overwritten by the same
@@ -480,8 +509,12 @@ int launch_exclusive_scan(uint32_t* cnt, int nbins, uint32_t* partial, uint32_t*
 {
     const int sblocks = (nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock;
     k_scan_reduce<<<sblocks, 256, 0, st>>>(cnt, nbins, partial);
-    k_scan_partials<<<1, 1024, 0, st>>>(partial, sblocks, keys_needed, overflow, key_capacity);
-    k_scan_apply<<<sblocks, 256, 0, st>>>(cnt, nbins, partial, start);
+    if (sblocks <= kScanFusedTiles) {
+        k_scan_apply<true><<<sblocks, 256, 0, st>>>(cnt, nbins, partial, start, keys_needed, overflow, key_capacity);
+    } else {
+        k_scan_partials<<<1, 1024, 0, st>>>(partial, sblocks, keys_needed, overflow, key_capacity);
+        k_scan_apply<false><<<sblocks, 256, 0, st>>>(cnt, nbins, partial, start, keys_needed, overflow, key_capacity);
+    }
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
 }
@@ -590,7 +623,7 @@ int launch_binning(gsvox_plan* p, int64_t n, cudaStream_t st)
     { LaunchScope ls(p, GSVOX_K_SCAN, st);
       int rc = launch_exclusive_scan(p->bin_count, p->nbins, p->scan_partial, p->bin_start, &p->status->keys_needed,
                                      &p->status->overflow, (unsigned long long)p->key_capacity, st);
-      p->launches[GSVOX_K_SCAN] += 2;                       // the scan is three kernels
+      p->launches[GSVOX_K_SCAN] += ((p->nbins + kScanItemsPerBlock - 1) / kScanItemsPerBlock <= kScanFusedTiles) ? 1 : 2;   // two or three kernels
       if (rc != GSVOX_OK) return rc; }
     if (n > 0) {
         LaunchScope ls(p, GSVOX_K_SCATTER, st);
