@@ -25,6 +25,7 @@ constexpr int kBwdThreads = 128;
 // A CTA of the first launch takes up to 4 segments of kSplitKeys keys (16 keys per thread); dense-but-even fields
 // (config 3: ~1000 keys in every brick) then run as one launch, only truly hot bricks spill into the second.
 constexpr int kBwdMainSegments = 4;
+constexpr int kZSwizzleCH = 9;           // channel groups this wide also swizzle the gradient tile by the slice z (backward_brick)
 
 __device__ __forceinline__ float ex2b(float x)
 {
@@ -71,7 +72,8 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
         #pragma unroll
         for (int k = 0; k < 8; ++k) km[k] = (!DIRECT && (kg.xm & (1u << k))) ? kk[k] : 0.f;
     }
-    uint32_t gaddr = sbase + ((((kg.z0 << 3) + kg.y0) << 3) << 2);     // byte address of the row in the tile
+    // byte address of the row in the tile (CH = 9: its offset inside the tile, the z swizzle below works on that)
+    uint32_t gaddr = (CH >= kZSwizzleCH ? 0u : sbase) + ((((kg.z0 << 3) + kg.y0) << 3) << 2);
     const uint32_t wrapstep = (uint32_t)(9 - kg.ny) << 5;              // last y of a slice -> y0 of the next
     int yc = kg.ny;
     for (int r = kg.nrows; r > 0; --r) {
@@ -108,7 +110,9 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
             #pragma unroll
             for (int k = 0; k < 8; ++k) av[k] = 0.f;
             // rows with y >= 4 hold their halves swapped when CH > 1 (stage loop); a lone channel of a wider C keeps the plain layout
-            const uint32_t ga0 = (CH > 1) ? (gaddr ^ ((gaddr >> 3) & 16u)) : gaddr, ga1 = ga0 ^ 16u;
+            // (bits 8..10 of the offset inside the tile are the slice z)
+            const uint32_t ga0 = (CH >= kZSwizzleCH) ? (sbase + (gaddr ^ ((gaddr >> 3) & 16u) ^ ((gaddr >> 4) & 0x70u)))
+                               : ((CH > 1) ? (gaddr ^ ((gaddr >> 3) & 16u)) : gaddr), ga1 = ga0 ^ 16u;
             #pragma unroll
             for (int ch = 0; ch < CH; ++ch) {
                 const float4 g0 = lds_v4(ga0 + ch * kBrickVox * 4), g1 = lds_v4(ga1 + ch * kBrickVox * 4);
@@ -175,7 +179,12 @@ __device__ __forceinline__ void backward_brick(const GsRec* __restrict__ rec, co
             // eight different bank groups, not four (thread-per-key LDS.128 of different rows: ncu counted 48 % of the
             // shared-memory wavefronts of k_backward<9> as bank conflicts, on a kernel whose l1tex pipe was 95 % busy)
             // (C = 1 keeps the plain layout: it is issue-bound, and the two extra address instructions per row cost it 4 %)
-            s_g[CH > 1 ? ((e & ~7) | ((x & 4) ^ (y & 4)) | (x & 3)) : e] = val;
+            // and to chunk ^ z: rows of equal y in different slices (keys of full y extent whose boxes start at different z
+            // walk in step) no longer share a bank group either
+            // (CH = 9 only: levels of full-brick keys pay 2 % for the extra address arithmetic, config 3 level 3 gains 11 %;
+            //  C = 3 is issue-bound and loses 1.5 % with it)
+            s_g[CH >= kZSwizzleCH ? ((e & ~63) | (((((y << 1) | (x >> 2)) ^ ((y >> 2) & 1) ^ z) & 15) << 2) | (x & 3))
+                                  : (CH > 1 ? ((e & ~7) | ((x & 4) ^ (y & 4)) | (x & 3)) : e)] = val;
         }
     }
     __syncthreads();
