@@ -270,6 +270,19 @@ int gsvox_project_scratch_bytes(const gsvox_grid* grid, int32_t B, size_t* bytes
 int gsvox_project_forward(const float* vol, int64_t vol_stride, const gsvox_grid* grid,
                           const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
                           void* scratch, float* drr, void* stream);
+/* The same forward projection for callers that cannot allocate device memory (code under CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc): no scratch argument, the y-fastest copy of the volumes lives
+ * in a 16 MB array built into the library (every GPU that loads the library holds it until the process exits).
+ * Limit: B * nx * ny * nz <= GSVOX_PROJECT_STATIC_MAX_VOXELS (one 200x200x100 volume; four of
+ * 128x128x64), else GSVOX_ELIMIT and nothing is enqueued.  Calls no cudaMalloc / cudaFree / allocating routine;
+ * the first call on a device looks the array's address up (cudaGetSymbolAddress), so make that call outside a
+ * capture.  All calls on one device SHARE the array: calls that overlap on the GPU (different streams, parallel
+ * graph branches) race on it; calls ordered on one stream do not.  Everything else as gsvox_project_forward,
+ * whose results it reproduces bit for bit.                                                                 */
+#define GSVOX_PROJECT_STATIC_MAX_VOXELS 4194304
+int gsvox_project_forward_static(const float* vol, int64_t vol_stride, const gsvox_grid* grid,
+                                 const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                                 float* drr, void* stream);
 /* Exact transpose: grad_vol[b] = P_b^T grad_drr[b], grad_vol [B,nz,ny,nx] OVERWRITTEN (fp32 atomics). */
 int gsvox_project_backward(const float* grad_drr, const gsvox_grid* grid, const gsvox_cone_geometry* geom,
                            const float* angles_host, int32_t B, void* scratch, float* grad_vol, void* stream);

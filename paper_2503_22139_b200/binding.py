@@ -22,7 +22,7 @@ EXPORTS = [
     "gsvox_last_cuda_error", "gsvox_version", "gsvox_dvf_forward", "gsvox_dvf_backward",
     "gsvox_mbc_combine_forward", "gsvox_mbc_combine_backward", "gsvox_warp_forward", "gsvox_warp_backward",
     "gsvox_plan_set_slab", "gsvox_backward_accumulate", "gsvox_backward_finish", "gsvox_plan_accumulators",
-    "gsvox_project_scratch_bytes", "gsvox_project_forward", "gsvox_project_backward",
+    "gsvox_project_scratch_bytes", "gsvox_project_forward", "gsvox_project_backward", "gsvox_project_forward_static",
     "gsvox_splat_workspace_bytes", "gsvox_splat_forward", "gsvox_splat_backward", "gsvox_splat_status",
     "gsvox_splat_drops", "gsvox_plan_set_deterministic", "gsvox_plan_unsorted_bins",
 ]
@@ -92,6 +92,7 @@ def lib():
     cgp = C.POINTER(GsvoxConeGeometry)
     L.gsvox_project_scratch_bytes.argtypes = [gp, i32, szp]
     L.gsvox_project_forward.argtypes = [vp, i64, gp, cgp, vp, i32, vp, vp, vp]
+    L.gsvox_project_forward_static.argtypes = [vp, i64, gp, cgp, vp, i32, vp, vp]
     L.gsvox_project_backward.argtypes = [vp, gp, cgp, vp, i32, vp, vp, vp]
     L.gsvox_splat_workspace_bytes.argtypes = [i64, cgp, i32, i64, szp]
     L.gsvox_splat_forward.argtypes = [vp, vp, vp, vp, i64, cgp, vp, i32, vp, C.c_size_t, i64, vp, vp]
@@ -263,6 +264,28 @@ def project_forward(vol, grid, geom, angles, out=None, scratch=None):
     _check(lib().gsvox_project_forward(_dev(vol, "vol", vshape if shared else (B,) + vshape), 0 if shared else V,
                                        C.byref(g), C.byref(cg), ang, B, _dev(scratch, "scratch"),
                                        _dev(out, "drr", (B, cg.nv, cg.nu)), _stream()))
+    return out
+
+
+PROJECT_STATIC_MAX_VOXELS = 4194304          # GSVOX_PROJECT_STATIC_MAX_VOXELS (include/gsvox.h)
+
+
+def project_forward_static(vol, grid, geom, angles, out):
+    """project_forward for callers that cannot allocate device memory: `out` [B,nv,nu] is required, the scratch is a
+    16 MB array built into libgsvox.so (B * voxels <= PROJECT_STATIC_MAX_VOXELS; shared by all calls on a device, so
+    calls that overlap on the GPU race).  Allocates nothing on the device."""
+    g, cg = make_grid(*grid), make_cone_geometry(geom)
+    ang = (C.c_float * len(angles))(*[float(a) for a in angles])
+    B = len(angles)
+    shared = vol.dim() == 3
+    vshape = (g.dims[2], g.dims[1], g.dims[0])
+    V = vshape[0] * vshape[1] * vshape[2]
+    if V * B > PROJECT_STATIC_MAX_VOXELS:
+        raise GsvoxError("project_forward_static: %d volumes of %d voxels exceed the built-in scratch of %d voxels; "
+                         "use project_forward with caller-owned scratch" % (B, V, PROJECT_STATIC_MAX_VOXELS))
+    _check(lib().gsvox_project_forward_static(_dev(vol, "vol", vshape if shared else (B,) + vshape), 0 if shared else V,
+                                              C.byref(g), C.byref(cg), ang, B,
+                                              _dev(out, "drr", (B, cg.nv, cg.nu)), _stream()))
     return out
 
 

@@ -18,6 +18,7 @@
 // sampling must be exact and hardware filtering has 8-bit weights.  L1/L2-bound gather: per sample 4
 // loads, algorithmic HBM bytes = 4V per volume + 4 per DRR pixel.
 #include <cmath>
+#include <mutex>
 #include "gsvox_internal.cuh"
 
 namespace gsvox {
@@ -369,4 +370,60 @@ extern "C" int gsvox_project_backward(const float* grad_drr, const gsvox_grid* g
     GSVOX_CUDA(cudaGetLastError());
     // fold the y-fastest scratch back: grad_vol[z][y][x] += scratch[z][x][y]  (a transpose with nx, ny swapped)
     return launch_transpose<true>((const float*)scratch, V, P.n[1], P.n[0], P.n[2], B, grad_vol, st);
+}
+
+// ------------------------------------------------------------------------------------------
+// gsvox_project_forward_static: the forward projector for callers that cannot allocate device memory (code under
+// CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  Same kernels as gsvox_project_forward; the
+// y-fastest copy of the volumes lives in the file-scope array below instead of caller-owned scratch:
+// GSVOX_PROJECT_STATIC_MAX_VOXELS floats = 16 MB, held by every GPU that loads the library until the process exits.
+// The array's name is a host-side stand-in in host code, NOT a device address: its device address is looked up once
+// per device (with that device current) by cudaGetSymbolAddress and cached here.  This entry point calls no
+// cudaMalloc / cudaFree / allocating library routine.  All calls on one device share the array: it keeps the last
+// call's contents (every call overwrites the B * V floats it reads, nothing has to start at zero), and two calls
+// that overlap on the GPU (different streams, or graph branches) race on it.
+// ------------------------------------------------------------------------------------------
+static __device__ __align__(256) float g_project_static_scratch[GSVOX_PROJECT_STATIC_MAX_VOXELS];
+
+constexpr int kProjStaticMaxDevices = 64;
+static float* g_project_static_addr[kProjStaticMaxDevices];     // [device] -> device address of the array, 0 = not looked up yet
+static std::mutex g_project_static_mu;
+
+static int project_static_scratch(float** ptr)
+{
+    int dev = -1;
+    GSVOX_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kProjStaticMaxDevices) return GSVOX_ELIMIT;
+    std::lock_guard<std::mutex> lk(g_project_static_mu);
+    if (!g_project_static_addr[dev]) {
+        float* p = nullptr;
+        GSVOX_CUDA(cudaGetSymbolAddress((void**)&p, g_project_static_scratch));
+        if (!p) return GSVOX_ECUDA;
+        g_project_static_addr[dev] = p;
+    }
+    *ptr = g_project_static_addr[dev];
+    return GSVOX_OK;
+}
+
+extern "C" int gsvox_project_forward_static(const float* vol, int64_t vol_stride, const gsvox_grid* grid,
+                                            const gsvox_cone_geometry* geom, const float* angles_host, int32_t B,
+                                            float* drr, void* stream)
+{
+    ProjParams P;
+    int rc = fill_params(grid, geom, angles_host, B, &P);
+    if (rc != GSVOX_OK) return rc;
+    const long long V = (long long)P.n[0] * P.n[1] * P.n[2];
+    if (!vol || !drr || (vol_stride != 0 && vol_stride != V)) return GSVOX_EINVAL;
+    if (V * B > (long long)GSVOX_PROJECT_STATIC_MAX_VOXELS) return GSVOX_ELIMIT;      // beyond the built-in scratch
+    float* scratch = nullptr;
+    rc = project_static_scratch(&scratch);
+    if (rc != GSVOX_OK) return rc;
+    P.vol_stride = vol_stride;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = launch_transpose<false>(vol, vol_stride, P.n[0], P.n[1], P.n[2], B, scratch, st);
+    if (rc != GSVOX_OK) return rc;
+    dim3 pg((P.nu + kProjThreads - 1) / kProjThreads, (unsigned)P.nv, (unsigned)B);
+    k_project_forward<<<pg, kProjThreads, 0, st>>>(vol, (const float*)scratch, P, drr);
+    GSVOX_CUDA(cudaGetLastError());
+    return GSVOX_OK;
 }
