@@ -107,12 +107,32 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
             av[0] = g0.x * G[0]; av[1] = g0.y * G[1]; av[2] = g0.z * G[2]; av[3] = g0.w * G[3];
             av[4] = g1.x * G[4]; av[5] = g1.y * G[5]; av[6] = g1.z * G[6]; av[7] = g1.w * G[7];
         } else {
-            #pragma unroll
-            for (int k = 0; k < 8; ++k) av[k] = 0.f;
             // rows with y >= 4 hold their halves swapped when CH > 1 (stage loop); a lone channel of a wider C keeps the plain layout
             // (bits 8..10 of the offset inside the tile are the slice z)
             const uint32_t ga0 = (CH >= kZSwizzleCH) ? (sbase + (gaddr ^ ((gaddr >> 3) & 16u) ^ ((gaddr >> 4) & 0x70u)))
                                : ((CH > 1) ? (gaddr ^ ((gaddr >> 3) & 16u)) : gaddr), ga1 = ga0 ^ 16u;
+            if (CH == 3) {
+                // packed pairs of neighbouring voxels: 8 FFMA2 + 2 per channel instead of 16 FFMA (a4 at C = 3 is issue-bound)
+                const f32x2 G2[4] = { pk2(G[0], G[1]), pk2(G[2], G[3]), pk2(G[4], G[5]), pk2(G[6], G[7]) };
+                f32x2 a2[4];
+                #pragma unroll
+                for (int ch = 0; ch < CH; ++ch) {
+                    const float4 g0 = lds_v4(ga0 + ch * kBrickVox * 4), g1 = lds_v4(ga1 + ch * kBrickVox * 4);
+                    const f32x2 gp[4] = { pk2(g0.x, g0.y), pk2(g0.z, g0.w), pk2(g1.x, g1.y), pk2(g1.z, g1.w) };
+                    const f32x2 w2 = pk2(wv[ch], wv[ch]);
+                    f32x2 d2 = mul2(gp[0], G2[0]);
+                    #pragma unroll
+                    for (int j = 1; j < 4; ++j) d2 = fma2(gp[j], G2[j], d2);
+                    #pragma unroll
+                    for (int j = 0; j < 4; ++j) a2[j] = (ch == 0) ? mul2(gp[j], w2) : fma2(gp[j], w2, a2[j]);
+                    float dl, dh; upk2(d2, dl, dh);
+                    dw[ch] += dl + dh;
+                }
+                #pragma unroll
+                for (int j = 0; j < 4; ++j) { a2[j] = mul2(a2[j], G2[j]); upk2(a2[j], av[2 * j], av[2 * j + 1]); }
+            } else {
+            #pragma unroll
+            for (int k = 0; k < 8; ++k) av[k] = 0.f;
             #pragma unroll
             for (int ch = 0; ch < CH; ++ch) {
                 const float4 g0 = lds_v4(ga0 + ch * kBrickVox * 4), g1 = lds_v4(ga1 + ch * kBrickVox * 4);
@@ -124,6 +144,7 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
             }
             #pragma unroll
             for (int k = 0; k < 8; ++k) av[k] *= G[k];
+            }
         }
         // x-moments about xs
         float U0, U1, U2;
