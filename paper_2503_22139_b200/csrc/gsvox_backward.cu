@@ -111,8 +111,8 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
             // (bits 8..10 of the offset inside the tile are the slice z)
             const uint32_t ga0 = (CH >= kZSwizzleCH) ? (sbase + (gaddr ^ ((gaddr >> 3) & 16u) ^ ((gaddr >> 4) & 0x70u)))
                                : ((CH > 1) ? (gaddr ^ ((gaddr >> 3) & 16u)) : gaddr), ga1 = ga0 ^ 16u;
-            if (CH == 3) {
-                // packed pairs of neighbouring voxels: 8 FFMA2 + 2 per channel instead of 16 FFMA (a4 at C = 3 is issue-bound)
+            if (CH >= 3) {
+                // packed pairs of neighbouring voxels: 8 FFMA2 + 2 per channel instead of 16 FFMA (a4 at C = 3 is issue-bound; C = 9 gains 3 % on full-brick keys)
                 const f32x2 G2[4] = { pk2(G[0], G[1]), pk2(G[2], G[3]), pk2(G[4], G[5]), pk2(G[6], G[7]) };
                 f32x2 a2[4];
                 #pragma unroll
