@@ -4,7 +4,7 @@
 //     steps 1-5 (Eq. 4; Sigma = R S S^T R^T per north_star).  The box bounds use
 //     the operation order of reading A5 with explicitly rounded intrinsics (__dmul_rn, ...),
 //     so no FMA contraction can change an integer bound.
-// a2  counting sort of (brick, Gaussian) keys by (brick, class): k_keys<0> -> 3-kernel exclusive
+// a2  counting sort of (brick, Gaussian) keys by (brick, class): k_keys<0> -> exclusive
 //     scan -> k_keys<1>.  Order inside a brick is whatever the atomics produce (sums are order
 //     independent within tolerance, reading A13).
 #include "gsvox_internal.cuh"
