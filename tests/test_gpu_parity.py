@@ -412,3 +412,36 @@ def test_cuda_graph_replay_matches_eager_and_follows_new_inputs(pkg):
     check_forward(out.cpu().numpy(), ref2)
     refs2 = oracle.backward(pos2, case.scale, case.quat, case.weight, case.grid, case.grad_out())
     check_grads([t.cpu().numpy() for t in grads], refs2)
+
+
+def test_box_of_2_to_the_23_bricks_takes_the_whole_warp_route(pkg):
+    """a2 walks the keys of ordinary Gaussians as a flat list whose brick index arithmetic (reciprocal multiplies) is
+    exact below 2^23 keys per Gaussian; a box of 2^23 bricks or more is parked and walked by the whole warp with true
+    division instead (gsvox_preprocess.cu, k_keys).  2048 x 2048 x 1024 voxels = 256 x 256 x 128 bricks = 2^23: one
+    Gaussian that covers the whole grid must appear exactly once in every brick, next to two ordinary ones.  Binning only:
+    a volume of 4.3e9 voxels is not voxelized here."""
+    dims = (2048, 2048, 1024)
+    grid = ((0.0, 0.0, 0.0), (1.0, 1.0, 1.0), dims)
+    pos = np.array([[1000.0, 1100.0, 500.0], [20.5, 30.25, 40.0], [2040.0, 2040.0, 1020.0]], np.float32)
+    scale = np.array([[900.0, 900.0, 900.0], [3.0, 2.0, 4.0], [2.5, 2.5, 2.5]], np.float32)
+    quat = np.array([[1, 0, 0, 0], [0.9, 0.1, -0.3, 0.2], [1, 0, 0, 0]], np.float32)
+    geo = oracle.geometry(pos, scale, quat, grid)
+    b = geo["box"].astype(np.int64)
+    assert b[0].tolist() == [0, 0, 0, 2047, 2047, 1023]
+    nbk = ((b[:, 3:] >> 3) - (b[:, :3] >> 3) + 1).prod(1)
+    assert nbk[0] == 1 << 23
+    plan = pkg.Plan(3, grid, max_channels=1, key_capacity=int(nbk.sum()) + 16)
+    plan.preprocess(dev(pos), dev(scale), dev(quat))
+    st = plan.status()
+    assert not st["overflow"] and st["culled_keys"] == 0
+    assert st["keys_needed"] == int(nbk.sum())
+    assert st["pairs"] == st["pairs_exec"] == int((b[:, 3:] - b[:, :3] + 1).prod(1).sum())
+    start, keys = plan.bins()
+    per_brick = np.diff(start)
+    assert per_brick.min() == 1 and per_brick.sum() == int(nbk.sum())
+    brick_of_key = np.repeat(np.arange(len(per_brick)), per_brick)
+    assert np.array_equal(np.sort(brick_of_key[keys == 0]), np.arange(1 << 23))          # Gaussian 0: once in every brick
+    for g in (1, 2):
+        exp = sorted((bz * 256 + by) * 256 + bx for bz in range(b[g, 2] >> 3, (b[g, 5] >> 3) + 1)
+                     for by in range(b[g, 1] >> 3, (b[g, 4] >> 3) + 1) for bx in range(b[g, 0] >> 3, (b[g, 3] >> 3) + 1))
+        assert sorted(brick_of_key[keys == g].tolist()) == exp
