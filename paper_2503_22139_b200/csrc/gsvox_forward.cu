@@ -660,9 +660,11 @@ static int launch_fwd_b1(gsvox_plan* p, const float* weight, int C, int c0, floa
     GSVOX_CUDA(cudaGetLastError());
     if (p->deterministic) return GSVOX_OK;
     p->launches[GSVOX_K_FORWARD] += 1;               // the hot-brick launch
-    if (vec) k_forward_b1_extra<CH, true><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
+    // single-warp CTAs: 32 resident per SM at C = 1 (64 registers), 16 at C = 3
+    constexpr int xgrid = (CH == 1) ? 2 * kSplitGrid : kSplitGrid;
+    if (vec) k_forward_b1_extra<CH, true><<<xgrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
                                                                      p->split_cap, weight, C, c0, out, p->gd);
-    else     k_forward_b1_extra<CH, false><<<kSplitGrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
+    else     k_forward_b1_extra<CH, false><<<xgrid, 32, 0, st>>>(p->rec, p->bin_start, p->keys, p->status, p->split_list,
                                                                       p->split_cap, weight, C, c0, out, p->gd);
     GSVOX_CUDA(cudaGetLastError());
     return GSVOX_OK;
