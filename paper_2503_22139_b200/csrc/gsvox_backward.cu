@@ -57,9 +57,12 @@ struct KeyGeom {
 
 struct Moments { float b0, bu0, bu1, bu2, b00, b01, b02, b11, b12, b22; };
 
-// Walk the rows of one key.  DIRECT: one EX2 per voxel (narrow Gaussians, class 0).  sbase is the
-// shared-window byte address of the gradient tile.
-template <int CH, bool SINGLE, bool DIRECT>
+// Walk the rows of one key.  MODE 0: the warp's keys all take the geometric chain; 1: all take one EX2 per voxel (narrow
+// Gaussians, class 0); 2: both kinds in this warp — ONE row loop, the lanes part only for the eight G values.  (Two loops
+// one after the other cost the warp rows_direct x 100 + rows_chain x 85 instructions; config 5's needle-only bricks hold
+// 17..64 keys, 5 % of them direct, so nearly every warp there paid both: ncu counted 15.5 of 32 lanes active.)
+// sbase is the shared-window byte address of the gradient tile.
+template <int CH, bool SINGLE, int MODE>
 __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, const float (&wv)[CH],
                                           Moments& m, float (&dw)[CH])
 {
@@ -70,7 +73,8 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
         const float c1 = kg.cc, c3 = c1 * c1 * c1, c6 = c3 * c3;
         const float kk[8] = { c6, c3, c1, 1.f, 1.f, c1, c3, c6 };
         #pragma unroll
-        for (int k = 0; k < 8; ++k) km[k] = (!DIRECT && (kg.xm & (1u << k))) ? kk[k] : 0.f;
+        for (int k = 0; k < 8; ++k)
+            km[k] = (MODE != 1 && (kg.xm & (1u << k))) ? ((MODE == 2 && kg.direct) ? 1.f : kk[k]) : 0.f;
     }
     // byte address of the row in the tile (CH = 9: its offset inside the tile, the z swizzle below works on that)
     uint32_t gaddr = (CH >= kZSwizzleCH ? 0u : sbase) + ((((kg.z0 << 3) + kg.y0) << 3) << 2);
@@ -81,7 +85,7 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
         const float xs = fmaf(kg.nl02, dz, fmaf(kg.nl01, dy, kg.cx));
         const float Es = fmaf(kg.nD2 * dz, dz, (kg.nD1 * u1) * u1);
         float G[8];
-        if (!DIRECT) {
+        if (MODE == 0 || (MODE == 2 && !kg.direct)) {
             // the row is the parabola E(k) = E3 + (k - 3) Lf - A (k - 3)(k - 4):  G(k) = G3 rho^(k-3) c^((k-3)(k-4)/2).
             // The geometric part is chained here (7 FMUL); the key-and-k part, together with the x mask of the box,
             // sits in km[k] (per key, hoisted out of the row loop) — as in a3, where it sits in the staged weights.
@@ -92,13 +96,21 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
             const float rf = ex2b(Lf), rb = ex2b(-Lf);
             G[4] = G[3] * rf; G[5] = G[4] * rf; G[6] = G[5] * rf; G[7] = G[6] * rf;
             G[2] = G[3] * rb; G[1] = G[2] * rb; G[0] = G[1] * rb;
-            #pragma unroll
-            for (int k = 0; k < 8; ++k) G[k] *= km[k];
+            if (MODE == 0) {
+                #pragma unroll
+                for (int k = 0; k < 8; ++k) G[k] *= km[k];
+            }
         } else {
             #pragma unroll
             for (int k = 0; k < 8; ++k) { const float t = (float)k - xs; G[k] = ex2b(fmaf(kg.negA * t, t, Es)); }
+            if (MODE == 1) {
+                #pragma unroll
+                for (int k = 0; k < 8; ++k) G[k] = (kg.xm & (1u << k)) ? G[k] : 0.f;      // voxels outside the box in x
+            }
+        }
+        if (MODE == 2) {                                            // km: the chain's factors, or the bare x mask of a direct key
             #pragma unroll
-            for (int k = 0; k < 8; ++k) G[k] = (kg.xm & (1u << k)) ? G[k] : 0.f;      // voxels outside the box in x
+            for (int k = 0; k < 8; ++k) G[k] *= km[k];
         }
         // a_k = (sum_c g_c w_c) G_k  (w factored out when SINGLE)
         float av[8];
@@ -148,7 +160,7 @@ __device__ __forceinline__ void walk_rows(const KeyGeom& kg, uint32_t sbase, con
         }
         // x-moments about xs
         float U0, U1, U2;
-        if (!DIRECT) {
+        if (MODE == 0) {
             // about the brick-local index, then shifted (wide profile: mild cancellation only)
             U0 = av[0]; float S1 = 0.f, S2 = 0.f;
             #pragma unroll
@@ -247,9 +259,13 @@ __device__ __forceinline__ void backward_brick(const GsRec* __restrict__ rec, co
         #pragma unroll
         for (int ch = 0; ch < CH; ++ch) dw[ch] = 0.f;
 
-        // class 0 (direct) keys sit at the front of the brick's range: at most one warp mixes paths
-        if (kg.direct) walk_rows<CH, SINGLE, true>(kg, sbase, wv, m, dw);
-        else           walk_rows<CH, SINGLE, false>(kg, sbase, wv, m, dw);
+        // class 0 (direct) keys sit at the front of the brick's range: at most one warp of a brick holds both kinds
+        // (the loop over wbase has a warp-uniform trip count: whole warps arrive here)
+        const bool any_direct = __any_sync(0xffffffffu, kg.direct && kg.nrows > 0);
+        const bool any_chain = __any_sync(0xffffffffu, !kg.direct && kg.nrows > 0);
+        if (any_direct && any_chain) walk_rows<CH, SINGLE, 2>(kg, sbase, wv, m, dw);
+        else if (any_direct)         walk_rows<CH, SINGLE, 1>(kg, sbase, wv, m, dw);
+        else                         walk_rows<CH, SINGLE, 0>(kg, sbase, wv, m, dw);
 
         if (active) {
             float* dst = acc + (size_t)gid * astride;
